@@ -117,8 +117,8 @@ CONFIGS = [
     _cfg("cfg1_2x2_b2", 2, 2, 2.0, 4.0, 0.0, 1, 8, 1000, 200, 9, 64),
     _cfg("cfg2_2x2_b10", 2, 2, 10.0, 4.0, 0.0, 256, 16, 500, 0, 41, 128),
     _cfg("cfg3_4x4_b10", 4, 4, 10.0, 4.0, -0.054654, 64, 32, 200, 0, 159, 384),
-    _cfg("cfg4_6x6_b20", 6, 6, 20.0, 6.0, -0.037689, 8, 64, 100, 0, 1070, 2048),
-    _cfg("cfg5_6x6_b40", 6, 6, 40.0, 6.0, -0.009099, 2, 128, 50, 0, 2156, 4224),
+    _cfg("cfg4_6x6_b20", 6, 6, 20.0, 6.0, -0.037689, 8, 64, 100, 0, 1070, 2304),
+    _cfg("cfg5_6x6_b40", 6, 6, 40.0, 6.0, -0.009099, 2, 128, 50, 0, 2156, 4608),
 ]
 
 

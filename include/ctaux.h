@@ -1,0 +1,178 @@
+/* ctaux.h -- C ABI of the B200-native CT-AUX walker (libctaux_b200.so).
+ *
+ * The library runs the hot path of the continuous-time auxiliary-field QMC cluster solver of
+ * DCA++ (arXiv:1901.01047, section 2.3) for B independent Markov chains
+ * ("walkers") on ONE sm_100a device:
+ *
+ *   S1  G0 interpolation and construction of A_sigma = N_sigma^{-1}
+ *       (Eq. (27); BASELINE.json: N^-1 = e^{-gamma sigma V} - G0 (e^{-gamma sigma V} - 1))
+ *   S2  candidate products for the determinant ratios of a block of proposals
+ *   S3  Metropolis proposals (vertex insertion / removal) evaluated over the small
+ *       delayed block (submatrix updates)
+ *   S4  the delayed rank-r flush  N <- N - U S^{-1} V^T  as FP64 tensor-core (DMMA) GEMMs
+ *   S5  from-scratch rebuild  N = A^{-1}  by LU with partial pivoting
+ *
+ * Conventions (every reading of a point the paper leaves open is listed in DESIGN.md):
+ *   - No torch types, no C++ types, no exceptions cross this boundary.
+ *   - Every function returns 0 (CTAUX_OK) or a negative CTAUX_E* code; nothing aborts the process.
+ *   - The caller owns every buffer it passes in.  `g0_table` and `seeds` are HOST pointers and are
+ *     copied during the call.  `workspace` is a DEVICE pointer (e.g. a torch uint8 tensor) of at
+ *     least ctaux_workspace_bytes() bytes, 256-byte aligned, which must stay alive and untouched
+ *     until ctaux_destroy(); the context sub-allocates it and owns nothing else on the device.
+ *   - `stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); all kernels of
+ *     the context are launched on it.  ctaux_sweep returns when the requested sweeps are done
+ *     (it polls a completion flag, because the number of proposal blocks is data dependent);
+ *     every ctaux_get_* synchronises the stream before reading.
+ *   - Matrices handed out are column-major with the leading dimension the caller states, in the
+ *     order of the walker's vertex LIST (ascending vertex id).
+ *   - There is no CPU fallback: without a CUDA device every call returns CTAUX_ECUDA.
+ */
+#ifndef CTAUX_H_
+#define CTAUX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CTAUX_OK 0
+#define CTAUX_EINVAL (-1)     /* bad argument / inconsistent parameters                       */
+#define CTAUX_ECAPACITY (-2)  /* a walker would exceed max_k, or the workspace is too small   */
+#define CTAUX_ECUDA (-3)      /* CUDA runtime error (see ctaux_last_cuda_error)               */
+#define CTAUX_ESINGULAR (-4)  /* A_sigma numerically singular during a rebuild                */
+#define CTAUX_ESTATE (-5)     /* call not valid in this state (e.g. sweep before reset)       */
+
+typedef struct ctaux_ctx ctaux_ctx; /* opaque */
+
+/* Parameters of ctaux_create.  Names follow the paper's input file where one exists. */
+typedef struct ctaux_params {
+  int32_t Lx, Ly;          /* periodic cluster, Nc = Lx*Ly, site i = x + Lx*y      */
+  double beta;             /* inverse temperature                                      */
+  double U;                /* on-site Hubbard U; N_corr = Nc            */
+  double K;                /* CT-AUX expansion parameter K of Eq. (22)            */
+  int32_t n_tau;           /* M = number of tau INTERVALS (`sp-time-intervals`);
+                              the table has M+1 points per row                                        */
+  const double* g0_table;  /* HOST, [Nc][M+1] row-major, STANDARD sign (G0 < 0 at r=0 on (0,beta)),
+                              row d = displacement dx + Lx*dy, column m = tau_m = m*beta/M with
+                              m=0 meaning 0+ and m=M meaning beta-                                    */
+  int32_t delay;           /* max buffered ACCEPTED changes per block = rank of the flush
+                              (`max-submatrix-size`).  Performance knob only:
+                              the Markov chain does not depend on it.  1 <= delay <= 256             */
+  int32_t n_walkers;       /* B independent chains batched on the device               */
+  int32_t init_k;          /* random vertices drawn at reset (`initial-configuration-size`) */
+  int32_t max_k;           /* capacity of the vertex list; exceeding it is CTAUX_ECAPACITY
+                              (`initial-matrix-size` idea)                              */
+  int32_t rebuild_every;   /* sweeps between from-scratch rebuilds of N (0 = never). Chain-neutral.   */
+  int32_t log_capacity;    /* decision-log entries kept per walker (0 = logging off)                  */
+  int32_t cand_window;     /* insertion candidates pre-expanded per block (0 = library default,
+                              about 1.25*delay+8).  Performance knob only.                            */
+  void* workspace;         /* DEVICE pointer, caller-owned                                            */
+  size_t workspace_bytes;
+  void* stream;            /* cudaStream_t                                                            */
+} ctaux_params;
+
+/* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */
+typedef struct ctaux_stats {
+  uint64_t proposals;      /* proposal counter p of the chain (runs on across sweep calls)            */
+  uint64_t next_id;        /* id the next accepted insertion will get                                 */
+  int64_t acc_ins, acc_rem;/* accepted insertions / removals since reset                              */
+  int64_t sweeps;          /* sweeps completed since reset                                            */
+  int64_t blocks;          /* proposal blocks run                                                     */
+  int64_t flushes;         /* blocks that ended in a rank-r flush (r > 0)                             */
+  int64_t rebuilds;        /* from-scratch rebuilds                                                   */
+  int64_t sum_rank;        /* sum of r over flushes                                                   */
+  int32_t k;               /* current expansion order                                                 */
+  int32_t sign;            /* sign of prod_sigma det A_sigma carried along the chain                  */
+  double flops_cand;       /* S2: 2*m*k*k (rows) + 2*n*n*m (columns), both spins                      */
+  double flops_flush;      /* S4: 2*k'*k'*r + 2*k'*r*r, both spins                                    */
+  double flops_rebuild;    /* S5: 2*k^3 per spin                                                      */
+  double min_margin;       /* min over proposals of |u - |R|| / |R|  (near-tie diagnostic, Q22)       */
+  double sum_k;            /* sum over proposals of k before the proposal (for <k>)                   */
+} ctaux_stats;
+
+/* One entry of the decision log (48 bytes). */
+typedef struct ctaux_log_entry {
+  uint64_t p;              /* proposal counter                                                        */
+  int32_t type;            /* 0 insert, 1 remove                                                      */
+  int32_t arg;             /* insert: site; remove: list position j (-1 when k == 0)                  */
+  double tau;              /* insert: proposed tau; remove: 0                                         */
+  int32_t spin;            /* insert: proposed auxiliary spin; remove: 0                              */
+  int32_t accepted;        /* 1 iff u < |R|                                                           */
+  double R;                /* signed acceptance ratio: K/(k+1) or k/K times prod_sigma det A'/det A   */
+  double u;                /* the uniform it was compared with                                        */
+} ctaux_log_entry;
+
+/* Device bytes ctaux_create needs for these parameters (workspace fields ignored). 0 on bad input. */
+size_t ctaux_workspace_bytes(const ctaux_params* prm);
+
+/* Build a context: copies the table to the device, precomputes e^{+-gamma} (Eq. (25)),
+ * carves the workspace.  *out is NULL on failure. */
+int ctaux_create(const ctaux_params* prm, ctaux_ctx** out);
+
+/* (Re)start all walkers: walker w draws init_k vertices from Philox4x32-10 keyed by seeds[w]
+ * (HOST array of n_walkers), builds A_sigma and N_sigma = A_sigma^{-1} (S1 + S5), sets the proposal
+ * counter to 0. */
+int ctaux_reset(ctaux_ctx* ctx, const uint64_t* seeds);
+
+/* Start every walker from a given configuration instead (HOST arrays of n_walkers*max_k entries,
+ * walker w at offset w*max_k, k[w] live entries; ids ascending).  Used to resume a chain. */
+int ctaux_set_state(ctaux_ctx* ctx, const uint64_t* seeds, const int32_t* k, const uint64_t* id,
+                    const int32_t* site, const double* tau, const int8_t* spin,
+                    const uint64_t* next_id, const uint64_t* proposals);
+
+/* Advance every walker by n_sweeps sweeps; a sweep is max(16, k at sweep start) proposals
+ * (S2, S3, S4 per block; S5 every rebuild_every sweeps).  Continues each walker's stream. */
+int ctaux_sweep(ctaux_ctx* ctx, int32_t n_sweeps);
+
+/* From-scratch rebuild of every walker's N from its configuration (S1 + S5), now. */
+int ctaux_rebuild(ctaux_ctx* ctx);
+
+/* Configuration of one walker in list order into HOST arrays with room for `cap` entries.
+ * Any of id/site/tau/spin may be NULL. *k receives the expansion order. */
+int ctaux_get_config(ctaux_ctx* ctx, int32_t walker, int32_t* k, uint64_t* id, int32_t* site,
+                     double* tau, int8_t* spin, int32_t cap);
+
+/* N_sigma of one walker (spin 0 = up, 1 = down): k x k, column-major, leading dimension ld >= k,
+ * into a HOST buffer, rows/columns in list order.  This is the incrementally updated matrix. */
+int ctaux_get_N(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N, int32_t ld);
+
+/* Same matrix, copied device-to-device into a DEVICE buffer (no host staging). */
+int ctaux_get_N_device(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N_dev, int32_t ld);
+
+int ctaux_get_stats(ctaux_ctx* ctx, int32_t walker, ctaux_stats* out);
+
+/* Copy log entries [first, first+count) of one walker into a HOST array; entries are numbered from
+ * the last reset and the log keeps the first log_capacity of them. Returns the number copied (>=0). */
+int64_t ctaux_get_log(ctaux_ctx* ctx, int32_t walker, ctaux_log_entry* out, int64_t first, int64_t count);
+
+/* Kernel launches issued by this context since creation (bench.py's gpu_launches). */
+int64_t ctaux_launch_count(ctaux_ctx* ctx);
+
+/* Device time (ms, CUDA events on the context stream) spent in each step class since the last
+ * ctaux_timing_reset: [0] S1+S2 prep, [1] S2 GEMMs, [2] S3 proposal, [3] S4 U/V build,
+ * [4] S4 flush GEMMs, [5] S5 rebuild, [6] other.  Only filled when timing is enabled (it
+ * serialises launches with events; off by default). */
+int ctaux_timing_enable(ctaux_ctx* ctx, int32_t on);
+int ctaux_timing_get(ctaux_ctx* ctx, double* ms /*[8]*/, int64_t* launches /*[8]*/);
+
+void ctaux_destroy(ctaux_ctx* ctx);
+
+const char* ctaux_strerror(int code);
+const char* ctaux_last_cuda_error(void);
+
+/* Stand-alone FP64 GEMM through the library's DMMA tile kernel (the kernel S2/S4/S5 use):
+ * C (MxN, ldc) = beta*C + alpha * A (MxK, lda) * B (KxN, ldb), all column-major DEVICE pointers.
+ * For measurement and tests. */
+int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
+                int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc);
+
+/* Debug / pin helper: Philox4x32-10 evaluated ON THE DEVICE for n (counter, key) pairs.
+ * ctr: HOST [n][4], key: HOST [n][2], out: HOST [n][4]. */
+int ctaux_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int32_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CTAUX_H_ */

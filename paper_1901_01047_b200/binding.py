@@ -1,0 +1,284 @@
+"""ctypes binding of include/ctaux.h.  Same names as the C ABI; marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+LOG_DTYPE = np.dtype([("p", "<u8"), ("type", "<i4"), ("arg", "<i4"), ("tau", "<f8"),
+                      ("spin", "<i4"), ("accepted", "<i4"), ("R", "<f8"), ("u", "<f8")])
+
+STEP_CLASSES = ["prep", "cand_gemm", "propose", "build_uv", "flush_gemm", "rebuild", "other", "usinv_gemm"]
+
+
+class CtauxError(RuntimeError):
+    def __init__(self, code, what, detail=""):
+        super().__init__(f"{what}: code {code} ({detail})")
+        self.code = code
+
+
+class _Params(C.Structure):
+    _fields_ = [("Lx", C.c_int32), ("Ly", C.c_int32), ("beta", C.c_double), ("U", C.c_double),
+                ("K", C.c_double), ("n_tau", C.c_int32), ("g0_table", C.c_void_p),
+                ("delay", C.c_int32), ("n_walkers", C.c_int32), ("init_k", C.c_int32),
+                ("max_k", C.c_int32), ("rebuild_every", C.c_int32), ("log_capacity", C.c_int32),
+                ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("stream", C.c_void_p)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("proposals", C.c_uint64), ("next_id", C.c_uint64), ("acc_ins", C.c_int64),
+                ("acc_rem", C.c_int64), ("sweeps", C.c_int64), ("blocks", C.c_int64),
+                ("flushes", C.c_int64), ("rebuilds", C.c_int64), ("sum_rank", C.c_int64),
+                ("k", C.c_int32), ("sign", C.c_int32), ("flops_cand", C.c_double),
+                ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
+                ("min_margin", C.c_double), ("sum_k", C.c_double)]
+
+
+EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
+           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_N", "ctaux_get_N_device", "ctaux_get_stats",
+           "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
+           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_debug_philox"]
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB_PATH
+
+
+def load_library():
+    """Load libctaux_b200.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    if not os.path.exists(path):
+        raise CtauxError(-3, "libctaux_b200.so missing", path)
+    L = C.CDLL(path)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.ctaux_workspace_bytes.restype = C.c_size_t
+    L.ctaux_workspace_bytes.argtypes = [C.POINTER(_Params)]
+    L.ctaux_create.argtypes = [C.POINTER(_Params), C.POINTER(vp)]
+    L.ctaux_reset.argtypes = [vp, vp]
+    L.ctaux_set_state.argtypes = [vp] + [vp] * 8
+    L.ctaux_sweep.argtypes = [vp, i32]
+    L.ctaux_rebuild.argtypes = [vp]
+    L.ctaux_get_config.argtypes = [vp, i32, C.POINTER(i32), vp, vp, vp, vp, i32]
+    L.ctaux_get_N.argtypes = [vp, i32, i32, vp, i32]
+    L.ctaux_get_N_device.argtypes = [vp, i32, i32, vp, i32]
+    L.ctaux_get_stats.argtypes = [vp, i32, C.POINTER(_Stats)]
+    L.ctaux_get_log.restype = i64
+    L.ctaux_get_log.argtypes = [vp, i32, vp, i64, i64]
+    L.ctaux_launch_count.restype = i64
+    L.ctaux_launch_count.argtypes = [vp]
+    L.ctaux_timing_enable.argtypes = [vp, i32]
+    L.ctaux_timing_get.argtypes = [vp, vp, vp]
+    L.ctaux_destroy.restype = None
+    L.ctaux_destroy.argtypes = [vp]
+    L.ctaux_strerror.restype = C.c_char_p
+    L.ctaux_strerror.argtypes = [C.c_int]
+    L.ctaux_last_cuda_error.restype = C.c_char_p
+    L.ctaux_dgemm.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32]
+    L.ctaux_debug_philox.argtypes = [vp, vp, vp, i32]
+    _lib = L
+    return L
+
+
+def exported_symbols():
+    L = load_library()
+    return {name: hasattr(L, name) for name in EXPORTS}
+
+
+def _check(rc, what):
+    if rc != 0:
+        L = load_library()
+        detail = L.ctaux_strerror(rc).decode()
+        if rc == -3:
+            detail += ": " + L.ctaux_last_cuda_error().decode()
+        raise CtauxError(rc, what, detail)
+
+
+class Walkers:
+    """B batched CT-AUX walkers on one GPU (ctaux_create / reset / sweep / get_*)."""
+
+    def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
+                 rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
+        self._torch = torch
+        self._L = load_library()
+        self.device = torch.device(device)
+        table = np.ascontiguousarray(g0_table, dtype=np.float64)
+        assert table.shape == (Lx * Ly, table.shape[1])
+        self._table = table
+        self.n_walkers, self.max_k = n_walkers, max_k
+        p = _Params()
+        p.Lx, p.Ly, p.beta, p.U, p.K = Lx, Ly, beta, U, K
+        p.n_tau = table.shape[1] - 1
+        p.g0_table = table.ctypes.data
+        p.delay, p.n_walkers, p.init_k, p.max_k = delay, n_walkers, init_k, max_k
+        p.rebuild_every, p.log_capacity, p.cand_window = rebuild_every, log_capacity, cand_window
+        nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
+        if nbytes == 0:
+            raise CtauxError(-1, "ctaux_workspace_bytes", "invalid parameters")
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        p.workspace = self._ws.data_ptr()
+        p.workspace_bytes = nbytes
+        p.stream = self._stream.cuda_stream
+        self.workspace_bytes = nbytes
+        self._params = p
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            _check(self._L.ctaux_create(C.byref(p), C.byref(h)), "ctaux_create")
+        self._h = h
+
+    @classmethod
+    def from_config(cls, cfg, table, n_walkers=None, **kw):
+        args = dict(delay=cfg["delay"], n_walkers=n_walkers or cfg["n_walkers"], init_k=cfg["init_k"],
+                    max_k=cfg["max_k"], rebuild_every=cfg["rebuild_every"])
+        args.update(kw)
+        return cls(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table, **args)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.ctaux_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    __del__ = close
+
+    def reset(self, seeds):
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        assert seeds.size == self.n_walkers
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_reset(self._h, seeds.ctypes.data), "ctaux_reset")
+
+    def set_state(self, seeds, configs, next_id, proposals):
+        """configs: list (per walker) of dicts with id/site/tau/spin arrays in list order."""
+        B, mk = self.n_walkers, self.max_k
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        k = np.array([len(c["site"]) for c in configs], dtype=np.int32)
+        ids = np.zeros((B, mk), np.uint64)
+        site = np.zeros((B, mk), np.int32)
+        tau = np.zeros((B, mk), np.float64)
+        spin = np.zeros((B, mk), np.int8)
+        for w, c in enumerate(configs):
+            ids[w, :k[w]] = c["id"]
+            site[w, :k[w]] = c["site"]
+            tau[w, :k[w]] = c["tau"]
+            spin[w, :k[w]] = c["spin"]
+        next_id = np.ascontiguousarray(next_id, dtype=np.uint64)
+        proposals = np.ascontiguousarray(proposals, dtype=np.uint64)
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_set_state(self._h, seeds.ctypes.data, k.ctypes.data, ids.ctypes.data,
+                                           site.ctypes.data, tau.ctypes.data, spin.ctypes.data,
+                                           next_id.ctypes.data, proposals.ctypes.data), "ctaux_set_state")
+
+    def sweep(self, n_sweeps):
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_sweep(self._h, int(n_sweeps)), "ctaux_sweep")
+
+    def rebuild(self):
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_rebuild(self._h), "ctaux_rebuild")
+
+    def get_config(self, w):
+        k = C.c_int32(0)
+        mk = self.max_k
+        ids, site = np.zeros(mk, np.uint64), np.zeros(mk, np.int32)
+        tau, spin = np.zeros(mk, np.float64), np.zeros(mk, np.int8)
+        _check(self._L.ctaux_get_config(self._h, w, C.byref(k), ids.ctypes.data, site.ctypes.data,
+                                        tau.ctypes.data, spin.ctypes.data, mk), "ctaux_get_config")
+        n = k.value
+        return dict(id=ids[:n].copy(), site=site[:n].copy(), tau=tau[:n].copy(), spin=spin[:n].copy())
+
+    def get_N(self, w, spin):
+        """k x k numpy array (row index = first index), list order."""
+        st = self.get_stats(w)
+        k = st["k"]
+        buf = np.zeros((k, k), np.float64, order="F")
+        if k:
+            _check(self._L.ctaux_get_N(self._h, w, spin, buf.ctypes.data, k), "ctaux_get_N")
+        return np.ascontiguousarray(buf)
+
+    def get_N_device(self, w, spin):
+        torch = self._torch
+        k = self.get_stats(w)["k"]
+        out = torch.empty((k, k), dtype=torch.float64, device=self.device)  # holds N^T in C order
+        if k:
+            _check(self._L.ctaux_get_N_device(self._h, w, spin, out.data_ptr(), k), "ctaux_get_N_device")
+        return out.t()
+
+    def get_stats(self, w):
+        s = _Stats()
+        _check(self._L.ctaux_get_stats(self._h, w, C.byref(s)), "ctaux_get_stats")
+        return {f: getattr(s, f) for f, _ in _Stats._fields_}
+
+    def get_log(self, w, first=0, count=None):
+        if count is None:
+            count = self._params.log_capacity
+        out = np.zeros(max(count, 0), LOG_DTYPE)
+        n = self._L.ctaux_get_log(self._h, w, out.ctypes.data, first, count) if count > 0 else 0
+        if n < 0:
+            _check(int(n), "ctaux_get_log")
+        return out[:n]
+
+    def launch_count(self):
+        return self._L.ctaux_launch_count(self._h)
+
+    def timing_enable(self, on=True):
+        _check(self._L.ctaux_timing_enable(self._h, 1 if on else 0), "ctaux_timing_enable")
+
+    def timing_get(self):
+        ms = np.zeros(8, np.float64)
+        nl = np.zeros(8, np.int64)
+        _check(self._L.ctaux_timing_get(self._h, ms.ctypes.data, nl.ctypes.data), "ctaux_timing_get")
+        return {name: dict(ms=float(ms[i]), launches=int(nl[i])) for i, name in enumerate(STEP_CLASSES)}
+
+
+def colmajor(rows, cols, device="cuda", fill=None, generator=None):
+    """A rows x cols float64 CUDA tensor stored column-major with an EVEN leading dimension
+    (the layout ctaux_dgemm wants): element (i, j) at data_ptr + 8*(i + j*ld)."""
+    import torch
+    ld = max(2, rows + (rows & 1))
+    if fill is None:
+        store = torch.zeros((cols, ld), dtype=torch.float64, device=device)
+    else:
+        store = fill(cols, ld).to(device)
+    return store[:, :rows].t()
+
+
+def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None):
+    """C = beta*C + alpha*A@B through the library's DMMA tile kernel.  A (M x K), B (K x N), C (M x N)
+    are torch float64 CUDA tensors stored column-major (stride(0) == 1) with even leading dimensions
+    (see colmajor())."""
+    import torch
+    L = load_library()
+    M, K = A.shape
+    K2, N = B.shape
+    assert K == K2 and A.dtype == torch.float64 and B.dtype == torch.float64
+    if C_out is None:
+        C_out = colmajor(M, N, A.device)
+    for t in (A, B, C_out):
+        assert t.shape[0] <= 1 or t.stride(0) == 1, "column-major operands required"
+    ld = lambda t: int(t.stride(1)) if t.shape[1] > 1 else max(2, t.shape[0] + (t.shape[0] & 1))
+    s = stream if stream is not None else torch.cuda.current_stream(A.device)
+    _check(L.ctaux_dgemm(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
+                         C_out.data_ptr(), ld(C_out)), "ctaux_dgemm")
+    return C_out
+
+
+def debug_philox(ctr, key):
+    L = load_library()
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    out = np.zeros_like(ctr)
+    _check(L.ctaux_debug_philox(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, ctr.shape[0]), "ctaux_debug_philox")
+    return out

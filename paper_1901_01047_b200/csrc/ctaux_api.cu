@@ -1,0 +1,718 @@
+// C ABI of the B200-native CT-AUX walker: host-side orchestration (include/ctaux.h).
+// Every step of the path runs in the kernels of walker_kernels.cuh / gemm_dmma.cuh; the host
+// only enqueues launches and polls the completion flag.
+#include "../../include/ctaux.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "gemm_dmma.cuh"
+#include "rebuild_lu.cuh"
+#include "walker_kernels.cuh"
+
+using namespace ctaux;
+
+static_assert(sizeof(LogEntry) == sizeof(ctaux_log_entry), "log entry layout");
+
+namespace {
+
+thread_local std::string g_last_cuda_error;
+
+#define CU_CHECK(expr)                                                             \
+  do {                                                                             \
+    cudaError_t _e = (expr);                                                       \
+    if (_e != cudaSuccess) {                                                       \
+      g_last_cuda_error = std::string(#expr) + ": " + cudaGetErrorString(_e);      \
+      return CTAUX_ECUDA;                                                          \
+    }                                                                              \
+  } while (0)
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+enum StepClass { C_PREP = 0, C_CAND_GEMM = 1, C_PROPOSE = 2, C_UV = 3, C_FLUSH_GEMM = 4, C_REBUILD = 5, C_OTHER = 6, C_USINV_GEMM = 7, N_CLASS = 8 };
+
+// GEMM tile configurations
+//  big:   128x128x16, 8 warps (2x4), 4 stages  -- flush / candidate columns at large k
+//  small:  64x64x16,  4 warps... (kept at 8 warps: 2x4 -> warp tile 32x16)
+#define GEMM_BIG 128, 128, 2, 4, 4
+#define GEMM_SMALL 64, 64, 2, 4, 4
+
+// ---- device-side problem descriptors ------------------------------------------------------
+struct DescCandRows {  // G1: N_ext[k:k+m, 0:k] = Bm (m x k) * N (k x k)
+  DevCtx c;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0 || st.k == 0) return false;
+    double* N = c.N(w, sp, st.n_cur);
+    d.M = st.m; d.N = st.k; d.K = st.k;
+    d.A = c.Bm + ((size_t)w * 2 + sp) * (size_t)c.ldm * c.cap; d.lda = c.ldm;
+    d.B = N; d.ldb = c.ld;
+    d.C = N + st.k; d.ldc = c.ld;
+    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = 1.0; d.beta = 0.0;
+    return true;
+  }
+};
+struct DescCandCols {  // G2: Gx (n x m) = N_ext (n x n) * gxC (n x m)
+  DevCtx c;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0) return false;
+    const int n = st.k + st.m;
+    d.M = n; d.N = st.m; d.K = n;
+    d.A = c.N(w, sp, st.n_cur); d.lda = c.ld;
+    d.B = c.gxC + (size_t)w * c.ld * c.mmax; d.ldb = c.ld;
+    d.C = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax; d.ldc = c.ld;
+    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = 1.0; d.beta = 0.0;
+    return true;
+  }
+};
+struct DescUSinv {  // G3: Ut (k' x r) = U (k' x r) * S^-1 (r x r)
+  DevCtx c;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.r == 0) return false;
+    d.M = st.k_new; d.N = st.r; d.K = st.r;
+    d.A = c.Um + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.lda = c.ld;
+    d.B = c.Sinv + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.delay; d.ldb = c.ldr;
+    d.C = c.Ut + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.ldc = c.ld;
+    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = 1.0; d.beta = 0.0;
+    return true;
+  }
+};
+struct DescFlush {  // G4: N_new[i',j'] = N_ext[map i', map j'] - (Ut * Vt)[i',j']
+  DevCtx c;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.r == 0) return false;
+    d.M = st.k_new; d.N = st.k_new; d.K = st.r;
+    d.A = c.Ut + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.lda = c.ld;
+    d.B = c.Vt + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.ld; d.ldb = c.ldr;
+    d.C = c.N(w, sp, st.n_cur); d.ldc = c.ld;
+    d.C0 = c.N(w, sp, st.n_src); d.ldc0 = c.ld;
+    d.rowmap = c.rowmap + (size_t)w * c.cap; d.colmap = d.rowmap;
+    d.alpha = -1.0; d.beta = 1.0;
+    return true;
+  }
+};
+struct DescPlain {  // ctaux_dgemm
+  GemmDesc d;
+  __device__ bool operator()(int, GemmDesc& o) const { o = d; return true; }
+};
+
+template <int BM, int BN, int WM, int WN, int STAGES, class Fn>
+cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s) {
+  using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
+  auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, Fn>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  if (tiles_x < 1) tiles_x = 1;
+  kern<<<dim3(tiles_x, problems), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(fn);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+struct ctaux_ctx {
+  ctaux_params prm;
+  DevCtx d;
+  cudaStream_t stream;
+  int* detsign;       // device [B*2]
+  uint64_t* seeds_d;  // device [B]
+  int* host_flag;     // pinned [2]
+  bool have_state;
+  int sweeps_since_rebuild;
+  int64_t launches;
+  bool sinv_smem;
+  int propose_smem;
+  bool small_tiles;
+  // timing
+  bool timing;
+  std::vector<cudaEvent_t> ev_pool;
+  std::vector<int> ev_class;
+  size_t ev_used;
+  double ms[N_CLASS];
+  int64_t nl[N_CLASS];
+};
+
+namespace {
+
+struct Layout {
+  size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, total;
+};
+
+bool derive_sizes(const ctaux_params* p, DevCtx& d) {
+  if (!p || p->Lx < 1 || p->Ly < 1 || p->n_tau < 1 || p->delay < 1 || p->delay > kMaxDelay ||
+      p->n_walkers < 1 || p->max_k < 1 || p->init_k < 0 || p->init_k > p->max_k || !(p->beta > 0) ||
+      !(p->K > 0) || p->U < 0 || p->rebuild_every < 0 || p->log_capacity < 0 || p->cand_window < 0)
+    return false;
+  memset(&d, 0, sizeof(d));
+  d.B = p->n_walkers; d.Lx = p->Lx; d.Ly = p->Ly; d.Nc = p->Lx * p->Ly; d.M = p->n_tau;
+  d.max_k = p->max_k; d.delay = p->delay;
+  int mmax = p->cand_window > 0 ? p->cand_window : (p->delay + p->delay / 4 + 8);
+  if (mmax > 480) mmax = 480;
+  d.mmax = mmax;
+  int winmax = 3 * mmax + 16;
+  if (winmax > 1024) winmax = 1024;
+  d.winmax = winmax;
+  d.cap = p->max_k + mmax;
+  if (d.cap > 8192) return false;
+  d.ld = round_up(d.cap, 8);
+  d.ldm = round_up(mmax, 8);
+  d.ldr = round_up(p->delay, 8);
+  d.log_capacity = p->log_capacity;
+  d.beta = p->beta; d.K = p->K; d.tau_scale = (double)p->n_tau / p->beta;
+  // Eq. (25): cosh(gamma) = 1 + U beta Ncorr / (2K)
+  const double ch = 1.0 + p->U * p->beta * (double)d.Nc / (2.0 * p->K);
+  d.egp = ch + sqrt(ch * ch - 1.0);
+  d.egm = 1.0 / d.egp;
+  return true;
+}
+
+Layout make_layout(const DevCtx& d) {
+  Layout L;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
+  const size_t B = d.B;
+  L.table = take((size_t)d.Nc * (d.M + 1) * 8);
+  L.ws = take(B * sizeof(WalkerState));
+  L.cfg_site = take(B * 2 * d.cap * 4);
+  L.cfg_tau = take(B * 2 * d.cap * 8);
+  L.cfg_spin = take(B * 2 * d.cap * 4);
+  L.cfg_id = take(B * 2 * d.cap * 8);
+  L.prop = take(B * d.winmax * sizeof(PropInfo));
+  L.Nbuf = take(B * 4 * (size_t)d.ld * d.ld * 8);
+  L.Bm = take(B * 2 * (size_t)d.ldm * d.cap * 8);
+  L.gxC = take(B * (size_t)d.ld * d.mmax * 8);
+  L.Gx = take(B * 2 * (size_t)d.ld * d.mmax * 8);
+  L.Um = take(B * 2 * (size_t)d.ld * d.delay * 8);
+  L.Ut = take(B * 2 * (size_t)d.ld * d.delay * 8);
+  L.Vt = take(B * 2 * (size_t)d.ldr * d.ld * 8);
+  L.Sinv = take(B * 2 * (size_t)d.ldr * d.delay * 8);
+  L.J = take(B * d.delay * 4);
+  L.rowmap = take(B * d.cap * 4);
+  L.log = take(B * (size_t)d.log_capacity * sizeof(LogEntry));
+  L.n_active = take(256);
+  L.colbuf = take(B * 2 * d.ld * 8);
+  L.rowbuf = take(B * 2 * d.ld * 8);
+  L.perm = take(B * 2 * d.ld * 4);
+  L.detsign = take(B * 2 * 4);
+  L.seeds = take(B * 8);
+  L.total = o;
+  return L;
+}
+
+// ---- timing helpers ------------------------------------------------------------------------
+void tick(ctaux_ctx* x, int cls) {
+  x->launches++;
+  x->nl[cls]++;
+}
+struct Scoped {
+  ctaux_ctx* x;
+  int cls;
+  size_t idx;
+  Scoped(ctaux_ctx* x_, int cls_) : x(x_), cls(cls_), idx(0) {
+    if (!x->timing) return;
+    if (x->ev_used + 2 > x->ev_pool.size()) {
+      for (int i = 0; i < 2; ++i) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        x->ev_pool.push_back(e);
+      }
+      x->ev_class.push_back(cls);
+    }
+    idx = x->ev_used;
+    x->ev_class[idx / 2] = cls;
+    x->ev_used += 2;
+    cudaEventRecord(x->ev_pool[idx], x->stream);
+  }
+  ~Scoped() {
+    if (!x->timing) return;
+    cudaEventRecord(x->ev_pool[idx + 1], x->stream);
+  }
+};
+void harvest_timing(ctaux_ctx* x) {  // call after a stream synchronise
+  if (!x->timing) return;
+  for (size_t i = 0; i + 1 < x->ev_used; i += 2) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, x->ev_pool[i], x->ev_pool[i + 1]) == cudaSuccess) x->ms[x->ev_class[i / 2]] += ms;
+  }
+  x->ev_used = 0;
+}
+
+int grid_for(size_t work, int threads, int cap_blocks = 4096) {
+  size_t b = (work + threads - 1) / threads;
+  if (b < 1) b = 1;
+  if (b > (size_t)cap_blocks) b = cap_blocks;
+  return (int)b;
+}
+
+// S5: from-scratch inverse of every walker's A (current configuration) into the current N buffer
+int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  // expansion orders are on the device: fetch the maximum (rebuilds are rare)
+  std::vector<WalkerState> h(d.B);
+  CU_CHECK(cudaMemcpyAsync(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(cudaStreamSynchronize(s));
+  harvest_timing(x);
+  int kmax = 0;
+  for (int w = 0; w < d.B; ++w) kmax = h[w].k > kmax ? h[w].k : kmax;
+  if (set_sign) {
+    std::vector<int> ones(d.B * 2, 1);
+    CU_CHECK(cudaMemcpyAsync(x->detsign, ones.data(), sizeof(int) * d.B * 2, cudaMemcpyHostToDevice, s));
+    CU_CHECK(cudaStreamSynchronize(s));
+  }
+  if (kmax > 0) {
+    const int P = d.B * 2;
+    const int pthreads = kmax >= 1024 ? 1024 : (kmax >= 256 ? 512 : 128);
+    {
+      Scoped t(x, C_REBUILD);
+      const int gb = grid_for((size_t)kmax * kmax, 256, 1024);
+      k_build_A<<<dim3(gb, P), 256, 0, s>>>(d, 1);
+      k_lu_init_identity<<<dim3(gb, P), 256, 0, s>>>(d);
+      tick(x, C_REBUILD); tick(x, C_REBUILD);
+    }
+    const int cb = grid_for((size_t)2 * kmax, 128, 64);
+    auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
+      if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
+      tick(x, C_REBUILD);
+      if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
+      return launch_gemm<GEMM_BIG>(DescLU{d, j0, which}, ((Mmax + 127) / 128) * ((Nmax + 127) / 128), P, s);
+    };
+    for (int j0 = 0; j0 < kmax; j0 += kLuNb) {  // factorisation + forward substitution
+      Scoped t(x, C_REBUILD);
+      const int j1 = j0 + kLuNb < kmax ? j0 + kLuNb : kmax;
+      k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, set_sign ? x->detsign : nullptr);
+      k_lu_swap<<<dim3(cb, P), 128, 0, s>>>(d, j0);
+      k_lu_trsm<<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
+      tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
+      CU_CHECK(trailing(j0, 0, kmax - j1, kmax - j1));
+      CU_CHECK(trailing(j0, 1, kmax - j1, kmax));
+    }
+    for (int j0 = (kmax - 1) / kLuNb * kLuNb; j0 >= 0; j0 -= kLuNb) {  // backward substitution
+      Scoped t(x, C_REBUILD);
+      k_lu_trsm<<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
+      tick(x, C_REBUILD);
+      CU_CHECK(trailing(j0, 2, j0, kmax));
+    }
+  }
+  if (set_sign) { k_set_sign_from_det<<<(d.B + 127) / 128, 128, 0, s>>>(d, x->detsign); tick(x, C_OTHER); }
+  if (count) { k_count_rebuild<<<(d.B + 127) / 128, 128, 0, s>>>(d); tick(x, C_OTHER); }
+  CU_CHECK(cudaGetLastError());
+  CU_CHECK(cudaStreamSynchronize(s));
+  harvest_timing(x);
+  // singular?
+  CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+  for (int w = 0; w < d.B; ++w)
+    if (h[w].status) return h[w].status;
+  return CTAUX_OK;
+}
+
+// one block step for all walkers: S1/S2 prep, S2 GEMMs, S3 proposals, S4 flush
+int enqueue_block_step(ctaux_ctx* x) {
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  const int P = d.B * 2;
+  {
+    Scoped t(x, C_PREP);
+    k_prep_window<<<d.B, 1024, 0, s>>>(d);
+    k_prep_fill<<<dim3(grid_for((size_t)d.cap * d.mmax, 256, 256), d.B), 256, 0, s>>>(d);
+    tick(x, C_PREP); tick(x, C_PREP);
+  }
+  {
+    Scoped t(x, C_CAND_GEMM);
+    cudaError_t e1, e2;
+    if (x->small_tiles) {
+      e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
+      e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
+    } else {
+      e1 = launch_gemm<GEMM_BIG>(DescCandRows{d}, (d.mmax + 127) / 128 * ((d.max_k + 127) / 128), P, s);
+      e2 = launch_gemm<GEMM_BIG>(DescCandCols{d}, (d.cap + 127) / 128 * ((d.mmax + 127) / 128), P, s);
+    }
+    CU_CHECK(e1); CU_CHECK(e2);
+    tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
+  }
+  {
+    Scoped t(x, C_PROPOSE);
+    k_propose<<<d.B, kPropThreads, x->propose_smem, s>>>(d, x->sinv_smem ? 1 : 0);
+    tick(x, C_PROPOSE);
+  }
+  {
+    Scoped t(x, C_UV);
+    k_build_uv<<<dim3(grid_for((size_t)d.max_k * d.delay, 256, 512), P), 256, 0, s>>>(d);
+    tick(x, C_UV);
+  }
+  {
+    Scoped t(x, C_USINV_GEMM);
+    cudaError_t e3;
+    if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    else e3 = launch_gemm<GEMM_BIG>(DescUSinv{d}, (d.max_k + 127) / 128 * ((d.delay + 127) / 128), P, s);
+    CU_CHECK(e3);
+    tick(x, C_USINV_GEMM);
+  }
+  {
+    Scoped t(x, C_FLUSH_GEMM);
+    cudaError_t e4;
+    if (x->small_tiles) {
+      const int tl = (d.max_k + 63) / 64;
+      e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
+    } else {
+      const int tl = (d.max_k + 127) / 128;
+      e4 = launch_gemm<GEMM_BIG>(DescFlush{d}, tl * tl, P, s);
+    }
+    CU_CHECK(e4);
+    tick(x, C_FLUSH_GEMM);
+  }
+  CU_CHECK(cudaGetLastError());
+  return CTAUX_OK;
+}
+
+int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  k_begin_sweeps<<<(d.B + 127) / 128, 128, 0, s>>>(d, n_sweeps);
+  tick(x, C_OTHER);
+  const int steps_per_poll = 8;
+  // every block consumes at least one proposal and a sweep has at most max(16, max_k) of them
+  const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + steps_per_poll;
+  for (long long done = 0;; done += steps_per_poll) {
+    if (done > max_steps) return CTAUX_ESTATE;
+    for (int i = 0; i < steps_per_poll; ++i) {
+      int rc = enqueue_block_step(x);
+      if (rc) return rc;
+    }
+    CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(cudaStreamSynchronize(s));
+    harvest_timing(x);
+    if (x->host_flag[0] <= 0) break;
+  }
+  // errors raised inside kernels
+  std::vector<WalkerState> h(d.B);
+  CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+  for (int w = 0; w < d.B; ++w)
+    if (h[w].status) return h[w].status;
+  return CTAUX_OK;
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+extern "C" {
+
+const char* ctaux_strerror(int code) {
+  switch (code) {
+    case CTAUX_OK: return "ok";
+    case CTAUX_EINVAL: return "invalid argument";
+    case CTAUX_ECAPACITY: return "capacity exceeded (max_k or workspace)";
+    case CTAUX_ECUDA: return "CUDA error";
+    case CTAUX_ESINGULAR: return "singular matrix in rebuild";
+    case CTAUX_ESTATE: return "invalid state for this call";
+    default: return "unknown error";
+  }
+}
+const char* ctaux_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+size_t ctaux_workspace_bytes(const ctaux_params* prm) {
+  DevCtx d;
+  if (!derive_sizes(prm, d)) return 0;
+  return make_layout(d).total;
+}
+
+int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
+  if (out) *out = nullptr;
+  DevCtx d;
+  if (!out || !derive_sizes(prm, d) || !prm->g0_table || !prm->workspace) return CTAUX_EINVAL;
+  if (((uintptr_t)prm->workspace & 255) != 0) return CTAUX_EINVAL;
+  int ndev = 0;
+  CU_CHECK(cudaGetDeviceCount(&ndev));
+  if (ndev == 0) { g_last_cuda_error = "no CUDA device"; return CTAUX_ECUDA; }
+  const Layout L = make_layout(d);
+  if (prm->workspace_bytes < L.total) return CTAUX_ECAPACITY;
+  ctaux_ctx* x = new ctaux_ctx();
+  x->prm = *prm;
+  x->stream = (cudaStream_t)prm->stream;
+  char* base = (char*)prm->workspace;
+  d.table = (const double*)(base + L.table);
+  d.ws = (WalkerState*)(base + L.ws);
+  d.cfg_site = (int32_t*)(base + L.cfg_site); d.cfg_tau = (double*)(base + L.cfg_tau);
+  d.cfg_spin = (int32_t*)(base + L.cfg_spin); d.cfg_id = (uint64_t*)(base + L.cfg_id);
+  d.prop = (PropInfo*)(base + L.prop);
+  d.Nbuf = (double*)(base + L.Nbuf); d.Bm = (double*)(base + L.Bm); d.gxC = (double*)(base + L.gxC);
+  d.Gx = (double*)(base + L.Gx); d.Um = (double*)(base + L.Um); d.Ut = (double*)(base + L.Ut);
+  d.Vt = (double*)(base + L.Vt); d.Sinv = (double*)(base + L.Sinv);
+  d.J = (int32_t*)(base + L.J); d.rowmap = (int32_t*)(base + L.rowmap);
+  d.log = (LogEntry*)(base + L.log); d.n_active = (int32_t*)(base + L.n_active);
+  d.colbuf = (double*)(base + L.colbuf); d.rowbuf = (double*)(base + L.rowbuf); d.perm = (int32_t*)(base + L.perm);
+  x->detsign = (int*)(base + L.detsign);
+  x->seeds_d = (uint64_t*)(base + L.seeds);
+  d.g00 = -prm->g0_table[0];
+  x->d = d;
+  x->have_state = false;
+  x->sweeps_since_rebuild = 0;
+  x->launches = 0;
+  x->timing = false;
+  x->ev_used = 0;
+  memset(x->ms, 0, sizeof(x->ms));
+  memset(x->nl, 0, sizeof(x->nl));
+  x->host_flag = nullptr;
+  cudaError_t e = cudaMemsetAsync(base, 0, L.total, x->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void*)d.table, prm->g0_table, (size_t)d.Nc * (d.M + 1) * 8, cudaMemcpyHostToDevice, x->stream);
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_flag, 2 * sizeof(int));
+  if (e == cudaSuccess) e = cudaStreamSynchronize(x->stream);
+  // proposal kernel shared memory: keep S^-1 of both spins in shared memory when it fits
+  int dev = 0, max_smem = 0;
+  if (e == cudaSuccess) e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e == cudaSuccess) {
+    ProposeSmem Ls = propose_smem_layout(d.cap, d.delay, d.winmax, true);
+    x->sinv_smem = Ls.total <= max_smem;
+    if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
+    x->propose_smem = Ls.total;
+    if (Ls.total > max_smem) { delete x; return CTAUX_ECAPACITY; }
+    static int propose_attr_max = 0;  // the attribute is per function, shared by all contexts
+    if (Ls.total > propose_attr_max) {
+      e = cudaFuncSetAttribute(k_propose, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total);
+      if (e == cudaSuccess) propose_attr_max = Ls.total;
+    }
+  }
+  if (e != cudaSuccess) {
+    g_last_cuda_error = std::string("ctaux_create: ") + cudaGetErrorString(e);
+    if (x->host_flag) cudaFreeHost(x->host_flag);
+    delete x;
+    return CTAUX_ECUDA;
+  }
+  x->small_tiles = d.max_k <= 512;
+  *out = x;
+  return CTAUX_OK;
+}
+
+void ctaux_destroy(ctaux_ctx* x) {
+  if (!x) return;
+  cudaStreamSynchronize(x->stream);
+  for (cudaEvent_t e : x->ev_pool) cudaEventDestroy(e);
+  if (x->host_flag) cudaFreeHost(x->host_flag);
+  delete x;
+}
+
+int ctaux_reset(ctaux_ctx* x, const uint64_t* seeds) {
+  if (!x || !seeds) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  CU_CHECK(cudaMemcpyAsync(x->seeds_d, seeds, sizeof(uint64_t) * d.B, cudaMemcpyHostToDevice, x->stream));
+  k_init_config<<<d.B, 128, 0, x->stream>>>(d, x->seeds_d, x->prm.init_k);
+  tick(x, C_OTHER);
+  CU_CHECK(cudaGetLastError());
+  x->sweeps_since_rebuild = 0;
+  int rc = do_rebuild(x, /*set_sign=*/true, /*count=*/false);
+  x->have_state = (rc == CTAUX_OK);
+  return rc;
+}
+
+int ctaux_set_state(ctaux_ctx* x, const uint64_t* seeds, const int32_t* k, const uint64_t* id,
+                    const int32_t* site, const double* tau, const int8_t* spin, const uint64_t* next_id,
+                    const uint64_t* proposals) {
+  if (!x || !seeds || !k || !id || !site || !tau || !spin || !next_id || !proposals) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  std::vector<int32_t> spin32((size_t)d.max_k);
+  for (int w = 0; w < d.B; ++w) {
+    if (k[w] < 0 || k[w] > d.max_k) return CTAUX_EINVAL;
+    const size_t off = ((size_t)w * 2 + 0) * d.cap, src = (size_t)w * d.max_k;
+    for (int i = 0; i < k[w]; ++i) spin32[i] = spin[src + i];
+    CU_CHECK(cudaMemcpyAsync(d.cfg_site + off, site + src, 4 * (size_t)k[w], cudaMemcpyHostToDevice, s));
+    CU_CHECK(cudaMemcpyAsync(d.cfg_tau + off, tau + src, 8 * (size_t)k[w], cudaMemcpyHostToDevice, s));
+    CU_CHECK(cudaMemcpyAsync(d.cfg_id + off, id + src, 8 * (size_t)k[w], cudaMemcpyHostToDevice, s));
+    CU_CHECK(cudaMemcpyAsync(d.cfg_spin + off, spin32.data(), 4 * (size_t)k[w], cudaMemcpyHostToDevice, s));
+    CU_CHECK(cudaStreamSynchronize(s));
+  }
+  // scalars: seeds | k | next_id | proposals staged through the (large enough) Um scratch
+  char* scratch = (char*)d.Um;
+  uint64_t* d_seeds = x->seeds_d;
+  int32_t* d_k = (int32_t*)scratch;
+  uint64_t* d_next = (uint64_t*)(scratch + align256(4 * (size_t)d.B));
+  uint64_t* d_p = (uint64_t*)(scratch + 2 * align256(8 * (size_t)d.B));
+  CU_CHECK(cudaMemcpyAsync(d_seeds, seeds, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(d_k, k, 4 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(d_next, next_id, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(d_p, proposals, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  k_set_state<<<(d.B + 127) / 128, 128, 0, s>>>(d, d_seeds, d_k, d_next, d_p);
+  tick(x, C_OTHER);
+  CU_CHECK(cudaGetLastError());
+  CU_CHECK(cudaStreamSynchronize(s));
+  x->sweeps_since_rebuild = 0;
+  int rc = do_rebuild(x, true, false);
+  x->have_state = (rc == CTAUX_OK);
+  return rc;
+}
+
+int ctaux_rebuild(ctaux_ctx* x) {
+  if (!x) return CTAUX_EINVAL;
+  if (!x->have_state) return CTAUX_ESTATE;
+  x->sweeps_since_rebuild = 0;
+  return do_rebuild(x, false, true);
+}
+
+int ctaux_sweep(ctaux_ctx* x, int32_t n_sweeps) {
+  if (!x || n_sweeps < 0) return CTAUX_EINVAL;
+  if (!x->have_state) return CTAUX_ESTATE;
+  int remaining = n_sweeps;
+  const int re = x->prm.rebuild_every;
+  while (remaining > 0) {
+    int chunk = remaining;
+    if (re > 0) {
+      const int until = re - x->sweeps_since_rebuild;
+      if (chunk > until) chunk = until;
+    }
+    int rc = run_sweeps_chunk(x, chunk);
+    if (rc) { x->have_state = false; return rc; }
+    remaining -= chunk;
+    x->sweeps_since_rebuild += chunk;
+    if (re > 0 && x->sweeps_since_rebuild >= re) {
+      rc = do_rebuild(x, false, true);
+      if (rc) { x->have_state = false; return rc; }
+      x->sweeps_since_rebuild = 0;
+    }
+  }
+  return CTAUX_OK;
+}
+
+int ctaux_get_config(ctaux_ctx* x, int32_t w, int32_t* k, uint64_t* id, int32_t* site, double* tau,
+                     int8_t* spin, int32_t cap) {
+  if (!x || w < 0 || w >= x->d.B || !k) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  WalkerState st;
+  CU_CHECK(cudaMemcpy(&st, d.ws + w, sizeof(st), cudaMemcpyDeviceToHost));
+  *k = st.k;
+  if (cap < st.k && (id || site || tau || spin)) return CTAUX_ECAPACITY;
+  const size_t off = ((size_t)w * 2 + st.cfg_cur) * d.cap;
+  if (id) CU_CHECK(cudaMemcpy(id, d.cfg_id + off, 8 * (size_t)st.k, cudaMemcpyDeviceToHost));
+  if (site) CU_CHECK(cudaMemcpy(site, d.cfg_site + off, 4 * (size_t)st.k, cudaMemcpyDeviceToHost));
+  if (tau) CU_CHECK(cudaMemcpy(tau, d.cfg_tau + off, 8 * (size_t)st.k, cudaMemcpyDeviceToHost));
+  if (spin) {
+    std::vector<int32_t> tmp(st.k);
+    CU_CHECK(cudaMemcpy(tmp.data(), d.cfg_spin + off, 4 * (size_t)st.k, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < st.k; ++i) spin[i] = (int8_t)tmp[i];
+  }
+  return CTAUX_OK;
+}
+
+static int get_N_impl(ctaux_ctx* x, int32_t w, int32_t sp, double* N, int32_t ld, cudaMemcpyKind kind) {
+  if (!x || w < 0 || w >= x->d.B || sp < 0 || sp > 1 || !N) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  WalkerState st;
+  CU_CHECK(cudaMemcpy(&st, d.ws + w, sizeof(st), cudaMemcpyDeviceToHost));
+  if (ld < st.k) return CTAUX_EINVAL;
+  if (st.k == 0) return CTAUX_OK;
+  const double* src = d.Nbuf + (((size_t)w * 2 + sp) * 2 + st.n_cur) * (size_t)d.ld * d.ld;
+  CU_CHECK(cudaMemcpy2D(N, (size_t)ld * 8, src, (size_t)d.ld * 8, (size_t)st.k * 8, st.k, kind));
+  return CTAUX_OK;
+}
+int ctaux_get_N(ctaux_ctx* x, int32_t w, int32_t sp, double* N, int32_t ld) {
+  return get_N_impl(x, w, sp, N, ld, cudaMemcpyDeviceToHost);
+}
+int ctaux_get_N_device(ctaux_ctx* x, int32_t w, int32_t sp, double* N, int32_t ld) {
+  return get_N_impl(x, w, sp, N, ld, cudaMemcpyDeviceToDevice);
+}
+
+int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
+  if (!x || w < 0 || w >= x->d.B || !out) return CTAUX_EINVAL;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  WalkerState st;
+  CU_CHECK(cudaMemcpy(&st, x->d.ws + w, sizeof(st), cudaMemcpyDeviceToHost));
+  out->proposals = st.p; out->next_id = st.next_id;
+  out->acc_ins = st.acc_ins; out->acc_rem = st.acc_rem; out->sweeps = st.sweeps;
+  out->blocks = st.blocks; out->flushes = st.flushes; out->rebuilds = st.rebuilds; out->sum_rank = st.sum_rank;
+  out->k = st.k; out->sign = st.sign;
+  out->flops_cand = st.flops_cand; out->flops_flush = st.flops_flush; out->flops_rebuild = st.flops_rebuild;
+  out->min_margin = st.min_margin; out->sum_k = st.sum_k;
+  return CTAUX_OK;
+}
+
+int64_t ctaux_get_log(ctaux_ctx* x, int32_t w, ctaux_log_entry* out, int64_t first, int64_t count) {
+  if (!x || w < 0 || w >= x->d.B || !out || first < 0 || count < 0) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  if (cudaStreamSynchronize(x->stream) != cudaSuccess) return CTAUX_ECUDA;
+  WalkerState st;
+  if (cudaMemcpy(&st, d.ws + w, sizeof(st), cudaMemcpyDeviceToHost) != cudaSuccess) return CTAUX_ECUDA;
+  int64_t have = st.log_count < d.log_capacity ? st.log_count : d.log_capacity;
+  if (first >= have) return 0;
+  if (first + count > have) count = have - first;
+  if (count == 0) return 0;
+  if (cudaMemcpy(out, d.log + (size_t)w * d.log_capacity + first, (size_t)count * sizeof(LogEntry),
+                 cudaMemcpyDeviceToHost) != cudaSuccess)
+    return CTAUX_ECUDA;
+  return count;
+}
+
+int64_t ctaux_launch_count(ctaux_ctx* x) { return x ? x->launches : 0; }
+
+int ctaux_timing_enable(ctaux_ctx* x, int32_t on) {
+  if (!x) return CTAUX_EINVAL;
+  cudaStreamSynchronize(x->stream);
+  harvest_timing(x);
+  x->timing = on != 0;
+  memset(x->ms, 0, sizeof(x->ms));
+  memset(x->nl, 0, sizeof(x->nl));
+  return CTAUX_OK;
+}
+int ctaux_timing_get(ctaux_ctx* x, double* ms, int64_t* launches) {
+  if (!x || !ms || !launches) return CTAUX_EINVAL;
+  cudaStreamSynchronize(x->stream);
+  harvest_timing(x);
+  for (int i = 0; i < N_CLASS; ++i) { ms[i] = x->ms[i]; launches[i] = x->nl[i]; }
+  return CTAUX_OK;
+}
+
+int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
+                const double* B, int32_t ldb, double beta, double* C, int32_t ldc) {
+  if (M < 0 || N < 0 || K < 0 || !C || ldc < M) return CTAUX_EINVAL;
+  if (K > 0 && (!A || !B || lda < M || ldb < K || (lda & 1) || (ldb & 1) || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)))
+    return CTAUX_EINVAL;
+  if (K == 0) { A = C; B = C; lda = ldb = 2; }  // never dereferenced: C = beta*C
+  if (M == 0 || N == 0) return CTAUX_OK;
+  DescPlain fn;
+  fn.d.M = M; fn.d.N = N; fn.d.K = K;
+  fn.d.A = A; fn.d.lda = lda; fn.d.B = B; fn.d.ldb = ldb; fn.d.C = C; fn.d.ldc = ldc;
+  fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
+  fn.d.alpha = alpha; fn.d.beta = beta;
+  const int tiles = ((M + 127) / 128) * ((N + 127) / 128);
+  CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream)));
+  return CTAUX_OK;
+}
+
+int ctaux_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int32_t n) {
+  if (!ctr || !key || !out || n < 0) return CTAUX_EINVAL;
+  if (n == 0) return CTAUX_OK;
+  uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+  CU_CHECK(cudaMalloc((void**)&dc, 16 * (size_t)n));
+  CU_CHECK(cudaMalloc((void**)&dk, 8 * (size_t)n));
+  CU_CHECK(cudaMalloc((void**)&dout, 16 * (size_t)n));
+  CU_CHECK(cudaMemcpy(dc, ctr, 16 * (size_t)n, cudaMemcpyHostToDevice));
+  CU_CHECK(cudaMemcpy(dk, key, 8 * (size_t)n, cudaMemcpyHostToDevice));
+  k_debug_philox<<<(n + 127) / 128, 128>>>(dc, dk, dout, n);
+  CU_CHECK(cudaGetLastError());
+  CU_CHECK(cudaMemcpy(out, dout, 16 * (size_t)n, cudaMemcpyDeviceToHost));
+  cudaFree(dc); cudaFree(dk); cudaFree(dout);
+  return CTAUX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,184 @@
+// Grouped FP64 GEMM on the sm_100a FP64 tensor pipe (mma.sync m8n8k4 -> SASS DMMA.8x8x4).
+//
+// Serves S2 (candidate rows / columns), S4 (U*S^-1 and the rank-r flush with its compaction
+// gather) and S5 (trailing updates of the blocked LU).  PAPER.md:226 ("rank-k_s operation"),
+// PAPER.md:373 ("large matrix-matrix multiplications").
+//
+// All operands are column-major.  One launch covers a GROUP of independent problems
+// (walker x spin); each problem's sizes and pointers come from a device-side descriptor
+// that a functor builds from the walker state, so no host round trip is needed when the
+// expansion order changes.
+//
+//   C[i,j] = beta * C0[rowmap[i], colmap[j]] + alpha * sum_k A[i,k] * B[k,j]
+//
+// Tiling: CTA tile BM x BN x 16, 256 threads = 8 warps, cp.async (16-byte, zero-filled
+// tails) multi-stage pipeline into shared memory; each warp owns a (BM/WM) x (BN/WN) tile of
+// 8x8 DMMA fragments held in registers.
+//   A_s[k][m]  (m contiguous, row stride BM+4): fragment reads hit 16 distinct 8-byte banks
+//   B_s[n][k]  (k contiguous, row stride 20)  : same
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ctaux {
+
+struct GemmDesc {
+  int M, N, K;
+  const double* A; int lda;      // M x K
+  const double* B; int ldb;      // K x N
+  double* C; int ldc;            // M x N
+  const double* C0; int ldc0;    // source of the beta term (may alias C when no maps are given)
+  const int* rowmap;             // nullptr = identity
+  const int* colmap;
+  double alpha, beta;
+};
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+template <int BM, int BN, int WM, int WN, int STAGES>
+struct GemmCfg {
+  static constexpr int BK = 16;
+  static constexpr int THREADS = WM * WN * 32;
+  static constexpr int LDA_S = BM + 4;   // doubles
+  static constexpr int LDB_S = BK + 4;
+  static constexpr int A_STAGE = BK * LDA_S;
+  static constexpr int B_STAGE = BN * LDB_S;
+  static constexpr int SMEM_BYTES = STAGES * (A_STAGE + B_STAGE) * 8;
+  static constexpr int TM = BM / WM / 8;  // 8x8 fragments per warp along M
+  static constexpr int TN = BN / WN / 8;
+};
+
+// One CTA computes one BM x BN tile of one problem.
+template <int BM, int BN, int WM, int WN, int STAGES>
+__device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int tile_n, double* smem) {
+  using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
+  constexpr int BK = Cfg::BK, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
+  constexpr int TM = Cfg::TM, TN = Cfg::TN, THREADS = Cfg::THREADS;
+  double* As = smem;
+  double* Bs = smem + STAGES * Cfg::A_STAGE;
+
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int wm = warp % WM, wn = warp / WM;
+  const int g = lane >> 2, q = lane & 3;
+  const int m0 = tile_m * BM, n0 = tile_n * BN;
+  const int M = d.M, N = d.N, K = d.K;
+
+  double acc[TM][TN][2];
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  const int nk = (K + BK - 1) / BK;
+
+  auto load_stage = [&](int kt, int st) {
+    const int k0 = kt * BK;
+    // A tile: BK columns (k) x BM rows (m), 16-byte chunks along m
+    constexpr int A_CHUNKS = BK * BM / 2;
+#pragma unroll
+    for (int c = tid; c < A_CHUNKS; c += THREADS) {
+      const int kk = c / (BM / 2), mm = (c % (BM / 2)) * 2;
+      const int gk = k0 + kk, gm = m0 + mm;
+      int bytes = 0;
+      if (gk < K) bytes = (gm + 1 < M) ? 16 : ((gm < M) ? 8 : 0);
+      const double* src = bytes ? (d.A + (size_t)gk * d.lda + gm) : d.A;
+      cp_async16(As + st * Cfg::A_STAGE + kk * LDA_S + mm, src, bytes);
+    }
+    // B tile: BN columns (n) x BK rows (k), 16-byte chunks along k
+    constexpr int B_CHUNKS = BN * BK / 2;
+#pragma unroll
+    for (int c = tid; c < B_CHUNKS; c += THREADS) {
+      const int nn = c / (BK / 2), kk = (c % (BK / 2)) * 2;
+      const int gk = k0 + kk, gn = n0 + nn;
+      int bytes = 0;
+      if (gn < N) bytes = (gk + 1 < K) ? 16 : ((gk < K) ? 8 : 0);
+      const double* src = bytes ? (d.B + (size_t)gn * d.ldb + gk) : d.B;
+      cp_async16(Bs + st * Cfg::B_STAGE + nn * LDB_S + kk, src, bytes);
+    }
+  };
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) {
+    if (s < nk) load_stage(s, s);
+    cp_async_commit();
+  }
+
+  for (int kt = 0; kt < nk; ++kt) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    {
+      const int nxt = kt + STAGES - 1;
+      if (nxt < nk) load_stage(nxt, nxt % STAGES);
+      cp_async_commit();
+    }
+    const double* a_s = As + (kt % STAGES) * Cfg::A_STAGE + wm * (TM * 8) + g;
+    const double* b_s = Bs + (kt % STAGES) * Cfg::B_STAGE + (wn * (TN * 8) + g) * LDB_S;
+#pragma unroll
+    for (int k4 = 0; k4 < BK; k4 += 4) {
+      double af[TM], bf[TN];
+#pragma unroll
+      for (int i = 0; i < TM; ++i) af[i] = a_s[(k4 + q) * LDA_S + i * 8];
+#pragma unroll
+      for (int j = 0; j < TN; ++j) bf[j] = b_s[j * 8 * LDB_S + k4 + q];
+#pragma unroll
+      for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+    }
+  }
+  cp_async_wait<0>();
+
+  // epilogue: thread holds C[row = g][cols 2q, 2q+1] of every 8x8 fragment
+  const double alpha = d.alpha, beta = d.beta;
+#pragma unroll
+  for (int j = 0; j < TN; ++j) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int col = n0 + wn * (TN * 8) + j * 8 + 2 * q + h;
+      if (col >= N) continue;
+      const int scol = d.colmap ? d.colmap[col] : col;
+#pragma unroll
+      for (int i = 0; i < TM; ++i) {
+        const int row = m0 + wm * (TM * 8) + i * 8 + g;
+        if (row >= M) continue;
+        double v = alpha * acc[i][j][h];
+        if (beta != 0.0) {
+          const int srow = d.rowmap ? d.rowmap[row] : row;
+          v += beta * d.C0[(size_t)scol * d.ldc0 + srow];
+        }
+        d.C[(size_t)col * d.ldc + row] = v;
+      }
+    }
+  }
+}
+
+// Grouped launch: blockIdx.y = problem, blockIdx.x = tile (tiles beyond the problem's own
+// count exit).  DescFn(problem) -> GemmDesc, evaluated on the device.
+template <int BM, int BN, int WM, int WN, int STAGES, class DescFn>
+__global__ void __launch_bounds__(WM * WN * 32, 1) gemm_grouped_kernel(DescFn fn) {
+  extern __shared__ __align__(16) double smem_gemm[];
+  GemmDesc d;
+  if (!fn(blockIdx.y, d)) return;
+  if (d.M <= 0 || d.N <= 0) return;
+  const int tm = (d.M + BM - 1) / BM, tn = (d.N + BN - 1) / BN;
+  // persistent over the tiles of this problem: grid.x CTAs stride over tm*tn tiles
+  for (int t = blockIdx.x; t < tm * tn; t += gridDim.x) {
+    gemm_tile<BM, BN, WM, WN, STAGES>(d, t % tm, t / tm, smem_gemm);
+    __syncthreads();
+  }
+}
+
+}  // namespace ctaux

@@ -1,0 +1,228 @@
+// S5: from-scratch rebuild  N_sigma = A_sigma^{-1}  by blocked right-looking LU with partial
+// pivoting, batched over all B*2 matrices (each with its own order k), followed by blocked
+// forward / backward substitution on the identity.  BASELINE.json: "a batched LU-based rebuild".
+//
+//   F = the non-current N buffer (A, overwritten by its LU factors: P A = L U)
+//   X = the current N buffer     (starts as I; row swaps make it P; then L^-1 P; then U^-1 L^-1 P)
+//
+// Per panel [j0, j1) of kLuNb columns:
+//   k_lu_panel : unblocked LU of the panel with partial pivoting (one CTA per matrix)
+//   k_lu_swap  : the panel's row interchanges applied to F outside the panel and to all of X
+//   k_lu_trsm  : rows j0..j1 of F (right of the panel) and of X  <-  L11^-1 * (those rows)
+//   GEMM       : trailing update of F (A22 -= L21 U12) and of X (X_below -= L21 X_panel)
+// Backward pass, panels from last to first:
+//   k_lu_trsm (upper) : X[j0:j1, :] <- U11^-1 X[j0:j1, :]
+//   GEMM              : X[0:j0, :] -= U[0:j0, j0:j1] X[j0:j1, :]
+// The trailing updates run on the DMMA GEMM tiles of gemm_dmma.cuh.
+#pragma once
+#include "gemm_dmma.cuh"
+#include "walker_state.cuh"
+
+namespace ctaux {
+
+constexpr int kLuNb = 32;
+
+__global__ void k_lu_init_identity(DevCtx c) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  double* X = c.N(w, sp, st.n_cur);
+  const size_t total = (size_t)k * k;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % k), j = (int)(idx / k);
+    X[(size_t)j * c.ld + i] = (i == j) ? 1.0 : 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_lu_panel(DevCtx c, int j0, int* detsign) {
+  const int w = blockIdx.x >> 1, sp = blockIdx.x & 1;
+  WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (j0 >= k) return;
+  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
+  const int ld = c.ld, tid = threadIdx.x, nt = blockDim.x;
+  __shared__ double s_val[32];
+  __shared__ int s_idx[32];
+  __shared__ int s_p;
+  __shared__ double s_row[kLuNb];
+  for (int col = j0; col < j1; ++col) {
+    // pivot search in column col, rows col..k-1 (ties: smallest row index, as a serial scan would)
+    double best = -1.0;
+    int bi = col;
+    for (int i = col + tid; i < k; i += nt) {
+      const double v = fabs(F[(size_t)col * ld + i]);
+      if (v > best) { best = v; bi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+    }
+    if ((tid & 31) == 0) { s_val[tid >> 5] = best; s_idx[tid >> 5] = bi; }
+    __syncthreads();
+    if (tid == 0) {
+      double b = s_val[0];
+      int ix = s_idx[0];
+      for (int q = 1; q < (nt >> 5); ++q)
+        if (s_val[q] > b || (s_val[q] == b && s_idx[q] < ix)) { b = s_val[q]; ix = s_idx[q]; }
+      s_p = ix;
+      ipiv[col] = ix;
+      if (!(b > 0.0)) st.status = -4;  // CTAUX_ESINGULAR
+      if (detsign) {
+        int sg = detsign[w * 2 + sp];
+        if (ix != col) sg = -sg;
+        if (F[(size_t)col * ld + ix] < 0.0) sg = -sg;
+        detsign[w * 2 + sp] = sg;
+      }
+    }
+    __syncthreads();
+    const int pr = s_p;
+    // interchange rows col <-> pr inside the panel; publish the pivot row
+    if (tid < j1 - j0) {
+      const int jj = j0 + tid;
+      double a = F[(size_t)jj * ld + col];
+      if (pr != col) {
+        const double b = F[(size_t)jj * ld + pr];
+        F[(size_t)jj * ld + col] = b;
+        F[(size_t)jj * ld + pr] = a;
+        a = b;
+      }
+      s_row[tid] = a;
+    }
+    __syncthreads();
+    const double piv = s_row[col - j0];
+    if (piv != 0.0) {
+      for (int i = col + 1 + tid; i < k; i += nt) {
+        const double l = F[(size_t)col * ld + i] / piv;
+        F[(size_t)col * ld + i] = l;
+        for (int jj = col + 1; jj < j1; ++jj) F[(size_t)jj * ld + i] -= l * s_row[jj - j0];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// one thread per column: apply the panel's interchanges to F (outside the panel) and to X (all columns)
+__global__ void k_lu_swap(DevCtx c, int j0) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (j0 >= k) return;
+  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+  const int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  double* X = c.N(w, sp, st.n_cur);
+  __shared__ int s_piv[kLuNb];
+  if (threadIdx.x < j1 - j0) s_piv[threadIdx.x] = ipiv[j0 + threadIdx.x];
+  __syncthreads();
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < 2 * k; t += gridDim.x * blockDim.x) {
+    double* col;
+    if (t < k) {
+      if (t >= j0 && t < j1) continue;
+      col = F + (size_t)t * c.ld;
+    } else {
+      col = X + (size_t)(t - k) * c.ld;
+    }
+    for (int q = 0; q < j1 - j0; ++q) {
+      const int p = s_piv[q];
+      if (p != j0 + q) {
+        const double a = col[j0 + q], b = col[p];
+        col[j0 + q] = b;
+        col[p] = a;
+      }
+    }
+  }
+}
+
+// Triangular solves with the kLuNb x kLuNb diagonal block, one thread per right-hand-side column.
+//   upper == 0: rows j0..j1 of F (columns >= j1) and of X (all columns)  <-  L11^-1 (unit lower)
+//   upper == 1: rows j0..j1 of X (all columns)                           <-  U11^-1
+__global__ void __launch_bounds__(128) k_lu_trsm(DevCtx c, int j0, int upper) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (j0 >= k) return;
+  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+  const int nb = j1 - j0, ld = c.ld;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  double* X = c.N(w, sp, st.n_cur);
+  __shared__ double T[kLuNb][kLuNb + 1];
+  for (int idx = threadIdx.x; idx < nb * nb; idx += blockDim.x) {
+    const int i = idx % nb, j = idx / nb;
+    T[i][j] = F[(size_t)(j0 + j) * ld + j0 + i];
+  }
+  __syncthreads();
+  const int ncolF = upper ? 0 : (k - j1);
+  const int total = ncolF + k;
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
+    double* col = (t < ncolF) ? (F + (size_t)(j1 + t) * ld + j0) : (X + (size_t)(t - ncolF) * ld + j0);
+    double x[kLuNb];
+#pragma unroll
+    for (int i = 0; i < kLuNb; ++i) x[i] = (i < nb) ? col[i] : 0.0;
+    if (!upper) {
+#pragma unroll
+      for (int i = 0; i < kLuNb; ++i) {
+        if (i < nb) {
+          double s = x[i];
+#pragma unroll
+          for (int l = 0; l < kLuNb; ++l)
+            if (l < i) s -= T[i][l] * x[l];
+          x[i] = s;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int i = kLuNb - 1; i >= 0; --i) {
+        if (i < nb) {
+          double s = x[i];
+#pragma unroll
+          for (int l = 0; l < kLuNb; ++l)
+            if (l > i && l < nb) s -= T[i][l] * x[l];
+          x[i] = s / T[i][i];
+        }
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < kLuNb; ++i)
+      if (i < nb) col[i] = x[i];
+  }
+}
+
+// GEMM descriptors of the trailing updates (alpha = -1, beta = 1, in place)
+struct DescLU {
+  DevCtx c;
+  int j0;
+  int which;  // 0: F trailing, 1: X forward (rows below the panel), 2: X backward (rows above)
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    const int k = st.k;
+    if (j0 >= k) return false;
+    const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+    const size_t ld = c.ld;
+    double* F = c.N(w, sp, st.n_cur ^ 1);
+    double* X = c.N(w, sp, st.n_cur);
+    d.K = j1 - j0;
+    d.lda = c.ld; d.ldb = c.ld; d.ldc = c.ld; d.ldc0 = c.ld;
+    d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = -1.0; d.beta = 1.0;
+    if (which == 0) {
+      d.M = k - j1; d.N = k - j1;
+      d.A = F + j1 + (size_t)j0 * ld; d.B = F + j0 + (size_t)j1 * ld; d.C = F + j1 + (size_t)j1 * ld;
+    } else if (which == 1) {
+      d.M = k - j1; d.N = k;
+      d.A = F + j1 + (size_t)j0 * ld; d.B = X + j0; d.C = X + j1;
+    } else {
+      d.M = j0; d.N = k;
+      d.A = F + (size_t)j0 * ld; d.B = X + j0; d.C = X;
+    }
+    d.C0 = d.C;
+    return d.M > 0 && d.N > 0;
+  }
+};
+
+}  // namespace ctaux

@@ -1,0 +1,538 @@
+// Kernels of the CT-AUX walker hot path other than the GEMM tiles.
+//   S1  k_build_A, k_prep_fill     (G0 interpolation, A and candidate rows/columns)
+//   S3  k_prep_window, k_propose   (Philox streams, Metropolis over the delayed block)
+//   S4  k_build_uv                 (U = X[:,J], V^T = rows J of N_ext)
+// Formulas: SURVEY.md Appendix A (derived from Eq. (19)-(27)); DESIGN.md.
+#pragma once
+#include "walker_state.cuh"
+
+namespace ctaux {
+
+// ---------------------------------------------------------------------------------------------
+// reset: walker w draws init_k vertices from Philox(counter=(i,0,0,0), key=seed)
+__global__ void k_init_config(DevCtx c, const uint64_t* seeds, int init_k) {
+  const int w = blockIdx.x;
+  WalkerState& st = c.ws[w];
+  const uint32_t k0 = (uint32_t)(seeds[w] & 0xffffffffu), k1 = (uint32_t)(seeds[w] >> 32);
+  const size_t off = c.cfg_off(w, 0);
+  for (int i = threadIdx.x; i < init_k; i += blockDim.x) {
+    uint32_t r[4];
+    philox4x32_10((uint32_t)i, 0u, 0u, 0u, k0, k1, r);
+    double tau = c.beta * unif53(r[2], r[3]);
+    if (tau >= c.beta) tau = nextafter(c.beta, 0.0);
+    c.cfg_spin[off + i] = ((r[0] >> 1) & 1u) ? -1 : +1;
+    c.cfg_site[off + i] = (int32_t)(((uint64_t)r[1] * (uint64_t)c.Nc) >> 32);
+    c.cfg_tau[off + i] = tau;
+    c.cfg_id[off + i] = (uint64_t)i;
+  }
+  if (threadIdx.x == 0) {
+    WalkerState z;
+    memset(&z, 0, sizeof(z));
+    z.key0 = k0; z.key1 = k1;
+    z.k = init_k; z.k_new = init_k;
+    z.next_id = (uint64_t)init_k;
+    z.sign = 1;
+    z.min_margin = 1e300;
+    st = z;
+  }
+}
+
+// set_state: configuration already copied into buffer 0 by the host; fill in the scalars
+__global__ void k_set_state(DevCtx c, const uint64_t* seeds, const int32_t* k, const uint64_t* next_id,
+                            const uint64_t* p) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.B) return;
+  WalkerState z;
+  memset(&z, 0, sizeof(z));
+  z.key0 = (uint32_t)(seeds[w] & 0xffffffffu); z.key1 = (uint32_t)(seeds[w] >> 32);
+  z.k = k[w]; z.k_new = k[w];
+  z.next_id = next_id[w]; z.p = p[w];
+  z.sign = 1;
+  z.min_margin = 1e300;
+  c.ws[w] = z;
+}
+
+// S1: A_sigma[i][j] = delta_ij E_j - g_ij (E_j - 1) into the current N buffer (column-major).
+__global__ void k_build_A(DevCtx c, int into_other) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  const size_t off = c.cfg_off(w, st.cfg_cur);
+  double* A = c.N(w, sp, into_other ? (st.n_cur ^ 1) : st.n_cur);
+  const size_t total = (size_t)k * k;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % k), j = (int)(idx / k);
+    const double Ej = c.E(sp, c.cfg_spin[off + j]);
+    double v;
+    if (i == j) v = Ej - c.g00 * (Ej - 1.0);
+    else v = -c.g(c.disp(c.cfg_site[off + i], c.cfg_site[off + j]), c.cfg_tau[off + i] - c.cfg_tau[off + j]) * (Ej - 1.0);
+    A[(size_t)j * c.ld + i] = v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Start of a ctaux_sweep chunk.
+__global__ void k_begin_sweeps(DevCtx c, int n_sweeps) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w == 0) *c.n_active = c.B;
+  if (w >= c.B) return;
+  c.ws[w].sweeps_left = n_sweeps;
+  c.ws[w].props_left = 0;
+  c.ws[w].active = 1;
+  c.ws[w].r = 0;
+}
+
+// S3a: expand the next window of proposals of every walker.  Philox is counter based, so the
+// words of proposals p, p+1, ... are known before any of them is decided.
+// Proposal p: wA = Philox(p_lo, p_hi, 0, 1), wB = Philox(p_lo, p_hi, 1, 1).
+__global__ void __launch_bounds__(1024) k_prep_window(DevCtx c) {
+  const int w = blockIdx.x;
+  WalkerState& st = c.ws[w];
+  __shared__ int s_scan[1024];
+  __shared__ int s_win;
+  const int tid = threadIdx.x;
+  if (!st.active || st.status) {
+    if (tid == 0) { st.m = 0; st.win = 0; st.r = 0; st.n_src = st.n_cur; }
+    return;
+  }
+  const int k = st.k;
+  const uint64_t p = st.p + (uint64_t)tid;
+  uint32_t wa[4] = {0, 0, 0, 0}, wb[4] = {0, 0, 0, 0};
+  const bool in = tid < c.winmax;
+  if (in) {
+    philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 0u, 1u, st.key0, st.key1, wa);
+    philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 1u, 1u, st.key0, st.key1, wb);
+  }
+  const int is_ins = (in && (wa[0] & 1u) == 0u) ? 1 : 0;
+  // inclusive scan of is_ins over the CTA
+  s_scan[tid] = is_ins;
+  if (tid == 0) s_win = c.winmax;
+  __syncthreads();
+  for (int off = 1; off < 1024; off <<= 1) {
+    int v = 0;
+    if (tid >= off) v = s_scan[tid - off];
+    __syncthreads();
+    s_scan[tid] += v;
+    __syncthreads();
+  }
+  const int cand = s_scan[tid] - is_ins;  // exclusive: index of this insertion among candidates
+  // the window ends before the first insertion that has no candidate slot left
+  if (is_ins && cand == c.mmax) s_win = tid;  // exactly one thread satisfies this
+  __syncthreads();
+  const int win = s_win;
+  if (in && tid < win) {
+    PropInfo pi;
+    pi.type_cand = (wa[0] & 1u) | ((uint32_t)(is_ins ? cand : 0) << 1);
+    pi.w1 = wa[1];
+    pi.u = unif53(wb[0], wb[1]);
+    c.prop[(size_t)w * c.winmax + tid] = pi;
+    if (is_ins) {  // candidate vertex -> extended slot k + cand of the current configuration buffer
+      const size_t off = c.cfg_off(w, st.cfg_cur) + k + cand;
+      double tau = c.beta * unif53(wa[2], wa[3]);
+      if (tau >= c.beta) tau = nextafter(c.beta, 0.0);
+      c.cfg_spin[off] = ((wa[0] >> 1) & 1u) ? -1 : +1;
+      c.cfg_site[off] = (int32_t)(((uint64_t)wa[1] * (uint64_t)c.Nc) >> 32);
+      c.cfg_tau[off] = tau;
+      c.cfg_id[off] = ~0ull;
+    }
+  }
+  if (tid == 0) {
+    const int m = (win > 0) ? (s_scan[win - 1]) : 0;
+    st.m = m < c.mmax ? m : c.mmax;
+    st.win = win;
+    st.r = 0;
+    st.n_src = st.n_cur;
+  }
+}
+
+// S1 for the block: candidate rows  Bm[c,j] = g(c,j)(E_j - 1)  (per spin),
+// candidate columns gxC[i,c] = g(i,c) over ALL extended slots i (spin independent), and the
+// [*, cand] block of N_ext (zeros + identity): a non-interacting slot has column e_c in A,
+// hence in N as well.
+__global__ void k_prep_fill(DevCtx c) {
+  const int w = blockIdx.y;
+  const WalkerState& st = c.ws[w];
+  const int m = st.m, k = st.k;
+  if (m == 0) return;
+  const int n = k + m;
+  const size_t off = c.cfg_off(w, st.cfg_cur);
+  const int32_t* site = c.cfg_site + off;
+  const double* tau = c.cfg_tau + off;
+  const int32_t* spin = c.cfg_spin + off;
+  double* Bm0 = c.Bm + ((size_t)w * 2 + 0) * (size_t)c.ldm * c.cap;
+  double* Bm1 = c.Bm + ((size_t)w * 2 + 1) * (size_t)c.ldm * c.cap;
+  double* gx = c.gxC + (size_t)w * c.ld * c.mmax;
+  double* N0 = c.N(w, 0, st.n_cur);
+  double* N1 = c.N(w, 1, st.n_cur);
+  const size_t total = (size_t)n * m;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % n), cc = (int)(idx / n);
+    const int sc = k + cc;
+    // column: g(i, c)
+    double gic;
+    if (i == sc) gic = c.g00;
+    else gic = c.g(c.disp(site[i], site[sc]), tau[i] - tau[sc]);
+    gx[(size_t)cc * c.ld + i] = gic;
+    // [*, cand] block of N_ext
+    const double e = (i == sc) ? 1.0 : 0.0;
+    N0[(size_t)sc * c.ld + i] = e;
+    N1[(size_t)sc * c.ld + i] = e;
+    // row: g(c, j)(E_j - 1), only against the live vertices j < k
+    if (i < k) {
+      const double gci = c.g(c.disp(site[sc], site[i]), tau[sc] - tau[i]);
+      Bm0[(size_t)i * c.ldm + cc] = gci * (c.E(0, spin[i]) - 1.0);
+      Bm1[(size_t)i * c.ldm + cc] = gci * (c.E(1, spin[i]) - 1.0);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S3: serial Metropolis over the window, one CTA per walker, both spins.
+// X_sigma = N_ext - G_ext (n x n, never formed):
+//   X[i,j] = (delta_ij - N_ext[i,j]) / (E0_j - 1)      j a block-start vertex
+//          =  delta_ij - Gx[i, j-k0]                   j a candidate
+// Buffered changes J = (j_1..j_r), dE_a;  S_ab = delta_ab/dE_a + X[j_a, j_b];
+// det A_{r+1} / det A_r = dE_new (s_nn - s_row S^-1 s_col)
+constexpr int kPropThreads = 256;
+constexpr int kGroup = kPropThreads / 2;  // threads per spin
+
+struct ProposeSmem {
+  // byte offsets into dynamic shared memory
+  int sinv, scol, srow, tv, tpv, red, snn, live0, live1, spin, J, jpos, prop, total;
+};
+
+__host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
+  ProposeSmem L;
+  int o = 0;
+  const int lds = delay | 1;
+  L.sinv = o; o += sinv_smem ? 2 * lds * delay * 8 : 0;
+  L.scol = o; o += 2 * delay * 8;
+  L.srow = o; o += 2 * delay * 8;
+  L.tv = o; o += 2 * delay * 8;
+  L.tpv = o; o += 2 * delay * 8;
+  L.red = o; o += 2 * 8 * 8;
+  L.snn = o; o += 2 * 8;
+  L.prop = o; o += winmax * 16;
+  L.live0 = o; o += cap * 4;
+  L.live1 = o; o += cap * 4;
+  L.J = o; o += delay * 4;
+  L.jpos = o; o += (winmax + 1) * 4;
+  L.spin = o; o += (cap + 15) / 16 * 16;
+  L.total = o;
+  return L;
+}
+
+__global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_smem) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const int w = blockIdx.x, tid = threadIdx.x;
+  WalkerState& st = c.ws[w];
+  if (!st.active || st.status || st.win == 0) return;
+  const ProposeSmem L = propose_smem_layout(c.cap, c.delay, c.winmax, sinv_smem != 0);
+  const int sp = tid / kGroup, lt = tid % kGroup;
+  const int lds = sinv_smem ? (c.delay | 1) : c.ldr;
+  double* Sbase = sinv_smem ? reinterpret_cast<double*>(smraw + L.sinv)
+                            : (c.Sinv + (size_t)w * 2 * (size_t)c.ldr * c.delay);
+  const size_t sstride = (size_t)lds * c.delay;  // spin stride of S^-1
+  double* Sv = Sbase + (size_t)sp * sstride;
+  double* scol = reinterpret_cast<double*>(smraw + L.scol) + sp * c.delay;
+  double* srow = reinterpret_cast<double*>(smraw + L.srow) + sp * c.delay;
+  double* tv = reinterpret_cast<double*>(smraw + L.tv) + sp * c.delay;
+  double* tpv = reinterpret_cast<double*>(smraw + L.tpv) + sp * c.delay;
+  double* red = reinterpret_cast<double*>(smraw + L.red);   // [2][8]
+  double* snn = reinterpret_cast<double*>(smraw + L.snn);   // [2]
+  PropInfo* prop = reinterpret_cast<PropInfo*>(smraw + L.prop);
+  int* live = reinterpret_cast<int*>(smraw + L.live0);
+  int* live_alt = reinterpret_cast<int*>(smraw + L.live1);
+  int* Js = reinterpret_cast<int*>(smraw + L.J);
+  int* jpos = reinterpret_cast<int*>(smraw + L.jpos);  // candidate index -> position in J (-1: not buffered)
+  signed char* spin_s = reinterpret_cast<signed char*>(smraw + L.spin);
+
+  const int k0 = st.k, m = st.m, win = st.win, n = k0 + m;
+  const int cfg_old = st.cfg_cur;
+  const size_t off_old = c.cfg_off(w, cfg_old), off_new = c.cfg_off(w, cfg_old ^ 1);
+  const double* Ncur = c.N(w, sp, st.n_cur);
+  const double* Gx = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
+  const int ld = c.ld;
+  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
+
+  for (int i = tid; i < n; i += kPropThreads) spin_s[i] = (signed char)c.cfg_spin[off_old + i];
+  for (int i = tid; i < k0; i += kPropThreads) live[i] = i;
+  for (int i = tid; i < win; i += kPropThreads) prop[i] = c.prop[(size_t)w * c.winmax + i];
+  for (int i = tid; i <= c.winmax; i += kPropThreads) jpos[i] = -1;
+  __syncthreads();
+
+  auto X = [&](int i, int j) -> double {
+    const double dlt = (i == j) ? 1.0 : 0.0;
+    if (j < k0) {
+      const bool em = ((sp == 0) == (spin_s[j] > 0));
+      return (dlt - Ncur[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
+    }
+    return dlt - Gx[(size_t)(j - k0) * ld + i];
+  };
+
+  int kcur = k0, r = 0, len = k0;
+  int props_left = st.props_left, sweeps_left = st.sweeps_left;
+  uint64_t next_id = st.next_id, p = st.p;
+  int sign = st.sign, status = 0, consumed = 0;
+  int64_t acc_ins = 0, acc_rem = 0, sweeps_done = 0;
+  double min_margin = st.min_margin, sum_k = 0.0;
+  int64_t log_count = st.log_count;
+  bool finished = false;
+
+  for (int i = 0; i < win; ++i) {
+    if (props_left == 0) {
+      if (sweeps_left == 0) { finished = true; break; }
+      --sweeps_left;
+      props_left = kcur > 16 ? kcur : 16;
+    }
+    const PropInfo pi = prop[i];
+    const int type = (int)(pi.type_cand & 1u);
+    int slot = -1, j = -1;
+    double pref = 0.0;
+    if (type == 0) {
+      slot = k0 + (int)(pi.type_cand >> 1);
+      pref = c.K / (double)(kcur + 1);
+    } else if (kcur > 0) {
+      j = (int)(((uint64_t)pi.w1 * (uint64_t)kcur) >> 32);
+      slot = live[j];
+      pref = (double)kcur / c.K;
+    }
+    bool accept = false;
+    double R = 0.0, stil_own = 1.0;
+    // removal of a vertex inserted earlier in this block: the two changes of that slot cancel, so
+    // the buffered insertion is taken OUT of the block (exact treatment of a twice-touched spin,
+    // PAPER.md:228): ratio = (S^-1)_aa / dE_a, then S^-1 is downdated.
+    const bool down = (type == 1 && slot >= k0);
+    int apos = -1;
+    if (down) {
+      apos = jpos[slot - k0];
+      const int s = spin_s[slot];
+      const double sa0 = Sbase[apos + (size_t)apos * lds], sa1 = Sbase[sstride + apos + (size_t)apos * lds];
+      R = pref * ((sa0 / (c.E(0, s) - 1.0)) * (sa1 / (c.E(1, s) - 1.0)));
+      accept = pi.u < fabs(R);
+      stil_own = sp == 0 ? sa0 : sa1;
+    } else if (slot >= 0) {
+      const int s = spin_s[slot];
+      const double E0 = c.E(0, s), E1 = c.E(1, s);
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (1.0 - E0);
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (1.0 - E1);
+      const double dE_own = sp == 0 ? dE0 : dE1;
+      for (int a = lt; a < r; a += kGroup) {
+        const int ja = Js[a];
+        scol[a] = X(ja, slot);
+        srow[a] = X(slot, ja);
+      }
+      if (lt == 0) snn[sp] = 1.0 / dE_own + X(slot, slot);
+      __syncthreads();
+      double part = 0.0;
+      for (int a = lt; a < r; a += kGroup) {
+        double t = 0.0, tp = 0.0;
+        for (int b = 0; b < r; ++b) {
+          t += Sv[a + (size_t)b * lds] * scol[b];
+          tp += srow[b] * Sv[b + (size_t)a * lds];
+        }
+        tv[a] = t;
+        tpv[a] = tp;
+        part += srow[a] * t;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      if ((tid & 31) == 0) red[sp * 8 + (lt >> 5)] = part;
+      __syncthreads();
+      const double dot0 = (red[0] + red[1]) + (red[2] + red[3]);
+      const double dot1 = (red[8] + red[9]) + (red[10] + red[11]);
+      const double stil0 = snn[0] - dot0, stil1 = snn[1] - dot1;
+      stil_own = sp == 0 ? stil0 : stil1;
+      R = pref * ((dE0 * stil0) * (dE1 * stil1));
+      accept = pi.u < fabs(R);
+    }
+    if (tid == 0) {
+      if (log_count < (int64_t)c.log_capacity) {
+        LogEntry e;
+        e.p = p; e.type = type;
+        e.arg = (type == 0) ? c.cfg_site[off_old + slot] : j;
+        e.tau = (type == 0) ? c.cfg_tau[off_old + slot] : 0.0;
+        e.spin = (type == 0) ? (int)spin_s[slot] : 0;
+        e.accepted = accept ? 1 : 0;
+        e.R = R; e.u = pi.u;
+        c.log[(size_t)w * c.log_capacity + log_count] = e;
+      }
+    }
+    ++log_count;
+    if (slot >= 0) {
+      const double aR = fabs(R);
+      const double mg = fabs(pi.u - aR) / fmax(aR, 1e-300);
+      if (mg < min_margin) min_margin = mg;
+    }
+    sum_k += (double)kcur;
+    if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }  // CTAUX_ECAPACITY
+    if (accept && down) {
+      // S^-1 <- S^-1 - S^-1[:,a] S^-1[a,:] / S^-1[a,a], then entry a is replaced by the last one
+      const double inv = 1.0 / stil_own;
+      for (int a = lt; a < r; a += kGroup) {
+        tv[a] = Sv[a + (size_t)apos * lds];
+        tpv[a] = Sv[apos + (size_t)a * lds];
+      }
+      __syncthreads();
+      for (int idx = lt; idx < r * r; idx += kGroup) {
+        const int a = idx % r, b = idx / r;
+        Sv[a + (size_t)b * lds] -= tv[a] * tpv[b] * inv;
+      }
+      __syncthreads();
+      const int last = r - 1;
+      if (apos != last) {
+        for (int b = lt; b < r; b += kGroup) Sv[apos + (size_t)b * lds] = Sv[last + (size_t)b * lds];
+        __syncthreads();
+        for (int a = lt; a < last; a += kGroup) Sv[a + (size_t)apos * lds] = Sv[a + (size_t)last * lds];
+      }
+      if (tid == 0) {
+        jpos[slot - k0] = -1;
+        if (apos != last) {
+          const int moved = Js[last];
+          Js[apos] = moved;
+          if (moved >= k0) jpos[moved - k0] = apos;
+        }
+      }
+      for (int idx = tid; idx < len - 1; idx += kPropThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
+      int* t = live; live = live_alt; live_alt = t;
+      --len; --kcur; ++acc_rem;
+      if (R < 0.0) sign = -sign;
+      --r;
+    } else if (accept) {
+      const double inv = 1.0 / stil_own;
+      for (int idx = lt; idx < r * r; idx += kGroup) {
+        const int a = idx % r, b = idx / r;
+        Sv[a + (size_t)b * lds] += tv[a] * tpv[b] * inv;
+      }
+      for (int a = lt; a < r; a += kGroup) {
+        Sv[a + (size_t)r * lds] = -tv[a] * inv;
+        Sv[r + (size_t)a * lds] = -tpv[a] * inv;
+      }
+      if (lt == 0) Sv[r + (size_t)r * lds] = inv;
+      if (tid == 0) Js[r] = slot;
+      if (type == 0) {
+        if (tid == 0) { live[len] = slot; c.cfg_id[off_old + slot] = next_id; jpos[slot - k0] = r; }
+        ++len; ++kcur; ++next_id; ++acc_ins;
+      } else {
+        for (int idx = tid; idx < len - 1; idx += kPropThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
+        int* t = live; live = live_alt; live_alt = t;
+        --len; --kcur; ++acc_rem;
+      }
+      if (R < 0.0) sign = -sign;
+      ++r;
+    }
+    __syncthreads();
+    --props_left; ++consumed; ++p;
+    if (props_left == 0) ++sweeps_done;
+    if (r == c.delay) break;
+  }
+  __syncthreads();
+  if (props_left == 0 && sweeps_left == 0) finished = true;
+
+  // ---- write back: new list (compacted), S^-1, J, scalars
+  int* rowmap = c.rowmap + (size_t)w * c.cap;
+  for (int i = tid; i < kcur; i += kPropThreads) {
+    const int sl = live[i];
+    rowmap[i] = sl;
+    c.cfg_site[off_new + i] = c.cfg_site[off_old + sl];
+    c.cfg_tau[off_new + i] = c.cfg_tau[off_old + sl];
+    c.cfg_spin[off_new + i] = c.cfg_spin[off_old + sl];
+    c.cfg_id[off_new + i] = c.cfg_id[off_old + sl];
+  }
+  if (sinv_smem) {
+    double* Sg = c.Sinv + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.delay;
+    for (int idx = lt; idx < r * r; idx += kGroup) {
+      const int a = idx % r, b = idx / r;
+      Sg[a + (size_t)b * c.ldr] = Sv[a + (size_t)b * lds];
+    }
+  }
+  for (int a = tid; a < r; a += kPropThreads) c.J[(size_t)w * c.delay + a] = Js[a];
+  if (tid == 0) {
+    st.k_new = kcur;
+    st.k = kcur;
+    st.m = k0;  // block-start order, read by k_build_uv (m is re-set by the next k_prep_window)
+    st.cfg_cur = cfg_old ^ 1;
+    st.r = r;
+    st.n_src = st.n_cur;
+    if (r > 0) st.n_cur ^= 1;
+    st.next_id = next_id; st.p = p; st.sign = sign;
+    st.sweeps_left = sweeps_left; st.props_left = props_left;
+    st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
+    st.blocks += 1;
+    if (r > 0) { st.flushes += 1; st.sum_rank += r; }
+    st.log_count = log_count;
+    st.min_margin = min_margin; st.sum_k += sum_k;
+    st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
+    st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r + 2.0 * (double)kcur * r * r);
+    if (status) st.status = status;
+    if (finished || status) {
+      st.active = 0;
+      atomicSub(c.n_active, 1);
+    }
+  }
+}
+
+// S4a: U[i', a] = X[rowmap[i'], J[a]],  Vt[a, j'] = N_ext[J[a], rowmap[j']]   (live rows/cols only)
+__global__ void k_build_uv(DevCtx c) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int r = st.r;
+  if (r == 0) return;
+  const int kn = st.k_new, k0 = st.m;  // m holds the block-start order after k_propose
+  const size_t off_old = c.cfg_off(w, st.cfg_cur ^ 1);
+  const double* Nsrc = c.N(w, sp, st.n_src);
+  const double* Gx = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
+  double* U = c.Um + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay;
+  double* Vt = c.Vt + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.ld;
+  const int* rowmap = c.rowmap + (size_t)w * c.cap;
+  const int* J = c.J + (size_t)w * c.delay;
+  const int ld = c.ld;
+  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
+  const size_t total = (size_t)kn * r;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    {  // U: consecutive threads walk down a column of N_ext / Gx
+      const int ip = (int)(idx % kn), a = (int)(idx / kn);
+      const int i = rowmap[ip], j = J[a];
+      const double dlt = (i == j) ? 1.0 : 0.0;
+      double x;
+      if (j < k0) {
+        const bool em = ((sp == 0) == (c.cfg_spin[off_old + j] > 0));
+        x = (dlt - Nsrc[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
+      } else {
+        x = dlt - Gx[(size_t)(j - k0) * ld + i];
+      }
+      U[(size_t)a * ld + ip] = x;
+    }
+    {  // Vt: consecutive threads write consecutive a (r contiguous)
+      const int a = (int)(idx % r), jp = (int)(idx / r);
+      Vt[(size_t)jp * c.ldr + a] = Nsrc[(size_t)rowmap[jp] * ld + J[a]];
+    }
+  }
+}
+
+__global__ void k_set_sign_from_det(DevCtx c, const int* detsign) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.B) return;
+  c.ws[w].sign = detsign[2 * w] * detsign[2 * w + 1];
+}
+
+__global__ void k_count_rebuild(DevCtx c) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.B) return;
+  WalkerState& st = c.ws[w];
+  st.rebuilds += 1;
+  st.flops_rebuild += 2.0 * 2.0 * (double)st.k * st.k * st.k;
+}
+
+__global__ void k_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t r[4];
+  philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1], r);
+  out[4 * i] = r[0]; out[4 * i + 1] = r[1]; out[4 * i + 2] = r[2]; out[4 * i + 3] = r[3];
+}
+
+}  // namespace ctaux

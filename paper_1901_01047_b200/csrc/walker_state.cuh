@@ -1,0 +1,127 @@
+// Device-side state of the batched CT-AUX walkers and small device helpers
+// (Philox4x32-10, G0 interpolation, E = e^{-gamma sigma s}).  SURVEY.md 8c.1 / DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ctaux {
+
+constexpr int kMaxDelay = 256;
+
+struct LogEntry {  // == ctaux_log_entry
+  uint64_t p;
+  int32_t type, arg;
+  double tau;
+  int32_t spin, accepted;
+  double R, u;
+};
+
+struct PropInfo {  // one pre-expanded proposal of the current window (16 bytes)
+  uint32_t type_cand;  // bit0: type (0 insert, 1 remove); bits 1..: candidate index (inserts)
+  uint32_t w1;         // word used for the removal index
+  double u;            // uniform for the Metropolis test
+};
+
+struct WalkerState {
+  uint32_t key0, key1;
+  int32_t k;        // expansion order at block start
+  int32_t cfg_cur;  // current configuration buffer (0/1)
+  int32_t n_cur;    // current N buffer (0/1), both spins
+  int32_t n_src;    // N buffer the pending flush reads (== n_cur when r == 0)
+  int32_t status;   // 0 ok, else CTAUX_E*
+  int32_t sign;
+  uint64_t next_id, p;
+  int32_t sweeps_left, props_left;
+  // current block
+  int32_t m;       // insertion candidates pre-expanded
+  int32_t win;     // proposals in the window
+  int32_t r;       // accepted changes (rank of the flush)
+  int32_t k_new;   // expansion order after the block
+  int32_t active;  // 1 while the walker still has proposals to do in this sweep call
+  int32_t pad0;
+  // statistics
+  int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count;
+  double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k;
+};
+
+// Everything a kernel needs: passed by value (fits the 4 KB parameter space easily).
+struct DevCtx {
+  int B, Lx, Ly, Nc, M;
+  int max_k, mmax, winmax, delay;
+  int cap;   // max_k + mmax : extended slots
+  int ld;    // leading dimension of every N / Gx / U buffer (cap rounded up to 8)
+  int ldm;   // leading dimension of Bm (mmax rounded up to 8)
+  int ldr;   // leading dimension of Vt / Sinv in global memory (delay rounded up to 8)
+  int log_capacity;
+  double beta, K, tau_scale, egp, egm, g00;
+  const double* table;  // [Nc][M+1]
+  WalkerState* ws;      // [B]
+  // configuration, double buffered, extended slots: [B][2][cap]
+  int32_t* cfg_site; double* cfg_tau; int32_t* cfg_spin; uint64_t* cfg_id;
+  PropInfo* prop;       // [B][winmax]
+  double* Nbuf;         // [B][2 spins][2 bufs][ld*ld]
+  double* Bm;           // [B][2][ldm*cap]   candidate rows  g(c,j)(E_j-1), m x k col-major
+  double* gxC;          // [B][ld*mmax]      g_ext[:, C], n x m col-major (spin independent)
+  double* Gx;           // [B][2][ld*mmax]   N_ext * g_ext[:, C]
+  double* Um;           // [B][2][ld*delay]  U = X[:, J]
+  double* Ut;           // [B][2][ld*delay]  U * S^-1
+  double* Vt;           // [B][2][ldr*ld]    rows J of N_ext, r x k' col-major
+  double* Sinv;         // [B][2][ldr*delay]
+  int32_t* J;           // [B][delay]
+  int32_t* rowmap;      // [B][cap]  new list position -> extended slot
+  LogEntry* log;        // [B][log_capacity]
+  int32_t* n_active;    // [1] walkers still active (device), mirrored to pinned host
+  // rebuild scratch
+  double* colbuf;       // [B][2][ld]
+  double* rowbuf;       // [B][2][ld]
+  int32_t* perm;        // [B][2][ld]
+
+  __device__ __forceinline__ size_t cfg_off(int w, int buf) const { return ((size_t)w * 2 + buf) * cap; }
+  __device__ __forceinline__ double* N(int w, int s, int buf) const {
+    return Nbuf + (((size_t)w * 2 + s) * 2 + buf) * (size_t)ld * ld;
+  }
+  __device__ __forceinline__ double E(int sidx, int s) const {
+    // sigma = +1 for sidx 0 (up), -1 for sidx 1; E = exp(-gamma sigma s)
+    return ((sidx == 0) == (s > 0)) ? egm : egp;
+  }
+  __device__ __forceinline__ int disp(int i, int j) const {
+    const int xi = i % Lx, yi = i / Lx, xj = j % Lx, yj = j / Lx;
+    int dx = xi - xj; if (dx < 0) dx += Lx;
+    int dy = yi - yj; if (dy < 0) dy += Ly;
+    return dx + Lx * dy;
+  }
+  // positive-convention propagator g = -G0 by linear interpolation, antiperiodic in tau
+  __device__ __forceinline__ double g(int d, double dtau) const {
+    double sg = 1.0;
+    if (dtau < 0.0) { sg = -1.0; dtau += beta; }
+    const double x = dtau * tau_scale;
+    int m = (int)floor(x);
+    if (m > M - 1) m = M - 1;
+    const double f = x - (double)m;
+    const double* T = table + (size_t)d * (M + 1);
+    const double t0 = __ldg(T + m), t1 = __ldg(T + m + 1);
+    return -sg * (t0 + f * (t1 - t0));
+  }
+};
+
+// ---------------------------------------------------------------- Philox4x32-10 (device + host)
+__host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                       uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__host__ __device__ __forceinline__ double unif53(uint32_t a, uint32_t b) {
+  const uint64_t u = ((uint64_t)a << 21) | (uint64_t)(b >> 11);
+  return (double)u * (1.0 / 9007199254740992.0);
+}
+
+}  // namespace ctaux

@@ -1,0 +1,159 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar (BASELINE.json north_star): accept/reject sequences and vertex
+configurations BIT-EXACT; N within relative Frobenius error 1e-10 in FP64."""
+import numpy as np
+import pytest
+
+from ctaux_workloads import get_config, table_for, walker_seeds
+from oracle.ctaux_oracle import T0, T1, OracleWalker, philox
+
+from parity_helpers import compare_configs, compare_logs, compare_N, frob_rel, full_parity, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _pkg():
+    import paper_1901_01047_b200 as pkg
+    return pkg
+
+
+def test_P12_device_philox_equals_oracle_philox():
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2 ** 32, size=(257, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(257, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    key[0] = 0
+    ctr[1] = [5, 0, 1, 1]
+    dev = _pkg().debug_philox(ctr, key)
+    for i in range(ctr.shape[0]):
+        assert dev[i].tolist() == philox(ctr[i], key[i]).tolist()
+
+
+@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (8, 8, 4), (130, 70, 33), (128, 128, 64), (257, 511, 100),
+                                   (1000, 40, 1000), (64, 1000, 7), (300, 300, 0)])
+def test_dgemm_tiles_against_torch_fp64(M, N, K):
+    """The DMMA tile kernel (several tiles + ragged tails) against torch's FP64 matmul."""
+    import torch
+    pkg = _pkg()
+    g = torch.Generator(device="cpu").manual_seed(M * 7 + N * 3 + K)
+    rnd = lambda r, c: torch.randn(r, c, generator=g, dtype=torch.float64)
+    A = pkg.colmajor(M, K, fill=rnd)
+    B = pkg.colmajor(K, N, fill=rnd)
+    C0 = pkg.colmajor(M, N, fill=rnd)
+    C = pkg.colmajor(M, N)
+    C.copy_(C0)
+    out = pkg.ctaux_dgemm(A, B, C, alpha=-1.5, beta=0.5)
+    ref = 0.5 * C0 - 1.5 * (A @ B)
+    torch.cuda.synchronize()
+    scale = float(ref.abs().max()) + 1e-300
+    assert float((out - ref).abs().max()) / scale < 1e-13 * max(K, 1)
+
+
+@pytest.mark.parametrize("ci,nw", [(0, 1), (1, 5), (2, 3)])
+def test_reset_builds_inverse(ci, nw):
+    """S1 + S5: N after reset equals the oracle's direct inverse of A built from the same vertices."""
+    cfg = get_config(ci)
+    table = table_for(cfg)
+    W = _pkg().Walkers.from_config(cfg, table, n_walkers=nw)
+    seeds = walker_seeds(nw, first=10)
+    W.reset(seeds)
+    for w in range(nw):
+        o = OracleWalker.from_config(cfg, table, int(seeds[w]), T0)
+        o.reset(cfg["init_k"])
+        compare_configs(W.get_config(w), o.config(), f"reset walker {w}")
+        compare_N(W, w, o, f"reset walker {w}")
+        assert W.get_stats(w)["sign"] == o.sign
+        # P7 on the device matrix itself: N A = 1
+        for s in range(2):
+            k = o.k
+            assert np.linalg.norm(W.get_N(w, s) @ o.A(s) - np.eye(k)) / np.sqrt(k) < 1e-10
+
+
+def test_config1_full_lockstep_T0():
+    """Config 1 in full (200 warm-up + 1000 sweeps, 1 walker, delay 8) against brute force T0."""
+    cfg = get_config(0)
+    W, orcs, worst = full_parity(cfg, 1, cfg["warmup_sweeps"] + cfg["sweeps"], T0)
+    assert W.get_stats(0)["rebuilds"] == 120
+
+
+def test_config2_batched_walkers_T0_prefix_and_T1():
+    cfg = get_config(1)
+    full_parity(cfg, 16, 12, T0)          # brute force on a prefix, 16 walkers
+    full_parity(cfg, 256, 40, T1)         # all 256 walkers, rank-1 oracle
+
+
+def test_config3_T1():
+    cfg = get_config(2)
+    full_parity(cfg, 64, 6, T1)
+    full_parity(cfg, 2, 1, T0)
+
+
+@pytest.mark.parametrize("delay,rebuild,cand", [(1, 0, 0), (8, 0, 3), (64, 3, 0), (16, 1, 40), (256, 0, 0)])
+def test_chain_independent_of_delay_rebuild_window(delay, rebuild, cand):
+    """Q18-Q20: delay, rebuild cadence and the candidate window are performance knobs only."""
+    cfg = get_config(1)
+    full_parity(cfg, 4, 10, T1, delay=delay, rebuild_every=rebuild, cand_window=cand)
+
+
+def test_sweep_calls_continue_the_chain():
+    cfg = get_config(1)
+    table = table_for(cfg)
+    pkg = _pkg()
+    seeds = walker_seeds(3, first=100)
+    a = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000)
+    a.reset(seeds)
+    for n in (1, 2, 3):
+        a.sweep(n)
+    b = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000)
+    b.reset(seeds)
+    b.sweep(6)
+    for w in range(3):
+        # block boundaries differ (a block ends with each sweep call), so R agrees to rounding only
+        compare_logs(a.get_log(w), b.get_log(w), f"split sweeps walker {w}")
+        compare_configs(a.get_config(w), b.get_config(w))
+        assert a.get_stats(w)["proposals"] == b.get_stats(w)["proposals"]
+
+
+def test_empty_start_and_tiny_cluster_edge_cases():
+    """Degenerate cases: empty initial configuration (removals on k=0 are rejected), 1x1 cluster."""
+    cfg = get_config(0)
+    full_parity(cfg, 3, 30, T0, init_k=0)
+    atom = dict(cfg, name="atom", Lx=1, Ly=1, mu=0.0)
+    full_parity(atom, 2, 30, T0, init_k=0)
+
+
+def test_set_state_resumes_an_oracle_chain():
+    """ctaux_set_state: continue on the device from a configuration produced by the oracle."""
+    cfg = get_config(1)
+    table = table_for(cfg)
+    o = OracleWalker.from_config(cfg, table, 9, T1)
+    o.reset(cfg["init_k"])
+    o.sweep(5)
+    c0, nid, p0 = o.config(), o.next_id, o.p
+    o.clear_log()
+    o.sweep(4)
+    W = _pkg().Walkers.from_config(cfg, table, n_walkers=1, log_capacity=2000)
+    W.set_state([9], [c0], [nid], [p0])
+    W.sweep(4)
+    compare_logs(W.get_log(0), o.log(), "resumed")
+    compare_configs(W.get_config(0), o.config(), "resumed")
+    compare_N(W, 0, o, "resumed")
+
+
+def test_capacity_error_is_loud():
+    cfg = get_config(1)
+    table = table_for(cfg)
+    pkg = _pkg()
+    W = pkg.Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table, delay=8, n_walkers=2,
+                    init_k=5, max_k=12)
+    W.reset(walker_seeds(2))
+    with pytest.raises(pkg.CtauxError) as ei:
+        W.sweep(50)
+    assert ei.value.code == -2
+
+
+@pytest.mark.slow
+def test_config4_prefix_T1():
+    """Config 4 (6x6, beta 20, k ~ 1100-1700): first 2 sweeps of 2 walkers against T1, N to 1e-10."""
+    cfg = get_config(3)
+    full_parity(cfg, 2, 2, T1)
