@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the B200-native CT-AUX walker hot path (contract: see DESIGN.md section 6).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4_6x6_b20] [--sweeps-per-step S]
+  python bench.py --impl reference ...     # the CPU oracle, as it stands, on the host cores
+
+A "step" is one pass of the whole hot path (S1..S5) over one batch of synthetic input:
+`ctaux_sweep(S)` for all walkers of the workload, S = rebuild_every sweeps, so that every step holds
+the S2 candidate GEMMs, the S3 proposal kernel, the S4 flushes and exactly one S5 rebuild.
+The default workload is BASELINE.json configs[3] (6x6 cluster, beta=20, U=6, 8 walkers, delay 64),
+the configuration the north_star's performance target is quoted on; all five configs are available
+through --config / --all-configs.  Inputs are synthetic (closed-form cluster G0, Philox streams).
+
+Prints ONE JSON line (rank 0).  No file under /root/reference is read.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from ctaux_workloads import CONFIGS, get_config, table_for, walker_seeds  # noqa: E402
+
+METRIC = "accepted vertex updates/sec per B200 (batched walkers)"
+UNIT = "updates/s"
+# FP64 peak used for the roofline: MEASURED_PEAKS.json holds no FP64 figure, so the rule of the
+# profiling guide is applied: measured bf16 dense peak x nominal ratio FP64 : bf16.
+NOMINAL_FP64_TFLOPS = 40.0    # NVIDIA B200 datasheet, FP64 (vector = tensor) per GPU
+NOMINAL_BF16_TFLOPS = 2250.0
+FALLBACK_BF16_TFLOPS = 1590.0
+FALLBACK_HBM_GBS = 6650.0
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            mp = json.load(f)
+        return dict(bf16=float(mp["bf16_tflops"]), bf16_sustained=float(mp.get("bf16_tflops_sustained", mp["bf16_tflops"])),
+                    hbm=float(mp["hbm_gbs"]), source="measured")
+    except Exception:
+        return dict(bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0, hbm=FALLBACK_HBM_GBS, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.rows = []
+        self._stop = threading.Event()
+        self._t = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm = sorted(float(r[0]) for r in self.rows)
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in self.rows), "reasons": sorted(reasons),
+                "samples": len(self.rows)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference): the oracle as it stands, never tuned.
+def oracle_sample(cfg, table, n_walkers, n_sweeps, mode_name="T1", first_seed=0):
+    """n_walkers chains (one per host thread), reset + n_sweeps sweeps each.  Returns
+    (accepted updates, proposals, seconds of the sweep loop, threads used)."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import ctaux_oracle as orc
+    mode = orc.T1 if mode_name == "T1" else orc.T0
+    walkers = []
+    for s in walker_seeds(n_walkers, first_seed):
+        w = orc.OracleWalker.from_config(cfg, table, int(s), mode)
+        w.reset(cfg["init_k"])
+        walkers.append(w)
+    threads = min(n_walkers, os.cpu_count() or 1)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(lambda w: w.sweep(n_sweeps), walkers))
+    dt = time.perf_counter() - t0
+    acc = sum(w.acc_ins + w.acc_rem for w in walkers)
+    props = sum(w.p for w in walkers)
+    return acc, props, dt, threads
+
+
+# sweeps of the bounded oracle sample per config (about 10-30 s of CPU work on 8 cores)
+ORACLE_SAMPLE_SWEEPS = {"cfg1_2x2_b2": 4000, "cfg2_2x2_b10": 300, "cfg3_4x4_b10": 40, "cfg4_6x6_b20": 3,
+                        "cfg5_6x6_b40": 1}
+
+
+def cpu_baseline(cfg, table):
+    cores = os.cpu_count() or 1
+    nw = cores
+    ns = ORACLE_SAMPLE_SWEEPS.get(cfg["name"], 1)
+    acc, props, dt, threads = oracle_sample(cfg, table, nw, ns)
+    return {"value": acc / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "proposals_per_s": props / dt,
+            "sample": f"oracle T1 (rank-1 updates, from-scratch inverse every sweep), {nw} walkers x first {ns} "
+                      f"sweep(s) from reset (init_k={cfg['init_k']}), one thread per walker, {dt:.1f} s"}
+
+
+def run_reference(args):
+    rank, world, local = dist_env()
+    if rank != 0:
+        return 0
+    cfg = get_config(args.config)
+    table = table_for(cfg)
+    cores = os.cpu_count() or 1
+    ns = max(1, ORACLE_SAMPLE_SWEEPS.get(cfg["name"], 1) // 4)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, table, cores, 1 if cfg["name"] in ("cfg4_6x6_b20", "cfg5_6x6_b40") else ns)
+    acc = props = 0
+    dt = 0.0
+    threads = cores
+    for step in range(args.steps):
+        a, p, t, threads = oracle_sample(cfg, table, cores, ns, first_seed=step * cores)
+        acc += a
+        props += p
+        dt += t
+    value = acc / dt
+    sample = (f"each step = {cores} oracle T1 walkers x first {ns} sweep(s) from reset, one thread per walker "
+              f"(bounded sample of {cfg['name']}: {cfg['n_walkers']} walkers x {cfg['sweeps']} sweeps)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "proposals_per_s": props / dt, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------
+def total_stats(W, n_walkers):
+    keys = ("proposals", "acc_ins", "acc_rem", "flops_cand", "flops_flush", "flops_usinv", "flops_rebuild",
+            "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds")
+    tot = {k: 0.0 for k in keys}
+    ks = []
+    for w in range(n_walkers):
+        st = W.get_stats(w)
+        for k in keys:
+            tot[k] += st[k]
+        ks.append(st["k"])
+    tot["k_mean"] = float(np.mean(ks))
+    return tot
+
+
+def diff(a, b):
+    return {k: a[k] - b[k] for k in a if k != "k_mean"}
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1901_01047_b200 import Walkers
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this package has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = get_config(args.config)
+    table = table_for(cfg)
+    B = args.walkers or cfg["n_walkers"]
+    delay = args.delay or cfg["delay"]
+    S = args.sweeps_per_step or cfg["rebuild_every"]
+    dev = f"cuda:{local}"
+    # replicas only: rank r runs its own walkers with disjoint seeds
+    seeds = walker_seeds(B, first=rank * B)
+    W = Walkers.from_config(cfg, table, n_walkers=B, delay=delay, rebuild_every=S, device=dev)
+    W.reset(seeds)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        W.sweep(S)
+    barrier()
+    W.timing_enable(True)
+    s0 = total_stats(W, B)
+    l0 = W.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(local) as clk:
+        ev[0].record(stream)
+        for i in range(args.steps):
+            W.sweep(S)
+            ev[i + 1].record(stream)
+        barrier()
+    ms_total = ev[0].elapsed_time(ev[-1])
+    s1 = total_stats(W, B)
+    l1 = W.launch_count()
+    tim = W.timing_get()
+    W.timing_enable(False)
+    d = diff(s1, s0)
+    acc = d["acc_ins"] + d["acc_rem"]
+
+    # max over ranks of the device time; sum over ranks of the work
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_max = float(t.item())
+        a = torch.tensor([acc, d["proposals"]], dtype=torch.float64, device=dev)
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+        acc_all, props_all = float(a[0].item()), float(a[1].item())
+    else:
+        ms_max, acc_all, props_all = ms_total, acc, d["proposals"]
+
+    out = None
+    if rank == 0:
+        peaks = measured_peaks()
+        fp64_peak = peaks["bf16_sustained"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS  # kernel timed inside a long step
+        fl = tim["flush_gemm"]
+        flush_tf = d["flops_flush"] / (fl["ms"] * 1e-3) / 1e12 if fl["ms"] > 0 else 0.0
+        per_launch_flops = d["flops_flush"] / max(fl["launches"], 1)
+        roofline = {"kernel": "gemm_grouped_kernel<DescFlush> (S4 rank-r flush, DMMA m8n8k4)", "bound": "tensor",
+                    "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak,
+                    "traffic": None,
+                    "peak_source": f"{peaks['source']} bf16 sustained {peaks['bf16_sustained']:.1f} TF x nominal FP64:bf16 "
+                                   f"{NOMINAL_FP64_TFLOPS:g}:{NOMINAL_BF16_TFLOPS:g}",
+                    "flops_per_launch": per_launch_flops, "ms_per_launch": fl["ms"] / max(fl["launches"], 1),
+                    "launches": fl["launches"], "mean_rank": d["sum_rank"] / max(d["flushes"], 1)}
+        steps_ms = {k: v["ms"] for k, v in tim.items()}
+        other = {"cand_gemm_tflops": d["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
+                 "rebuild_tflops": d["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}
+        out = {"metric": METRIC, "value": acc_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
+               "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
+                          "K": cfg["K"], "walkers_per_gpu": B, "delay": delay, "sweeps_per_step": S,
+                          "rebuild_every": S, "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
+                          "working set fits L2 (latency-bound chain; no flush between steps)",
+                          "parallelism": "replicas only"},
+               "proposals_per_s": props_all / (ms_max * 1e-3), "k_mean": s1["k_mean"],
+               "mean_k_over_proposals": d["sum_k"] / max(d["proposals"], 1),
+               "acceptance": acc / max(d["proposals"], 1),
+               "gpu_launches": int(l1 - l0), "roofline": roofline, "step_ms_by_class": steps_ms, "gemm": other}
+        out["clocks"] = clk.summary()
+    return W, cfg, table, out, (rank, world, local)
+
+
+def run_e2e(W, cfg, B, S, steps, rank):
+    """Same metric through the public API with HOST buffers: every step uploads the walkers' state
+    from host arrays (ctaux_set_state: configuration H2D + S1/S5), runs ctaux_sweep(S) and reads the
+    result back (ctaux_get_config + ctaux_get_N of every walker, D2H)."""
+    import torch
+    seeds = walker_seeds(B, first=rank * B)
+    cfgs = [W.get_config(w) for w in range(B)]
+    stats = [W.get_stats(w) for w in range(B)]
+    acc = 0
+    h2d = d2h = 0
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        W.set_state(seeds, cfgs, [s["next_id"] for s in stats], [s["proposals"] for s in stats])
+        h2d += sum(len(c["site"]) * (8 + 4 + 8 + 1) for c in cfgs) + 8 * B * 4
+        a0 = 0
+        W.sweep(S)
+        cfgs, new_stats = [], []
+        for w in range(B):
+            c = W.get_config(w)
+            cfgs.append(c)
+            st = W.get_stats(w)
+            new_stats.append(st)
+            acc += st["acc_ins"] + st["acc_rem"]      # counters restart at set_state
+            k = st["k"]
+            for s in range(2):
+                W.get_N(w, s)
+            d2h += k * (8 + 4 + 8 + 1) + 2 * k * k * 8
+        stats = new_stats
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    return {"value": acc / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d / steps), "d2h_bytes_per_step": int(d2h / steps),
+            "steps": steps, "ms_per_step": 1e3 * dt / steps,
+            "what": "ctaux_set_state(host arrays) + ctaux_sweep + ctaux_get_config/get_N to host, every step"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg4_6x6_b20", choices=[c["name"] for c in CONFIGS])
+    ap.add_argument("--walkers", type=int, default=0, help="walkers per GPU (default: the config's)")
+    ap.add_argument("--delay", type=int, default=0)
+    ap.add_argument("--sweeps-per-step", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
+    if args.impl == "reference":
+        return run_reference(args)
+    W, cfg, table, out, (rank, world, local) = run_gpu(args)
+    B = args.walkers or cfg["n_walkers"]
+    S = args.sweeps_per_step or cfg["rebuild_every"]
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(W, cfg, B, S, min(args.steps, 3), rank)
+        if world > 1:
+            import torch
+            import torch.distributed as dist
+            t = torch.tensor([e2e["value"]], dtype=torch.float64, device=f"cuda:{local}")
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            e2e["value"] = float(t.item())
+    if rank == 0:
+        out["e2e"] = e2e
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(cfg, table)
+        print(json.dumps(out))
+    W.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -86,10 +86,11 @@ typedef struct ctaux_stats {
   int32_t k;               /* current expansion order                                                 */
   int32_t sign;            /* sign of prod_sigma det A_sigma carried along the chain                  */
   double flops_cand;       /* S2: 2*m*k*k (rows) + 2*n*n*m (columns), both spins                      */
-  double flops_flush;      /* S4: 2*k'*k'*r + 2*k'*r*r, both spins                                    */
+  double flops_flush;      /* S4: 2*k'*k'*r (the rank-r update itself), both spins                    */
   double flops_rebuild;    /* S5: 2*k^3 per spin                                                      */
   double min_margin;       /* min over proposals of |u - |R|| / |R|  (near-tie diagnostic, Q22)       */
   double sum_k;            /* sum over proposals of k before the proposal (for <k>)                   */
+  double flops_usinv;      /* S4: 2*k'*r*r (U * S^-1), both spins                                     */
 } ctaux_stats;
 
 /* One entry of the decision log (48 bytes). */

@@ -35,7 +35,7 @@ class _Stats(C.Structure):
                 ("flushes", C.c_int64), ("rebuilds", C.c_int64), ("sum_rank", C.c_int64),
                 ("k", C.c_int32), ("sign", C.c_int32), ("flops_cand", C.c_double),
                 ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
-                ("min_margin", C.c_double), ("sum_k", C.c_double)]
+                ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double)]
 
 
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",

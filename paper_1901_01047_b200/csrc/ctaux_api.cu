@@ -643,7 +643,7 @@ int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   out->blocks = st.blocks; out->flushes = st.flushes; out->rebuilds = st.rebuilds; out->sum_rank = st.sum_rank;
   out->k = st.k; out->sign = st.sign;
   out->flops_cand = st.flops_cand; out->flops_flush = st.flops_flush; out->flops_rebuild = st.flops_rebuild;
-  out->min_margin = st.min_margin; out->sum_k = st.sum_k;
+  out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
   return CTAUX_OK;
 }
 

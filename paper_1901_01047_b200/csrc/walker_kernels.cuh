@@ -465,7 +465,8 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
     st.log_count = log_count;
     st.min_margin = min_margin; st.sum_k += sum_k;
     st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
-    st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r + 2.0 * (double)kcur * r * r);
+    st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);
+    st.flops_usinv += 2.0 * (2.0 * (double)kcur * r * r);
     if (status) st.status = status;
     if (finished || status) {
       st.active = 0;

@@ -41,7 +41,7 @@ struct WalkerState {
   int32_t pad0;
   // statistics
   int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count;
-  double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k;
+  double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k, flops_usinv;
 };
 
 // Everything a kernel needs: passed by value (fits the 4 KB parameter space easily).
