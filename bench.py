@@ -215,7 +215,8 @@ def run_gpu(args):
     dev = f"cuda:{local}"
     # replicas only: rank r runs its own walkers with disjoint seeds
     seeds = walker_seeds(B, first=rank * B)
-    W = Walkers.from_config(cfg, table, n_walkers=B, delay=delay, rebuild_every=S, device=dev)
+    W = Walkers.from_config(cfg, table, n_walkers=B, delay=delay, rebuild_every=S, device=dev,
+                            cand_window=args.cand_window)
     W.reset(seeds)
     stream = torch.cuda.current_stream()
 
@@ -336,6 +337,7 @@ def main():
     ap.add_argument("--walkers", type=int, default=0, help="walkers per GPU (default: the config's)")
     ap.add_argument("--delay", type=int, default=0)
     ap.add_argument("--sweeps-per-step", type=int, default=0)
+    ap.add_argument("--cand-window", type=int, default=0, help="insertion candidates pre-expanded per block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

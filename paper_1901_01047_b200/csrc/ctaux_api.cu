@@ -40,8 +40,8 @@ enum StepClass { C_PREP = 0, C_CAND_GEMM = 1, C_PROPOSE = 2, C_UV = 3, C_FLUSH_G
 // GEMM tile configurations
 //  big:   128x128x16, 8 warps (2x4), 4 stages  -- flush / candidate columns at large k
 //  small:  64x64x16,  4 warps... (kept at 8 warps: 2x4 -> warp tile 32x16)
-#define GEMM_BIG 128, 128, 2, 4, 4
-#define GEMM_SMALL 64, 64, 2, 4, 4
+#define GEMM_BIG 128, 64, 4, 2, 4, 2
+#define GEMM_SMALL 64, 64, 2, 4, 4, 2
 
 // ---- device-side problem descriptors ------------------------------------------------------
 struct DescCandRows {  // G1: N_ext[k:k+m, 0:k] = Bm (m x k) * N (k x k)
@@ -112,10 +112,10 @@ struct DescPlain {  // ctaux_dgemm
   __device__ bool operator()(int, GemmDesc& o) const { o = d; return true; }
 };
 
-template <int BM, int BN, int WM, int WN, int STAGES, class Fn>
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class Fn>
 cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s) {
   using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
-  auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, Fn>;
+  auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, MINB, Fn>;
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
@@ -295,7 +295,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
       if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
-      return launch_gemm<GEMM_BIG>(DescLU{d, j0, which}, ((Mmax + 127) / 128) * ((Nmax + 127) / 128), P, s);
+      return launch_gemm<GEMM_BIG>(DescLU{d, j0, which}, ((Mmax + 127) / 128) * ((Nmax + 63) / 64), P, s);
     };
     for (int j0 = 0; j0 < kmax; j0 += kLuNb) {  // factorisation + forward substitution
       Scoped t(x, C_REBUILD);
@@ -344,8 +344,8 @@ int enqueue_block_step(ctaux_ctx* x) {
       e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
       e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
-      e1 = launch_gemm<GEMM_BIG>(DescCandRows{d}, (d.mmax + 127) / 128 * ((d.max_k + 127) / 128), P, s);
-      e2 = launch_gemm<GEMM_BIG>(DescCandCols{d}, (d.cap + 127) / 128 * ((d.mmax + 127) / 128), P, s);
+      e1 = launch_gemm<GEMM_BIG>(DescCandRows{d}, (d.mmax + 127) / 128 * ((d.max_k + 63) / 64), P, s);
+      e2 = launch_gemm<GEMM_BIG>(DescCandCols{d}, (d.cap + 127) / 128 * ((d.mmax + 63) / 64), P, s);
     }
     CU_CHECK(e1); CU_CHECK(e2);
     tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
@@ -364,7 +364,7 @@ int enqueue_block_step(ctaux_ctx* x) {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
     if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
-    else e3 = launch_gemm<GEMM_BIG>(DescUSinv{d}, (d.max_k + 127) / 128 * ((d.delay + 127) / 128), P, s);
+    else e3 = launch_gemm<GEMM_BIG>(DescUSinv{d}, (d.max_k + 127) / 128 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
   }
@@ -375,8 +375,7 @@ int enqueue_block_step(ctaux_ctx* x) {
       const int tl = (d.max_k + 63) / 64;
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
-      const int tl = (d.max_k + 127) / 128;
-      e4 = launch_gemm<GEMM_BIG>(DescFlush{d}, tl * tl, P, s);
+      e4 = launch_gemm<GEMM_BIG>(DescFlush{d}, ((d.max_k + 127) / 128) * ((d.max_k + 63) / 64), P, s);
     }
     CU_CHECK(e4);
     tick(x, C_FLUSH_GEMM);
@@ -694,7 +693,7 @@ int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, con
   fn.d.A = A; fn.d.lda = lda; fn.d.B = B; fn.d.ldb = ldb; fn.d.C = C; fn.d.ldc = ldc;
   fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
   fn.d.alpha = alpha; fn.d.beta = beta;
-  const int tiles = ((M + 127) / 128) * ((N + 127) / 128);
+  const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
   CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream)));
   return CTAUX_OK;
 }

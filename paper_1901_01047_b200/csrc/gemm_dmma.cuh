@@ -76,12 +76,20 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
   const int m0 = tile_m * BM, n0 = tile_n * BN;
   const int M = d.M, N = d.N, K = d.K;
 
-  double acc[TM][TN][2];
+  // index maps of this thread's fragment rows / columns (C0 gather = compaction of the flush)
+  int crow[TM], srow[TM], ccol[TN][2], scol[TN][2];
 #pragma unroll
-  for (int i = 0; i < TM; ++i)
+  for (int i = 0; i < TM; ++i) {
+    crow[i] = m0 + wm * (TM * 8) + i * 8 + g;
+    srow[i] = (d.rowmap && crow[i] < M) ? d.rowmap[crow[i]] : crow[i];
+  }
 #pragma unroll
-    for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
+  for (int j = 0; j < TN; ++j)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      ccol[j][h] = n0 + wn * (TN * 8) + j * 8 + 2 * q + h;
+      scol[j][h] = (d.colmap && ccol[j][h] < N) ? d.colmap[ccol[j][h]] : ccol[j][h];
+    }
   const int nk = (K + BK - 1) / BK;
 
   auto load_stage = [&](int kt, int st) {
@@ -116,6 +124,42 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
     cp_async_commit();
   }
 
+  // Accumulators start from C0[gather] (scaled by beta/alpha when that is not 1): the loads are in
+  // flight while the pipeline fills and the epilogue is a pure store.  The common in-place update
+  // C = C0 - A*B (alpha = -1, beta = 1: flush, LU trailing updates) flips the sign bit of the A
+  // fragments instead, so the C0 values go straight into the accumulator registers.
+  const bool negA = (d.alpha == -1.0 && d.beta == 1.0);
+  const double alpha_eff = negA ? 1.0 : d.alpha;
+  double acc[TM][TN][2];
+  if (d.beta != 0.0) {
+    const double bscale = d.beta / alpha_eff;
+#pragma unroll
+    for (int j = 0; j < TN; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const double* c0col = d.C0 + (size_t)scol[j][h] * d.ldc0;
+        const bool cok = ccol[j][h] < N;
+#pragma unroll
+        for (int i = 0; i < TM; ++i) acc[i][j][h] = (cok && crow[i] < M) ? c0col[srow[i]] : 0.0;
+      }
+    if (bscale != 1.0) {
+#pragma unroll
+      for (int j = 0; j < TN; ++j)
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int i = 0; i < TM; ++i) acc[i][j][h] *= bscale;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < TN; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int i = 0; i < TM; ++i) acc[i][j][h] = 0.0;
+  }
+  const int sign_flip = negA ? (int)0x80000000 : 0;
+
   for (int kt = 0; kt < nk; ++kt) {
     cp_async_wait<STAGES - 2>();
     __syncthreads();
@@ -130,7 +174,10 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
     for (int k4 = 0; k4 < BK; k4 += 4) {
       double af[TM], bf[TN];
 #pragma unroll
-      for (int i = 0; i < TM; ++i) af[i] = a_s[(k4 + q) * LDA_S + i * 8];
+      for (int i = 0; i < TM; ++i) {
+        const double a = a_s[(k4 + q) * LDA_S + i * 8];
+        af[i] = __hiloint2double(__double2hiint(a) ^ sign_flip, __double2loint(a));
+      }
 #pragma unroll
       for (int j = 0; j < TN; ++j) bf[j] = b_s[j * 8 * LDB_S + k4 + q];
 #pragma unroll
@@ -142,33 +189,22 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
   cp_async_wait<0>();
 
   // epilogue: thread holds C[row = g][cols 2q, 2q+1] of every 8x8 fragment
-  const double alpha = d.alpha, beta = d.beta;
 #pragma unroll
-  for (int j = 0; j < TN; ++j) {
+  for (int j = 0; j < TN; ++j)
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const int col = n0 + wn * (TN * 8) + j * 8 + 2 * q + h;
-      if (col >= N) continue;
-      const int scol = d.colmap ? d.colmap[col] : col;
+      if (ccol[j][h] >= N) continue;
+      double* ccolp = d.C + (size_t)ccol[j][h] * d.ldc;
 #pragma unroll
-      for (int i = 0; i < TM; ++i) {
-        const int row = m0 + wm * (TM * 8) + i * 8 + g;
-        if (row >= M) continue;
-        double v = alpha * acc[i][j][h];
-        if (beta != 0.0) {
-          const int srow = d.rowmap ? d.rowmap[row] : row;
-          v += beta * d.C0[(size_t)scol * d.ldc0 + srow];
-        }
-        d.C[(size_t)col * d.ldc + row] = v;
-      }
+      for (int i = 0; i < TM; ++i)
+        if (crow[i] < M) ccolp[crow[i]] = (alpha_eff == 1.0) ? acc[i][j][h] : alpha_eff * acc[i][j][h];
     }
-  }
 }
 
 // Grouped launch: blockIdx.y = problem, blockIdx.x = tile (tiles beyond the problem's own
 // count exit).  DescFn(problem) -> GemmDesc, evaluated on the device.
-template <int BM, int BN, int WM, int WN, int STAGES, class DescFn>
-__global__ void __launch_bounds__(WM * WN * 32, 1) gemm_grouped_kernel(DescFn fn) {
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class DescFn>
+__global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn fn) {
   extern __shared__ __align__(16) double smem_gemm[];
   GemmDesc d;
   if (!fn(blockIdx.y, d)) return;

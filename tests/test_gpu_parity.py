@@ -63,10 +63,14 @@ def test_reset_builds_inverse(ci, nw):
         compare_configs(W.get_config(w), o.config(), f"reset walker {w}")
         compare_N(W, w, o, f"reset walker {w}")
         assert W.get_stats(w)["sign"] == o.sign
-        # P7 on the device matrix itself: N A = 1
+        # P7 on the device matrix itself: A N = 1.  A's columns carry the factors E_j (up to e^gamma),
+        # so the residual is taken on the column-equilibrated matrix A D^-1 (D N is its inverse).
         for s in range(2):
             k = o.k
-            assert np.linalg.norm(W.get_N(w, s) @ o.A(s) - np.eye(k)) / np.sqrt(k) < 1e-10
+            A = o.A(s)
+            dcol = np.abs(A).max(axis=0)
+            res = (A / dcol) @ (dcol[:, None] * W.get_N(w, s)) - np.eye(k)
+            assert np.linalg.norm(res) / np.sqrt(k) < 1e-10
 
 
 def test_config1_full_lockstep_T0():
