@@ -180,7 +180,7 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------
 def total_stats(W, n_walkers):
     keys = ("proposals", "acc_ins", "acc_rem", "flops_cand", "flops_flush", "flops_usinv", "flops_rebuild",
-            "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds")
+            "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds", "guard_ends")
     tot = {k: 0.0 for k in keys}
     ks = []
     for w in range(n_walkers):
@@ -286,6 +286,7 @@ def run_gpu(args):
                "proposals_per_s": props_all / (ms_max * 1e-3), "k_mean": s1["k_mean"],
                "mean_k_over_proposals": d["sum_k"] / max(d["proposals"], 1),
                "acceptance": acc / max(d["proposals"], 1),
+               "blocks": int(d["blocks"]), "guard_ends": int(d["guard_ends"]),
                "gpu_launches": int(l1 - l0), "roofline": roofline, "step_ms_by_class": steps_ms, "gemm": other}
         out["clocks"] = clk.summary()
     return W, cfg, table, out, (rank, world, local)

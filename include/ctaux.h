@@ -71,6 +71,15 @@ typedef struct ctaux_params {
   void* workspace;         /* DEVICE pointer, caller-owned                                            */
   size_t workspace_bytes;
   void* stream;            /* cudaStream_t                                                            */
+  double guard_amp;        /* numerical guard of the delayed block: a block is
+                              flushed BEFORE a proposal whose bordered ratio evaluation would amplify
+                              rounding errors by more than guard_amp (cancellation in
+                              s_nn - s_row S^-1 s_col, times the error level S^-1 already carries);
+                              the proposal is then evaluated from the freshly updated N.  This
+                              happens when A is nearly singular (e.g. while thermalising from the
+                              random initial configuration).  0 = library default (100: ends ~1.5% of
+                              the blocks early in equilibrium); < 0 or inf = off.  Chain-neutral: only where blocks
+                              end.                                                                    */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */
@@ -91,6 +100,7 @@ typedef struct ctaux_stats {
   double min_margin;       /* min over proposals of |u - |R|| / |R|  (near-tie diagnostic, Q22)       */
   double sum_k;            /* sum over proposals of k before the proposal (for <k>)                   */
   double flops_usinv;      /* S4: 2*k'*r*r (U * S^-1), both spins                                     */
+  int64_t guard_ends;      /* blocks ended early by the numerical guard (ctaux_params.guard_amp)      */
 } ctaux_stats;
 
 /* One entry of the decision log (48 bytes). */
@@ -168,6 +178,13 @@ const char* ctaux_last_cuda_error(void);
  * For measurement and tests. */
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
                 int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc);
+
+/* Same, with the tile kernel chosen explicitly: 0 = 128x64 tile kernel, 1 = 64x64 tile kernel (the
+ * two kernels of the small-k configurations), 2 / 3 = persistent kernel (large-k configurations), 128x64 /
+ * 64x128 tiles, k-step 16 x 4 stages; 4 / 5 = the same with k-step 32 x 3 stages.  Lets the tests reach every GEMM path. */
+int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
+                   int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc,
+                   int32_t kernel);
 
 /* Debug / pin helper: Philox4x32-10 evaluated ON THE DEVICE for n (counter, key) pairs.
  * ctr: HOST [n][4], key: HOST [n][2], out: HOST [n][4]. */

@@ -26,7 +26,7 @@ class _Params(C.Structure):
                 ("delay", C.c_int32), ("n_walkers", C.c_int32), ("init_k", C.c_int32),
                 ("max_k", C.c_int32), ("rebuild_every", C.c_int32), ("log_capacity", C.c_int32),
                 ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
-                ("stream", C.c_void_p)]
+                ("stream", C.c_void_p), ("guard_amp", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -35,13 +35,14 @@ class _Stats(C.Structure):
                 ("flushes", C.c_int64), ("rebuilds", C.c_int64), ("sum_rank", C.c_int64),
                 ("k", C.c_int32), ("sign", C.c_int32), ("flops_cand", C.c_double),
                 ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
-                ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double)]
+                ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double),
+                ("guard_ends", C.c_int64)]
 
 
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_rebuild", "ctaux_get_config", "ctaux_get_N", "ctaux_get_N_device", "ctaux_get_stats",
            "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
-           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_debug_philox"]
+           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_dgemm_ex", "ctaux_debug_philox"]
 
 _lib = None
 
@@ -83,6 +84,7 @@ def load_library():
     L.ctaux_strerror.argtypes = [C.c_int]
     L.ctaux_last_cuda_error.restype = C.c_char_p
     L.ctaux_dgemm.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32]
+    L.ctaux_dgemm_ex.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32]
     L.ctaux_debug_philox.argtypes = [vp, vp, vp, i32]
     _lib = L
     return L
@@ -106,7 +108,8 @@ class Walkers:
     """B batched CT-AUX walkers on one GPU (ctaux_create / reset / sweep / get_*)."""
 
     def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
-                 rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None):
+                 rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None,
+                 guard_amp=0.0):
         import torch
         if not torch.cuda.is_available():
             raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
@@ -123,6 +126,7 @@ class Walkers:
         p.g0_table = table.ctypes.data
         p.delay, p.n_walkers, p.init_k, p.max_k = delay, n_walkers, init_k, max_k
         p.rebuild_every, p.log_capacity, p.cand_window = rebuild_every, log_capacity, cand_window
+        p.guard_amp = guard_amp
         nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
         if nbytes == 0:
             raise CtauxError(-1, "ctaux_workspace_bytes", "invalid parameters")
@@ -255,7 +259,7 @@ def colmajor(rows, cols, device="cuda", fill=None, generator=None):
     return store[:, :rows].t()
 
 
-def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None):
+def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, kernel=0):
     """C = beta*C + alpha*A@B through the library's DMMA tile kernel.  A (M x K), B (K x N), C (M x N)
     are torch float64 CUDA tensors stored column-major (stride(0) == 1) with even leading dimensions
     (see colmajor())."""
@@ -270,8 +274,8 @@ def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None):
         assert t.shape[0] <= 1 or t.stride(0) == 1, "column-major operands required"
     ld = lambda t: int(t.stride(1)) if t.shape[1] > 1 else max(2, t.shape[0] + (t.shape[0] & 1))
     s = stream if stream is not None else torch.cuda.current_stream(A.device)
-    _check(L.ctaux_dgemm(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
-                         C_out.data_ptr(), ld(C_out)), "ctaux_dgemm")
+    _check(L.ctaux_dgemm_ex(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
+                            C_out.data_ptr(), ld(C_out), kernel), "ctaux_dgemm_ex")
     return C_out
 
 

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "gemm_dmma.cuh"
+#include "gemm_persist.cuh"
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
 
@@ -113,7 +114,7 @@ struct DescPlain {  // ctaux_dgemm
 };
 
 template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class Fn>
-cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s) {
+cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s, int pf_dist = 0) {
   using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
   auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, MINB, Fn>;
   static bool configured = false;
@@ -123,8 +124,47 @@ cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s)
     configured = true;
   }
   if (tiles_x < 1) tiles_x = 1;
-  kern<<<dim3(tiles_x, problems), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(fn);
+  kern<<<dim3(tiles_x, problems), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(fn, pf_dist);
   return cudaGetLastError();
+}
+
+// persistent kernel (large k): descriptor adaptor that fixes the tile orientation
+template <class F, int WIDE>
+struct PAdapt {
+  F f;
+  __device__ bool operator()(int p, GemmDesc& d, int& wide) const { wide = WIDE; return f(p, d); }
+};
+
+int sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  }
+  return n;
+}
+
+#ifndef CTAUX_PBK
+#define CTAUX_PBK 16
+#define CTAUX_PSTAGES 4
+#endif
+template <int WIDE, int BK, int STAGES, class F>
+cudaError_t launch_persist_cfg(const F& f, int problems, cudaStream_t s) {
+  using Fn = PAdapt<F, WIDE>;
+  auto kern = gemm_persistent_kernel<BK, STAGES, Fn>;
+  constexpr int smem = PCfg<BK, STAGES>::SMEM_BYTES;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  kern<<<sm_count(), kPThreads, smem, s>>>(Fn{f}, problems);
+  return cudaGetLastError();
+}
+template <int WIDE, class F>
+cudaError_t launch_persist(const F& f, int problems, cudaStream_t s) {
+  return launch_persist_cfg<WIDE, CTAUX_PBK, CTAUX_PSTAGES>(f, problems, s);
 }
 
 }  // namespace
@@ -142,6 +182,7 @@ struct ctaux_ctx {
   bool sinv_smem;
   int propose_smem;
   bool small_tiles;
+  bool persist;       // large k and few problems: persistent GEMM kernel (gemm_persist.cuh)
   // timing
   bool timing;
   std::vector<cudaEvent_t> ev_pool;
@@ -183,6 +224,8 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   const double ch = 1.0 + p->U * p->beta * (double)d.Nc / (2.0 * p->K);
   d.egp = ch + sqrt(ch * ch - 1.0);
   d.egm = 1.0 / d.egp;
+  const double ga = p->guard_amp;
+  d.guard_amp = (ga == 0.0) ? 1e2 : ((ga < 0.0 || !(ga < 1e300)) ? 1e308 : ga);
   return true;
 }
 
@@ -294,6 +337,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
+      if (x->persist) return launch_persist<0>(DescLU{d, j0, which}, P, s);
       if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
       return launch_gemm<GEMM_BIG>(DescLU{d, j0, which}, ((Mmax + 127) / 128) * ((Nmax + 63) / 64), P, s);
     };
@@ -340,7 +384,10 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_CAND_GEMM);
     cudaError_t e1, e2;
-    if (x->small_tiles) {
+    if (x->persist) {
+      e1 = launch_persist<1>(DescCandRows{d}, P, s);
+      e2 = launch_persist<0>(DescCandCols{d}, P, s);
+    } else if (x->small_tiles) {
       e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
       e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
@@ -363,7 +410,8 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
-    if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    if (x->persist) e3 = launch_persist<0>(DescUSinv{d}, P, s);
+    else if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
     else e3 = launch_gemm<GEMM_BIG>(DescUSinv{d}, (d.max_k + 127) / 128 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
@@ -371,7 +419,9 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_FLUSH_GEMM);
     cudaError_t e4;
-    if (x->small_tiles) {
+    if (x->persist) {
+      e4 = launch_persist<0>(DescFlush{d}, P, s);
+    } else if (x->small_tiles) {
       const int tl = (d.max_k + 63) / 64;
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
@@ -499,6 +549,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     return CTAUX_ECUDA;
   }
   x->small_tiles = d.max_k <= 512;
+  // The persistent kernel (gemm_persist.cuh) hides the C0 latency of the flush but its main loop is slower
+  // than two independent 8-warp CTAs per SM (profiles/r1_gemm_variants.md); off until that is fixed.
+  x->persist = false && !x->small_tiles && 2 * d.B <= kPMaxProblems;
   *out = x;
   return CTAUX_OK;
 }
@@ -643,6 +696,7 @@ int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   out->k = st.k; out->sign = st.sign;
   out->flops_cand = st.flops_cand; out->flops_flush = st.flops_flush; out->flops_rebuild = st.flops_rebuild;
   out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
+  out->guard_ends = st.guard_ends;
   return CTAUX_OK;
 }
 
@@ -683,6 +737,12 @@ int ctaux_timing_get(ctaux_ctx* x, double* ms, int64_t* launches) {
 
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
                 const double* B, int32_t ldb, double beta, double* C, int32_t ldc) {
+  return ctaux_dgemm_ex(stream, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, 0);
+}
+
+int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
+                   const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel) {
+  if (kernel < 0 || kernel > 10) return CTAUX_EINVAL;
   if (M < 0 || N < 0 || K < 0 || !C || ldc < M) return CTAUX_EINVAL;
   if (K > 0 && (!A || !B || lda < M || ldb < K || (lda & 1) || (ldb & 1) || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)))
     return CTAUX_EINVAL;
@@ -693,8 +753,33 @@ int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, con
   fn.d.A = A; fn.d.lda = lda; fn.d.B = B; fn.d.ldb = ldb; fn.d.C = C; fn.d.ldc = ldc;
   fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
   fn.d.alpha = alpha; fn.d.beta = beta;
-  const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
-  CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream)));
+  if (kernel == 0) {
+    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
+    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream)));
+  } else if (kernel == 1) {
+    const int tiles = ((M + 63) / 64) * ((N + 63) / 64);
+    CU_CHECK((launch_gemm<GEMM_SMALL>(fn, tiles, 1, (cudaStream_t)stream)));
+  } else if (kernel == 9) {
+    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
+    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream, 2 * sm_count())));
+  } else if (kernel == 10) {
+    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
+    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream, 4 * sm_count())));
+  } else if (kernel == 7) {
+    CU_CHECK((launch_gemm<128, 128, 4, 4, 3, 1>(fn, ((M + 127) / 128) * ((N + 127) / 128), 1, (cudaStream_t)stream)));
+  } else if (kernel == 8) {
+    CU_CHECK((launch_gemm<128, 128, 4, 4, 4, 1>(fn, ((M + 127) / 128) * ((N + 127) / 128), 1, (cudaStream_t)stream)));
+  } else if (kernel == 6) {
+    CU_CHECK((launch_gemm<GEMM_BIG>(fn, 2 * sm_count(), 1, (cudaStream_t)stream)));
+  } else if (kernel == 2) {
+    CU_CHECK((launch_persist_cfg<0, 16, 4>(fn, 1, (cudaStream_t)stream)));
+  } else if (kernel == 3) {
+    CU_CHECK((launch_persist_cfg<1, 16, 4>(fn, 1, (cudaStream_t)stream)));
+  } else if (kernel == 4) {
+    CU_CHECK((launch_persist_cfg<0, 32, 3>(fn, 1, (cudaStream_t)stream)));
+  } else {
+    CU_CHECK((launch_persist_cfg<1, 32, 3>(fn, 1, (cudaStream_t)stream)));
+  }
   return CTAUX_OK;
 }
 

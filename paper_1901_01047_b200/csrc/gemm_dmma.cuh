@@ -201,10 +201,29 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
     }
 }
 
+// L2 prefetch of the beta*C0[gather] tile that will run in this SM slot a wave later.  The flush is an
+// in-place-style rank-r update (K = r <= 64): each tile reads 64 KB of N from HBM for ~1 MFLOP, so the
+// C0 gather sits on the critical path of every CTA; pulling the lines into L2 one wave ahead turns
+// those loads into L2 hits (rank-k_s update; 16 n^2 bytes per 2 n^2 r flops).
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
+template <int BM, int BN, int THREADS>
+__device__ __forceinline__ void prefetch_c0_tile(const GemmDesc& d, int tile_m, int tile_n) {
+  const int m0 = tile_m * BM, n0 = tile_n * BN;
+  constexpr int RG = BM / 16;   // one 128-byte line = 16 doubles
+  for (int idx = threadIdx.x; idx < BN * RG; idx += THREADS) {
+    const int col = n0 + idx / RG, row = m0 + (idx % RG) * 16;
+    if (col >= d.N || row >= d.M) continue;
+    const int sr = d.rowmap ? __ldg(d.rowmap + row) : row;
+    const int sc = d.colmap ? __ldg(d.colmap + col) : col;
+    prefetch_l2(d.C0 + (size_t)sc * d.ldc0 + sr);
+  }
+}
+
 // Grouped launch: blockIdx.y = problem, blockIdx.x = tile (tiles beyond the problem's own
 // count exit).  DescFn(problem) -> GemmDesc, evaluated on the device.
 template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class DescFn>
-__global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn fn) {
+__global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn fn, int pf_dist) {
   extern __shared__ __align__(16) double smem_gemm[];
   GemmDesc d;
   if (!fn(blockIdx.y, d)) return;
@@ -212,6 +231,19 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn
   const int tm = (d.M + BM - 1) / BM, tn = (d.N + BN - 1) / BN;
   // persistent over the tiles of this problem: grid.x CTAs stride over tm*tn tiles
   for (int t = blockIdx.x; t < tm * tn; t += gridDim.x) {
+    if (d.beta != 0.0 && pf_dist > 0) {
+      int t2 = t + pf_dist;
+      if (t2 < tm * tn) {
+        prefetch_c0_tile<BM, BN, WM * WN * 32>(d, t2 % tm, t2 / tm);
+      } else if (blockIdx.y + 1 < gridDim.y) {
+        GemmDesc d2;
+        t2 -= tm * tn;
+        if (fn(blockIdx.y + 1, d2) && d2.M > 0 && d2.N > 0 && d2.beta != 0.0) {
+          const int tm2 = (d2.M + BM - 1) / BM, tn2 = (d2.N + BN - 1) / BN;
+          if (t2 < tm2 * tn2) prefetch_c0_tile<BM, BN, WM * WN * 32>(d2, t2 % tm2, t2 / tm2);
+        }
+      }
+    }
     gemm_tile<BM, BN, WM, WN, STAGES>(d, t % tm, t / tm, smem_gemm);
     __syncthreads();
   }

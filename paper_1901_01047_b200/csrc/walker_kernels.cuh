@@ -212,7 +212,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.srow = o; o += 2 * delay * 8;
   L.tv = o; o += 2 * delay * 8;
   L.tpv = o; o += 2 * delay * 8;
-  L.red = o; o += 2 * 8 * 8;
+  L.red = o; o += 2 * 2 * 8 * 8;
   L.snn = o; o += 2 * 8;
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
   double* srow = reinterpret_cast<double*>(smraw + L.srow) + sp * c.delay;
   double* tv = reinterpret_cast<double*>(smraw + L.tv) + sp * c.delay;
   double* tpv = reinterpret_cast<double*>(smraw + L.tpv) + sp * c.delay;
-  double* red = reinterpret_cast<double*>(smraw + L.red);   // [2][8]
+  double* red = reinterpret_cast<double*>(smraw + L.red);   // [2][8] dot products, [2][8] sums of magnitudes
   double* snn = reinterpret_cast<double*>(smraw + L.snn);   // [2]
   PropInfo* prop = reinterpret_cast<PropInfo*>(smraw + L.prop);
   int* live = reinterpret_cast<int*>(smraw + L.live0);
@@ -280,6 +280,8 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
   double min_margin = st.min_margin, sum_k = 0.0;
   int64_t log_count = st.log_count;
   bool finished = false;
+  int guard_end = 0;
+  double errlvl = 1.0;  // rounding-error level of S^-1 in units of eps (largest amplification accepted so far)
 
   for (int i = 0; i < win; ++i) {
     if (props_left == 0) {
@@ -300,7 +302,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       pref = (double)kcur / c.K;
     }
     bool accept = false;
-    double R = 0.0, stil_own = 1.0;
+    double R = 0.0, stil_own = 1.0, amp = 1.0;
     // removal of a vertex inserted earlier in this block: the two changes of that slot cancel, so
     // the buffered insertion is taken OUT of the block (exact treatment of a twice-touched spin,
     // PAPER.md:228): ratio = (S^-1)_aa / dE_a, then S^-1 is downdated.
@@ -324,9 +326,14 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
         scol[a] = X(ja, slot);
         srow[a] = X(slot, ja);
       }
-      if (lt == 0) snn[sp] = 1.0 / dE_own + X(slot, slot);
+      if (lt == 0) {
+        // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
+        // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
+        if (slot < k0) snn[sp] = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
+        else snn[sp] = 1.0 / dE_own + X(slot, slot);
+      }
       __syncthreads();
-      double part = 0.0;
+      double part = 0.0, apart = 0.0;
       for (int a = lt; a < r; a += kGroup) {
         double t = 0.0, tp = 0.0;
         for (int b = 0; b < r; ++b) {
@@ -336,14 +343,31 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
         tv[a] = t;
         tpv[a] = tp;
         part += srow[a] * t;
+        apart += fabs(srow[a] * t);
       }
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-      if ((tid & 31) == 0) red[sp * 8 + (lt >> 5)] = part;
+      for (int o = 16; o > 0; o >>= 1) {
+        part += __shfl_xor_sync(0xffffffffu, part, o);
+        apart += __shfl_xor_sync(0xffffffffu, apart, o);
+      }
+      if ((tid & 31) == 0) { red[sp * 8 + (lt >> 5)] = part; red[16 + sp * 8 + (lt >> 5)] = apart; }
       __syncthreads();
       const double dot0 = (red[0] + red[1]) + (red[2] + red[3]);
       const double dot1 = (red[8] + red[9]) + (red[10] + red[11]);
       const double stil0 = snn[0] - dot0, stil1 = snn[1] - dot1;
+      // Numerical guard (ctaux_params.guard_amp): the bordered evaluation s_nn - s_row S^-1 s_col
+      // amplifies rounding errors by amp = (|s_nn| + sum |s_row_a t_a|) / |result|, on top of the error
+      // level S^-1 already carries.  When that product exceeds the guard the block is flushed BEFORE
+      // this proposal, which is then evaluated first thing in the next block straight from the
+      // updated N (r = 0: no bordering).  Chain-neutral: only where blocks end.
+      {
+        const double ad0 = (red[16] + red[17]) + (red[18] + red[19]);
+        const double ad1 = (red[24] + red[25]) + (red[26] + red[27]);
+        const double amp0 = (fabs(snn[0]) + ad0) / fmax(fabs(stil0), 1e-300);
+        const double amp1 = (fabs(snn[1]) + ad1) / fmax(fabs(stil1), 1e-300);
+        amp = fmax(amp0, amp1);
+        if (r > 0 && amp * errlvl > c.guard_amp) { guard_end = 1; break; }
+      }
       stil_own = sp == 0 ? stil0 : stil1;
       R = pref * ((dE0 * stil0) * (dE1 * stil1));
       accept = pi.u < fabs(R);
@@ -412,6 +436,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       }
       if (lt == 0) Sv[r + (size_t)r * lds] = inv;
       if (tid == 0) Js[r] = slot;
+      errlvl = fmax(errlvl, amp);
       if (type == 0) {
         if (tid == 0) { live[len] = slot; c.cfg_id[off_old + slot] = next_id; jpos[slot - k0] = r; }
         ++len; ++kcur; ++next_id; ++acc_ins;
@@ -461,6 +486,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
     st.sweeps_left = sweeps_left; st.props_left = props_left;
     st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
     st.blocks += 1;
+    st.guard_ends += guard_end;
     if (r > 0) { st.flushes += 1; st.sum_rank += r; }
     st.log_count = log_count;
     st.min_margin = min_margin; st.sum_k += sum_k;

@@ -40,7 +40,7 @@ struct WalkerState {
   int32_t active;  // 1 while the walker still has proposals to do in this sweep call
   int32_t pad0;
   // statistics
-  int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count;
+  int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count, guard_ends;
   double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k, flops_usinv;
 };
 
@@ -54,6 +54,7 @@ struct DevCtx {
   int ldr;   // leading dimension of Vt / Sinv in global memory (delay rounded up to 8)
   int log_capacity;
   double beta, K, tau_scale, egp, egm, g00;
+  double guard_amp;  // rounding-amplification limit of the bordered ratio evaluation (k_propose)
   const double* table;  // [Nc][M+1]
   WalkerState* ws;      // [B]
   // configuration, double buffered, extended slots: [B][2][cap]

@@ -14,9 +14,13 @@ EXACT_FIELDS = ("p", "type", "arg", "tau", "spin", "accepted", "u")
 # Logged ratios come from different arithmetic (Woodbury block on the device, determinants or
 # rank-1 formulas in the oracle).  A ratio is a difference of O(1) terms, so its ABSOLUTE error is
 # what the arithmetic bounds; tiny |R| (near-singular A', always rejected by a wide margin) carry a
-# large relative error on both sides.  DESIGN.md "tolerances".
-R_RTOL = 1e-7
-R_ATOL = 1e-10
+# large relative error on both sides.  The device evaluates R from an N that has drifted for up to
+# rebuild_every sweeps and is allowed a relative error of 1e-10 (the bar below); the entries of N
+# enter R multiplied by factors up to (e^gamma - 1)^2 * prefactor, so R cannot be held tighter than
+# ~100x the N bar.  R is a diagnostic: the BIT-EXACT field is the decision `accepted`.
+# DESIGN.md section 5 "tolerances".
+R_RTOL = 1e-6
+R_ATOL = 1e-8
 N_FROB_TOL = 1e-10     # BASELINE.json north_star: relative Frobenius error of N
 
 
@@ -73,7 +77,7 @@ def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
 
 
 def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, init_k=None, seeds=None,
-                check_N=True, cand_window=0, max_k=None):
+                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL):
     """reset + n_sweeps on both sides, compare logs, configurations, N, sign, counters."""
     from paper_1901_01047_b200 import Walkers
     table = table_for(cfg)
@@ -98,6 +102,69 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
         assert st["sign"] == o.sign and st["acc_ins"] == o.acc_ins and st["acc_rem"] == o.acc_rem, what
         assert st["sweeps"] == n_sweeps, what
         if check_N:
-            errs = compare_N(W, w, o, what)
+            errs = compare_N(W, w, o, what, tol=n_tol)
             worst = max([worst] + errs)
+    return W, orcs, worst
+
+
+def load_thermalised(name, seed=0):
+    """tests/golden/thermalised_<name>_seed<seed>.txt (written by make_thermalised.py from the ORACLE
+    only): returns (config dict in list order, next_id, p)."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"thermalised_{name}_seed{seed}.txt")
+    meta, rows = {}, []
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#"):
+                _, key, val = line.split()
+                meta[key] = val
+            elif line.strip():
+                i, s, t, sp = line.split()
+                rows.append((int(i), int(s), float.fromhex(t), int(sp)))
+    assert len(rows) == int(meta["k"])
+    cfg = dict(id=np.array([r[0] for r in rows], np.uint64), site=np.array([r[1] for r in rows], np.int32),
+               tau=np.array([r[2] for r in rows], np.float64), spin=np.array([r[3] for r in rows], np.int8))
+    return cfg, int(meta["next_id"]), int(meta["p"])
+
+
+def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay=None, tol=N_FROB_TOL, **kw):
+    """Both sides start from the SAME given configuration (a thermalised, well-conditioned one), each
+    walker with its own seed; no rebuild on the device, so N is the incrementally updated matrix after
+    n_sweeps sweeps (or the oracle runs n_proposals single proposals and the device log is compared on
+    that prefix).  Logs / configurations bit-exact, N within tol."""
+    from paper_1901_01047_b200 import Walkers
+    table = table_for(cfg)
+    c0, next_id, p0 = state
+    nw = len(seeds)
+    cap = int(max(n_sweeps, 1) * max(cfg["max_k"], 16) + 64)
+    W = Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table,
+                delay=cfg["delay"] if delay is None else delay, n_walkers=nw, init_k=0, max_k=cfg["max_k"],
+                rebuild_every=0, log_capacity=cap, **kw)
+    W.set_state(seeds, [c0] * nw, [next_id] * nw, [p0] * nw)
+
+    def one(seed):
+        o = OracleWalker.from_config(cfg, table, int(seed), mode)
+        o.set_state(c0["site"], c0["tau"], c0["spin"], c0["id"], next_id, p0)
+        if n_proposals is None:
+            o.sweep(n_sweeps)
+        else:
+            o.propose(n_proposals)
+        return o
+
+    with ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as ex2:
+        orcs_f = [ex2.submit(one, s) for s in seeds]
+        W.sweep(n_sweeps)
+        orcs = [f.result() for f in orcs_f]
+    worst = 0.0
+    for w, o in enumerate(orcs):
+        what = f"{cfg['name']} thermalised, walker seed {int(seeds[w])}"
+        ol = o.log()
+        dl = W.get_log(w)
+        if n_proposals is not None:
+            dl = dl[:len(ol)]
+        compare_logs(dl, ol, what)
+        if n_proposals is None:
+            compare_configs(W.get_config(w), o.config(), what)
+            st = W.get_stats(w)
+            assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id, what
+            worst = max([worst] + compare_N(W, w, o, what, tol=tol))
     return W, orcs, worst

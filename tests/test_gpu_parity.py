@@ -7,7 +7,14 @@ import pytest
 from ctaux_workloads import get_config, table_for, walker_seeds
 from oracle.ctaux_oracle import T0, T1, OracleWalker, philox
 
-from parity_helpers import compare_configs, compare_logs, compare_N, frob_rel, full_parity, run_oracle
+from parity_helpers import (compare_configs, compare_logs, compare_N, frob_rel, full_parity, load_thermalised,
+                            parity_from_state, run_oracle)
+
+# N while THERMALISING from the random initial configuration (Q17): A is nearly singular there
+# (cond ~ 1e6), and even plain rank-1 updates drift to ~1e-9 within a few sweeps without a rebuild
+# (DESIGN.md section 5).  Decisions and configurations stay bit-exact; N is held to 1e-10 from a
+# thermalised start (test_*_thermalised_*) and after every rebuild.
+N_TOL_THERMALISING = 5e-8
 
 pytestmark = pytest.mark.gpu
 
@@ -29,10 +36,17 @@ def test_P12_device_philox_equals_oracle_philox():
         assert dev[i].tolist() == philox(ctr[i], key[i]).tolist()
 
 
-@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (8, 8, 4), (130, 70, 33), (128, 128, 64), (257, 511, 100),
-                                   (1000, 40, 1000), (64, 1000, 7), (300, 300, 0)])
-def test_dgemm_tiles_against_torch_fp64(M, N, K):
-    """The DMMA tile kernel (several tiles + ragged tails) against torch's FP64 matmul."""
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("M,N,K,alpha,beta", [(1, 1, 1, -1.5, 0.5), (8, 8, 4, -1.5, 0.5), (130, 70, 33, -1.5, 0.5),
+                                              (128, 128, 64, -1.0, 1.0), (257, 511, 100, -1.5, 0.5),
+                                              (1000, 40, 1000, 1.0, 0.0), (64, 1000, 7, -1.0, 1.0),
+                                              (300, 300, 0, 2.0, 0.5), (1900, 1834, 64, -1.0, 1.0),
+                                              (64, 1834, 1834, 1.0, 0.0), (1898, 64, 1898, 1.0, 0.0),
+                                              (700, 900, 129, 1.0, 1.0)])
+def test_dgemm_tiles_against_torch_fp64(M, N, K, alpha, beta, kernel):
+    """Every DMMA GEMM path (0/1: tile kernels of the small configs, 2/3: persistent kernel in both
+    tile orientations; several tiles, several K chunks, ragged tails, the in-place C0 - A*B form)
+    against torch's FP64 matmul."""
     import torch
     pkg = _pkg()
     g = torch.Generator(device="cpu").manual_seed(M * 7 + N * 3 + K)
@@ -42,8 +56,8 @@ def test_dgemm_tiles_against_torch_fp64(M, N, K):
     C0 = pkg.colmajor(M, N, fill=rnd)
     C = pkg.colmajor(M, N)
     C.copy_(C0)
-    out = pkg.ctaux_dgemm(A, B, C, alpha=-1.5, beta=0.5)
-    ref = 0.5 * C0 - 1.5 * (A @ B)
+    out = pkg.ctaux_dgemm(A, B, C, alpha=alpha, beta=beta, kernel=kernel)
+    ref = beta * C0 + alpha * (A @ B)
     torch.cuda.synchronize()
     scale = float(ref.abs().max()) + 1e-300
     assert float((out - ref).abs().max()) / scale < 1e-13 * max(K, 1)
@@ -88,8 +102,17 @@ def test_config2_batched_walkers_T0_prefix_and_T1():
 
 def test_config3_T1():
     cfg = get_config(2)
-    full_parity(cfg, 64, 6, T1)
-    full_parity(cfg, 2, 1, T0)
+    full_parity(cfg, 64, 6, T1, n_tol=N_TOL_THERMALISING)
+    full_parity(cfg, 64, 10, T1)          # ends on the config's rebuild cadence: N fresh from S5
+    full_parity(cfg, 2, 1, T0, n_tol=N_TOL_THERMALISING)
+
+
+def test_config3_thermalised_start_N_1e10():
+    """Config 3 from the oracle-thermalised configuration (40 sweeps), 16 seeds, 8 sweeps WITHOUT any
+    rebuild on the device: the incrementally updated N (about 65 flushes of rank <= 32) within 1e-10."""
+    cfg = get_config(2)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(16), 8, T1)
+    assert sum(W.get_stats(w)["flushes"] for w in range(16)) > 500
 
 
 @pytest.mark.parametrize("delay,rebuild,cand", [(1, 0, 0), (8, 0, 3), (64, 3, 0), (16, 1, 40), (256, 0, 0)])
@@ -158,6 +181,14 @@ def test_capacity_error_is_loud():
 
 @pytest.mark.slow
 def test_config4_prefix_T1():
-    """Config 4 (6x6, beta 20, k ~ 1100-1700): first 2 sweeps of 2 walkers against T1, N to 1e-10."""
+    """Config 4 (6x6, beta 20) from reset, k ~ 1100-1300: first 2 sweeps of 2 walkers against T1."""
     cfg = get_config(3)
-    full_parity(cfg, 2, 2, T1)
+    full_parity(cfg, 2, 2, T1, n_tol=N_TOL_THERMALISING)
+
+
+@pytest.mark.slow
+def test_config4_thermalised_start_N_1e10():
+    """Config 4 at its full size (k ~ 1720, delay 64, the launch configuration bench.py times) from the
+    oracle-thermalised configuration: 4 seeds x 1 sweep without rebuild, logs bit-exact, N within 1e-10."""
+    cfg = get_config(3)
+    parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(4), 1, T1)
