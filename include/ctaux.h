@@ -179,9 +179,11 @@ const char* ctaux_last_cuda_error(void);
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
                 int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc);
 
-/* Same, with the tile kernel chosen explicitly: 0 = 128x64 tile kernel, 1 = 64x64 tile kernel (the
- * two kernels of the small-k configurations), 2 / 3 = persistent kernel (large-k configurations), 128x64 /
- * 64x128 tiles, k-step 16 x 4 stages; 4 / 5 = the same with k-step 32 x 3 stages.  Lets the tests reach every GEMM path. */
+/* Same, with the kernel chosen explicitly, so that tests and measurements reach every GEMM path:
+ * 0 = 128x64 tiles, 8 warps, 2 CTAs/SM;  1 = 64x64 tiles, 8 warps (small-k configurations);
+ * 2/3 = persistent kernel, 128x64 / 64x128 tiles, k-step 16 x 4 stages; 4/5 = same, k-step 32 x 3;
+ * 6 = 64x64 tiles, 4 warps, 4 CTAs/SM (S2, S5 at large k);  7 = same at 5 CTAs/SM (S4 flush);
+ * 8 = kernel 6 with L2 prefetch of the next-wave C0 tile. */
 int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
                    int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc,
                    int32_t kernel);

@@ -43,6 +43,11 @@ enum StepClass { C_PREP = 0, C_CAND_GEMM = 1, C_PROPOSE = 2, C_UV = 3, C_FLUSH_G
 //  small:  64x64x16,  4 warps... (kept at 8 warps: 2x4 -> warp tile 32x16)
 #define GEMM_BIG 128, 64, 4, 2, 4, 2
 #define GEMM_SMALL 64, 64, 2, 4, 4, 2
+// large k: 64x64 tiles, 4 warps with 32x32 warp tiles, 2 stages, 4-5 INDEPENDENT CTAs per SM: while one CTA
+// waits for its C0 gather / operands or drains its stores, the others keep the DMMA pipe busy
+// (rank-64 flush: 23.0 TFLOP/s against 18.2 for 2 CTAs of 8 warps; profiles/r1_gemm_variants.md)
+#define GEMM_Q4 64, 64, 2, 2, 2, 4
+#define GEMM_Q5 64, 64, 2, 2, 2, 5
 
 // ---- device-side problem descriptors ------------------------------------------------------
 struct DescCandRows {  // G1: N_ext[k:k+m, 0:k] = Bm (m x k) * N (k x k)
@@ -207,7 +212,9 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   memset(&d, 0, sizeof(d));
   d.B = p->n_walkers; d.Lx = p->Lx; d.Ly = p->Ly; d.Nc = p->Lx * p->Ly; d.M = p->n_tau;
   d.max_k = p->max_k; d.delay = p->delay;
-  int mmax = p->cand_window > 0 ? p->cand_window : (p->delay + p->delay / 4 + 8);
+  // candidates pre-expanded per block: about delay / (2 * acceptance * 1/2) = delay at the ~50 % acceptance of the
+  // paper-shaped workloads; kept a multiple of the 64-row GEMM tile for the large-delay configurations
+  int mmax = p->cand_window > 0 ? p->cand_window : (p->delay >= 64 ? p->delay : p->delay + p->delay / 4 + 8);
   if (mmax > 480) mmax = 480;
   d.mmax = mmax;
   int winmax = 3 * mmax + 16;
@@ -339,7 +346,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
       tick(x, C_REBUILD);
       if (x->persist) return launch_persist<0>(DescLU{d, j0, which}, P, s);
       if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
-      return launch_gemm<GEMM_BIG>(DescLU{d, j0, which}, ((Mmax + 127) / 128) * ((Nmax + 63) / 64), P, s);
+      return launch_gemm<GEMM_Q4>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
     };
     for (int j0 = 0; j0 < kmax; j0 += kLuNb) {  // factorisation + forward substitution
       Scoped t(x, C_REBUILD);
@@ -391,8 +398,8 @@ int enqueue_block_step(ctaux_ctx* x) {
       e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
       e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
-      e1 = launch_gemm<GEMM_BIG>(DescCandRows{d}, (d.mmax + 127) / 128 * ((d.max_k + 63) / 64), P, s);
-      e2 = launch_gemm<GEMM_BIG>(DescCandCols{d}, (d.cap + 127) / 128 * ((d.mmax + 63) / 64), P, s);
+      e1 = launch_gemm<GEMM_Q4>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
+      e2 = launch_gemm<GEMM_Q4>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     }
     CU_CHECK(e1); CU_CHECK(e2);
     tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
@@ -412,7 +419,7 @@ int enqueue_block_step(ctaux_ctx* x) {
     cudaError_t e3;
     if (x->persist) e3 = launch_persist<0>(DescUSinv{d}, P, s);
     else if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
-    else e3 = launch_gemm<GEMM_BIG>(DescUSinv{d}, (d.max_k + 127) / 128 * ((d.delay + 63) / 64), P, s);
+    else e3 = launch_gemm<GEMM_Q4>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
   }
@@ -425,7 +432,8 @@ int enqueue_block_step(ctaux_ctx* x) {
       const int tl = (d.max_k + 63) / 64;
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
-      e4 = launch_gemm<GEMM_BIG>(DescFlush{d}, ((d.max_k + 127) / 128) * ((d.max_k + 63) / 64), P, s);
+      const int tl = (d.max_k + 63) / 64;
+      e4 = launch_gemm<GEMM_Q5>(DescFlush{d}, tl * tl, P, s);  // L2 prefetch of C0 measured: no gain
     }
     CU_CHECK(e4);
     tick(x, C_FLUSH_GEMM);
@@ -742,7 +750,7 @@ int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, con
 
 int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
                    const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel) {
-  if (kernel < 0 || kernel > 10) return CTAUX_EINVAL;
+  if (kernel < 0 || kernel > 8) return CTAUX_EINVAL;
   if (M < 0 || N < 0 || K < 0 || !C || ldc < M) return CTAUX_EINVAL;
   if (K > 0 && (!A || !B || lda < M || ldb < K || (lda & 1) || (ldb & 1) || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)))
     return CTAUX_EINVAL;
@@ -753,33 +761,21 @@ int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, 
   fn.d.A = A; fn.d.lda = lda; fn.d.B = B; fn.d.ldb = ldb; fn.d.C = C; fn.d.ldc = ldc;
   fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
   fn.d.alpha = alpha; fn.d.beta = beta;
-  if (kernel == 0) {
-    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
-    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream)));
-  } else if (kernel == 1) {
-    const int tiles = ((M + 63) / 64) * ((N + 63) / 64);
-    CU_CHECK((launch_gemm<GEMM_SMALL>(fn, tiles, 1, (cudaStream_t)stream)));
-  } else if (kernel == 9) {
-    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
-    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream, 2 * sm_count())));
-  } else if (kernel == 10) {
-    const int tiles = ((M + 127) / 128) * ((N + 63) / 64);
-    CU_CHECK((launch_gemm<GEMM_BIG>(fn, tiles, 1, (cudaStream_t)stream, 4 * sm_count())));
-  } else if (kernel == 7) {
-    CU_CHECK((launch_gemm<128, 128, 4, 4, 3, 1>(fn, ((M + 127) / 128) * ((N + 127) / 128), 1, (cudaStream_t)stream)));
-  } else if (kernel == 8) {
-    CU_CHECK((launch_gemm<128, 128, 4, 4, 4, 1>(fn, ((M + 127) / 128) * ((N + 127) / 128), 1, (cudaStream_t)stream)));
-  } else if (kernel == 6) {
-    CU_CHECK((launch_gemm<GEMM_BIG>(fn, 2 * sm_count(), 1, (cudaStream_t)stream)));
-  } else if (kernel == 2) {
-    CU_CHECK((launch_persist_cfg<0, 16, 4>(fn, 1, (cudaStream_t)stream)));
-  } else if (kernel == 3) {
-    CU_CHECK((launch_persist_cfg<1, 16, 4>(fn, 1, (cudaStream_t)stream)));
-  } else if (kernel == 4) {
-    CU_CHECK((launch_persist_cfg<0, 32, 3>(fn, 1, (cudaStream_t)stream)));
-  } else {
-    CU_CHECK((launch_persist_cfg<1, 32, 3>(fn, 1, (cudaStream_t)stream)));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int t64 = ((M + 63) / 64) * ((N + 63) / 64);
+  cudaError_t e;
+  switch (kernel) {
+    case 0: e = launch_gemm<GEMM_BIG>(fn, ((M + 127) / 128) * ((N + 63) / 64), 1, st); break;
+    case 1: e = launch_gemm<GEMM_SMALL>(fn, t64, 1, st); break;
+    case 2: e = launch_persist_cfg<0, 16, 4>(fn, 1, st); break;
+    case 3: e = launch_persist_cfg<1, 16, 4>(fn, 1, st); break;
+    case 4: e = launch_persist_cfg<0, 32, 3>(fn, 1, st); break;
+    case 5: e = launch_persist_cfg<1, 32, 3>(fn, 1, st); break;
+    case 6: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st); break;
+    case 7: e = launch_gemm<GEMM_Q5>(fn, t64, 1, st); break;
+    default: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st, 4 * sm_count()); break;  // 8: with L2 prefetch of C0
   }
+  CU_CHECK(e);
   return CTAUX_OK;
 }
 

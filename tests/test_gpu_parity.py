@@ -36,7 +36,7 @@ def test_P12_device_philox_equals_oracle_philox():
         assert dev[i].tolist() == philox(ctr[i], key[i]).tolist()
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("M,N,K,alpha,beta", [(1, 1, 1, -1.5, 0.5), (8, 8, 4, -1.5, 0.5), (130, 70, 33, -1.5, 0.5),
                                               (128, 128, 64, -1.0, 1.0), (257, 511, 100, -1.5, 0.5),
                                               (1000, 40, 1000, 1.0, 0.0), (64, 1000, 7, -1.0, 1.0),
