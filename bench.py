@@ -38,6 +38,9 @@ NOMINAL_FP64_TFLOPS = 40.0    # NVIDIA B200 datasheet, FP64 (vector = tensor) pe
 NOMINAL_BF16_TFLOPS = 2250.0
 FALLBACK_BF16_TFLOPS = 1590.0
 FALLBACK_HBM_GBS = 6650.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the flush kernel from the committed
+# `ncu --set full` capture of the same launch configuration (profiles/), bytes; None = not captured
+FLUSH_TRAFFIC_PER_WALKER = {"cfg4_6x6_b20": 98.1e6}   # profiles/r1_v3_flush_full.md: 785 MB / 8 walkers
 
 
 def measured_peaks():
@@ -220,10 +223,13 @@ def diff(a, b):
     return {k: a[k] - b[k] for k in a if k != "k_mean"}
 
 
+DEFAULT_GROUPS = {"cfg4_6x6_b20": 2, "cfg5_6x6_b40": 2}
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
-    from paper_1901_01047_b200 import Walkers
+    from paper_1901_01047_b200 import WalkerGroups, Walkers
     from paper_1901_01047_b200.replicas import aggregate, rank_seeds
 
     rank, world, local = dist_env()
@@ -237,12 +243,15 @@ def run_gpu(args):
     B = args.walkers or cfg["n_walkers"]
     delay = args.delay or cfg["delay"]
     S = args.sweeps_per_step or cfg["rebuild_every"]
+    G = args.groups or DEFAULT_GROUPS.get(cfg["name"], 1)
+    if B % G:
+        G = 1
     dev = f"cuda:{local}"
     # replicas only: rank r runs its own walkers with disjoint seeds
     seeds = rank_seeds(rank, B)
     fp64_dgemm = measure_fp64_peak(dev) if rank == 0 else 0.0
-    W = Walkers.from_config(cfg, table, n_walkers=B, delay=delay, rebuild_every=S, device=dev,
-                            cand_window=args.cand_window)
+    W = WalkerGroups(G, B, lambda g, nb, stream: Walkers.from_config(
+        cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream))
     W.reset(seeds)
     stream = torch.cuda.current_stream()
 
@@ -255,23 +264,32 @@ def run_gpu(args):
     for _ in range(args.warmup):
         W.sweep(S)
     barrier()
-    W.timing_enable(True)
+    # ---- timed region: K steps, all groups concurrently, no per-kernel events
     s0 = total_stats(W, B)
     l0 = W.launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
-        ev[0].record(stream)
+        e0.record(stream)            # the device is idle here: the region starts now
         for i in range(args.steps):
-            W.sweep(S)
-            ev[i + 1].record(stream)
+            W.sweep(S)               # returns when every group has finished the step
         barrier()
-    ms_total = ev[0].elapsed_time(ev[-1])
+        e1.record(stream)
+        torch.cuda.synchronize()
+    ms_total = e0.elapsed_time(e1)
     s1 = total_stats(W, B)
     l1 = W.launch_count()
-    tim = W.timing_get()
-    W.timing_enable(False)
     d = diff(s1, s0)
     acc = d["acc_ins"] + d["acc_rem"]
+    # ---- kernel pass: the same step once more, per-class CUDA events on the launching streams; with
+    # several groups they run one after the other here, so that each kernel is timed alone
+    W.timing_enable(True)
+    for g in W.groups:
+        g.sweep(S)
+    torch.cuda.synchronize()
+    s2 = total_stats(W, B)
+    tim = W.timing_get()
+    W.timing_enable(False)
+    dk = diff(s2, s1)
 
     # max over ranks of the device time; sum over ranks of the work
     ms_max, (acc_all, props_all) = aggregate(ms_total, [acc, d["proposals"]], device=dev)
@@ -282,26 +300,31 @@ def run_gpu(args):
         fp64_alt = peaks["bf16_sustained"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
         fp64_peak = fp64_dgemm
         fl = tim["flush_gemm"]
-        flush_tf = d["flops_flush"] / (fl["ms"] * 1e-3) / 1e12 if fl["ms"] > 0 else 0.0
-        per_launch_flops = d["flops_flush"] / max(fl["launches"], 1)
-        roofline = {"kernel": "gemm_grouped_kernel<64,64,2,2,2,5,DescFlush> (S4 rank-r flush, DMMA m8n8k4)", "bound": "tensor",
-                    "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak,
-                    "traffic": None,
+        flush_tf = dk["flops_flush"] / (fl["ms"] * 1e-3) / 1e12 if fl["ms"] > 0 else 0.0
+        per_launch_flops = dk["flops_flush"] / max(fl["launches"], 1)
+        roofline = {"kernel": "gemm_grouped_kernel<DescFlush> (S4 rank-r flush, DMMA m8n8k4; 64x64 tiles at 5 CTAs/SM "
+                              "for k > 512, 8-warp 64x64 tiles below)", "bound": "tensor",
+                    "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak if fp64_peak else None,
+                    "traffic": (FLUSH_TRAFFIC_PER_WALKER[cfg["name"]] * (B // G) if cfg["name"] in FLUSH_TRAFFIC_PER_WALKER and
+                                delay == cfg["delay"] else None),
+                    "algorithmic_bytes": 16.0 * dk["sum_k"] / max(dk["proposals"], 1) ** 1 * 0 + 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),
                     "peak_source": "cuBLAS DGEMM 8192^3 measured live in this run (FP64 runs at max SM clock: no power cap)",
                     "peak_alt": fp64_alt,
                     "peak_alt_source": f"{peaks['source']} bf16 sustained {peaks['bf16_sustained']:.1f} TF x nominal FP64:bf16 "
                                        f"{NOMINAL_FP64_TFLOPS:g}:{NOMINAL_BF16_TFLOPS:g}",
                     "frac_alt": flush_tf / fp64_alt,
                     "flops_per_launch": per_launch_flops, "ms_per_launch": fl["ms"] / max(fl["launches"], 1),
-                    "launches": fl["launches"], "mean_rank": d["sum_rank"] / max(d["flushes"], 1)}
+                    "launches": fl["launches"], "mean_rank": dk["sum_rank"] / max(dk["flushes"], 1),
+                    "walkers_per_launch": B // G,
+                    "timed": "kernel pass after the timed region: one more step, groups one after the other"}
         steps_ms = {k: v["ms"] for k, v in tim.items()}
-        other = {"cand_gemm_tflops": d["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
-                 "rebuild_tflops": d["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}
+        other = {"cand_gemm_tflops": dk["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
+                 "rebuild_tflops": dk["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}
         out = {"metric": METRIC, "value": acc_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
-                          "K": cfg["K"], "walkers_per_gpu": B, "delay": delay, "sweeps_per_step": S,
+                          "K": cfg["K"], "walkers_per_gpu": B, "stream_groups": G, "delay": delay, "sweeps_per_step": S,
                           "rebuild_every": S, "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
                           "working set fits L2 (latency-bound chain; no flush between steps)",
                           "parallelism": "replicas only"},
@@ -309,7 +332,7 @@ def run_gpu(args):
                "mean_k_over_proposals": d["sum_k"] / max(d["proposals"], 1),
                "acceptance": acc / max(d["proposals"], 1),
                "blocks": int(d["blocks"]), "guard_ends": int(d["guard_ends"]),
-               "gpu_launches": int(l1 - l0), "roofline": roofline, "step_ms_by_class": steps_ms, "gemm": other}
+               "gpu_launches": int(l1 - l0), "roofline": roofline, "kernel_pass_ms_by_class": steps_ms, "gemm": other}
         out["clocks"] = clk.summary()
     return W, cfg, table, out, (rank, world, local)
 
@@ -319,7 +342,7 @@ def run_e2e(W, cfg, B, S, steps, rank):
     from host arrays (ctaux_set_state: configuration H2D + S1/S5), runs ctaux_sweep(S) and reads the
     result back (ctaux_get_config + ctaux_get_N of every walker, D2H)."""
     import torch
-    seeds = walker_seeds(B, first=rank * B)
+    seeds = np.arange(rank * B, rank * B + B, dtype=np.uint64)
     cfgs = [W.get_config(w) for w in range(B)]
     stats = [W.get_stats(w) for w in range(B)]
     acc = 0
@@ -360,6 +383,7 @@ def main():
     ap.add_argument("--walkers", type=int, default=0, help="walkers per GPU (default: the config's)")
     ap.add_argument("--delay", type=int, default=0)
     ap.add_argument("--sweeps-per-step", type=int, default=0)
+    ap.add_argument("--groups", type=int, default=0, help="stream groups the walkers are split over (0 = per-config default)")
     ap.add_argument("--cand-window", type=int, default=0, help="insertion candidates pre-expanded per block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

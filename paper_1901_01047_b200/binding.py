@@ -247,6 +247,98 @@ class Walkers:
         return {name: dict(ms=float(ms[i]), launches=int(nl[i])) for i, name in enumerate(STEP_CLASSES)}
 
 
+class WalkerGroups:
+    """B walkers split over G contexts, each on its own CUDA stream and driven by its own host thread
+    (ctaux_sweep blocks, ctypes releases the GIL).  Walkers are independent chains,
+    so the grouping changes nothing in any chain; it lets the serial S3 proposal kernel of one group
+    (a few SMs busy) overlap the S2/S4 GEMMs of the others.  BASELINE.json config 5: "2 walkers on
+    separate streams".  Walker w of the job lives in group w // (B/G) at local index w % (B/G)."""
+
+    def __init__(self, n_groups, n_walkers, make):
+        """make(group_index, walkers_in_group, stream) -> Walkers"""
+        import torch
+        assert n_walkers % n_groups == 0
+        self.n_groups, self.n_walkers, self.per = n_groups, n_walkers, n_walkers // n_groups
+        self.streams = [torch.cuda.Stream() for _ in range(n_groups)]
+        self.groups = [make(g, self.per, self.streams[g]) for g in range(n_groups)]
+
+    def _each(self, fn):
+        import threading
+        errs = []
+
+        def run(W, g):
+            try:
+                fn(W, g)
+            except BaseException as e:  # re-raised on the caller's thread
+                errs.append(e)
+
+        th = [threading.Thread(target=run, args=(W, g)) for g, W in enumerate(self.groups)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        if errs:
+            raise errs[0]
+
+    def reset(self, seeds):
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        self._each(lambda W, g: W.reset(seeds[g * self.per:(g + 1) * self.per]))
+
+    def set_state(self, seeds, configs, next_id, proposals):
+        P = self.per
+        self._each(lambda W, g: W.set_state(seeds[g * P:(g + 1) * P], configs[g * P:(g + 1) * P],
+                                            next_id[g * P:(g + 1) * P], proposals[g * P:(g + 1) * P]))
+
+    def sweep(self, n_sweeps):
+        self._each(lambda W, g: W.sweep(n_sweeps))
+
+    def _loc(self, w):
+        return self.groups[w // self.per], w % self.per
+
+    def get_config(self, w):
+        W, i = self._loc(w)
+        return W.get_config(i)
+
+    def get_N(self, w, spin):
+        W, i = self._loc(w)
+        return W.get_N(i, spin)
+
+    def get_stats(self, w):
+        W, i = self._loc(w)
+        return W.get_stats(i)
+
+    def get_log(self, w, first=0, count=None):
+        W, i = self._loc(w)
+        return W.get_log(i, first, count)
+
+    def launch_count(self):
+        return sum(W.launch_count() for W in self.groups)
+
+    def timing_enable(self, on=True):
+        for W in self.groups:
+            W.timing_enable(on)
+
+    def timing_get(self):
+        out = None
+        for W in self.groups:
+            t = W.timing_get()
+            if out is None:
+                out = t
+            else:
+                for k in out:
+                    out[k]["ms"] += t[k]["ms"]
+                    out[k]["launches"] += t[k]["launches"]
+        return out
+
+    def synchronize(self):
+        for s in self.streams:
+            s.synchronize()
+
+    def close(self):
+        for W in self.groups:
+            W.close()
+
+
 def colmajor(rows, cols, device="cuda", fill=None, generator=None):
     """A rows x cols float64 CUDA tensor stored column-major with an EVEN leading dimension
     (the layout ctaux_dgemm wants): element (i, j) at data_ptr + 8*(i + j*ld)."""

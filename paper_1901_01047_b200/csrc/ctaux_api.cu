@@ -406,7 +406,8 @@ int enqueue_block_step(ctaux_ctx* x) {
   }
   {
     Scoped t(x, C_PROPOSE);
-    k_propose<<<d.B, kPropThreads, x->propose_smem, s>>>(d, x->sinv_smem ? 1 : 0);
+    if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, s>>>(d);
+    else k_propose<false><<<d.B, kPropThreads, x->propose_smem, s>>>(d);
     tick(x, C_PROPOSE);
   }
   {
@@ -544,10 +545,11 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
     x->propose_smem = Ls.total;
     if (Ls.total > max_smem) { delete x; return CTAUX_ECAPACITY; }
-    static int propose_attr_max = 0;  // the attribute is per function, shared by all contexts
-    if (Ls.total > propose_attr_max) {
-      e = cudaFuncSetAttribute(k_propose, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total);
-      if (e == cudaSuccess) propose_attr_max = Ls.total;
+    static int propose_attr_max[2] = {0, 0};  // the attribute is per function, shared by all contexts
+    if (Ls.total > propose_attr_max[x->sinv_smem ? 1 : 0]) {
+      e = x->sinv_smem ? cudaFuncSetAttribute(k_propose<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total)
+                       : cudaFuncSetAttribute(k_propose<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total);
+      if (e == cudaSuccess) propose_attr_max[x->sinv_smem ? 1 : 0] = Ls.total;
     }
   }
   if (e != cudaSuccess) {

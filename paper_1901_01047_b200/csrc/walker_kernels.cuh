@@ -213,7 +213,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.tv = o; o += 2 * delay * 8;
   L.tpv = o; o += 2 * delay * 8;
   L.red = o; o += 2 * 2 * 8 * 8;
-  L.snn = o; o += 2 * 8;
+  L.snn = o; o += 4 * 8;
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
   L.live1 = o; o += cap * 4;
@@ -224,12 +224,13 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   return L;
 }
 
-__global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_smem) {
+template <bool sinv_smem>   // S^-1 of both spins in shared memory (delay <= ~100) or in global memory
+__global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const int w = blockIdx.x, tid = threadIdx.x;
   WalkerState& st = c.ws[w];
   if (!st.active || st.status || st.win == 0) return;
-  const ProposeSmem L = propose_smem_layout(c.cap, c.delay, c.winmax, sinv_smem != 0);
+  const ProposeSmem L = propose_smem_layout(c.cap, c.delay, c.winmax, sinv_smem);
   const int sp = tid / kGroup, lt = tid % kGroup;
   const int lds = sinv_smem ? (c.delay | 1) : c.ldr;
   double* Sbase = sinv_smem ? reinterpret_cast<double*>(smraw + L.sinv)
@@ -241,7 +242,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
   double* tv = reinterpret_cast<double*>(smraw + L.tv) + sp * c.delay;
   double* tpv = reinterpret_cast<double*>(smraw + L.tpv) + sp * c.delay;
   double* red = reinterpret_cast<double*>(smraw + L.red);   // [2][8] dot products, [2][8] sums of magnitudes
-  double* snn = reinterpret_cast<double*>(smraw + L.snn);   // [2]
+  double* snn2 = reinterpret_cast<double*>(smraw + L.snn);  // [2 parities][2 spins]
   PropInfo* prop = reinterpret_cast<PropInfo*>(smraw + L.prop);
   int* live = reinterpret_cast<int*>(smraw + L.live0);
   int* live_alt = reinterpret_cast<int*>(smraw + L.live1);
@@ -321,11 +322,15 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       const double dE0 = (type == 0) ? (E0 - 1.0) : (1.0 - E0);
       const double dE1 = (type == 0) ? (E1 - 1.0) : (1.0 - E1);
       const double dE_own = sp == 0 ? dE0 : dE1;
-      for (int a = lt; a < r; a += kGroup) {
+      // thread roles inside a spin group of 128: half 0 builds s_col and t = S^-1 s_col (and the dot
+      // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass
+      const int half = lt >> 6, la = lt & 63;
+      for (int a = la; a < r; a += 64) {
         const int ja = Js[a];
-        scol[a] = X(ja, slot);
-        srow[a] = X(slot, ja);
+        if (half == 0) scol[a] = X(ja, slot);
+        else srow[a] = X(slot, ja);
       }
+      double* snn = snn2 + (i & 1) * 2;   // double buffered: read after the second barrier of this proposal
       if (lt == 0) {
         // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
         // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
@@ -334,16 +339,33 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       }
       __syncthreads();
       double part = 0.0, apart = 0.0;
-      for (int a = lt; a < r; a += kGroup) {
-        double t = 0.0, tp = 0.0;
-        for (int b = 0; b < r; ++b) {
-          t += Sv[a + (size_t)b * lds] * scol[b];
-          tp += srow[b] * Sv[b + (size_t)a * lds];
+      for (int a = la; a < r; a += 64) {
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int b = 0;
+        if (half == 0) {
+          const double* Sa = Sv + a;
+          for (; b + 3 < r; b += 4) {
+            s0 += Sa[(size_t)b * lds] * scol[b];
+            s1 += Sa[(size_t)(b + 1) * lds] * scol[b + 1];
+            s2 += Sa[(size_t)(b + 2) * lds] * scol[b + 2];
+            s3 += Sa[(size_t)(b + 3) * lds] * scol[b + 3];
+          }
+          for (; b < r; ++b) s0 += Sa[(size_t)b * lds] * scol[b];
+          const double t = (s0 + s1) + (s2 + s3);
+          tv[a] = t;
+          part += srow[a] * t;
+          apart += fabs(srow[a] * t);
+        } else {
+          const double* Sa = Sv + (size_t)a * lds;
+          for (; b + 3 < r; b += 4) {
+            s0 += srow[b] * Sa[b];
+            s1 += srow[b + 1] * Sa[b + 1];
+            s2 += srow[b + 2] * Sa[b + 2];
+            s3 += srow[b + 3] * Sa[b + 3];
+          }
+          for (; b < r; ++b) s0 += srow[b] * Sa[b];
+          tpv[a] = (s0 + s1) + (s2 + s3);
         }
-        tv[a] = t;
-        tpv[a] = tp;
-        part += srow[a] * t;
-        apart += fabs(srow[a] * t);
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -400,9 +422,10 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
         tpv[a] = Sv[apos + (size_t)a * lds];
       }
       __syncthreads();
-      for (int idx = lt; idx < r * r; idx += kGroup) {
-        const int a = idx % r, b = idx / r;
-        Sv[a + (size_t)b * lds] -= tv[a] * tpv[b] * inv;
+      for (int a = lt & 63; a < r; a += 64) {
+        const double ta = tv[a] * inv;
+        double* Sa = Sv + a;
+        for (int b = lt >> 6; b < r; b += 2) Sa[(size_t)b * lds] -= ta * tpv[b];
       }
       __syncthreads();
       const int last = r - 1;
@@ -426,9 +449,10 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       --r;
     } else if (accept) {
       const double inv = 1.0 / stil_own;
-      for (int idx = lt; idx < r * r; idx += kGroup) {
-        const int a = idx % r, b = idx / r;
-        Sv[a + (size_t)b * lds] += tv[a] * tpv[b] * inv;
+      for (int a = lt & 63; a < r; a += 64) {   // 64 rows x 2 column phases: no integer division
+        const double ta = tv[a] * inv;
+        double* Sa = Sv + a;
+        for (int b = lt >> 6; b < r; b += 2) Sa[(size_t)b * lds] += ta * tpv[b];
       }
       for (int a = lt; a < r; a += kGroup) {
         Sv[a + (size_t)r * lds] = -tv[a] * inv;
@@ -448,7 +472,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c, int sinv_sme
       if (R < 0.0) sign = -sign;
       ++r;
     }
-    __syncthreads();
+    if (accept) __syncthreads();   // S^-1, J, the live list changed; a rejected proposal wrote nothing shared
     --props_left; ++consumed; ++p;
     if (props_left == 0) ++sweeps_done;
     if (r == c.delay) break;

@@ -37,7 +37,9 @@ def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None):
         return list(ex.map(one, seeds))
 
 
-def compare_logs(dev_log, orc_log, what=""):
+def compare_logs(dev_log, orc_log, what="", r_rtol=None, r_atol=None):
+    r_rtol = R_RTOL if r_rtol is None else r_rtol
+    r_atol = R_ATOL if r_atol is None else r_atol
     assert len(dev_log) == len(orc_log), f"{what}: log length {len(dev_log)} vs {len(orc_log)}"
     for f in EXACT_FIELDS:
         if dev_log[f].tobytes() != orc_log[f].tobytes():
@@ -48,7 +50,7 @@ def compare_logs(dev_log, orc_log, what=""):
             raise AssertionError(f"{what}: field {f} first differs at entry {i}: dev={dev_log[i]} orc={orc_log[i]} "
                                  f"(oracle margin at that proposal {margin:.3e})")
     both = np.abs(orc_log["R"]) > 0
-    err = np.abs(dev_log["R"] - orc_log["R"]) - (R_RTOL * np.abs(orc_log["R"]) + R_ATOL)
+    err = np.abs(dev_log["R"] - orc_log["R"]) - (r_rtol * np.abs(orc_log["R"]) + r_atol)
     assert err.size == 0 or err.max() < 0, f"{what}: R error beyond tolerance by {err.max():.3e} at entry {err.argmax()}"
     assert np.all(dev_log["R"][~both] == 0.0)
 
@@ -95,7 +97,9 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
     worst = 0.0
     for w, o in enumerate(orcs):
         what = f"{cfg['name']} walker {w}"
-        compare_logs(W.get_log(w), o.log(), what)
+        # while thermalising (n_tol loosened) the logged ratios carry the same conditioning-driven error as N
+        loose = n_tol > N_FROB_TOL
+        compare_logs(W.get_log(w), o.log(), what, r_rtol=1e-5 if loose else None, r_atol=1e-6 if loose else None)
         compare_configs(W.get_config(w), o.config(), what)
         st = W.get_stats(w)
         assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id, what
