@@ -223,7 +223,7 @@ def diff(a, b):
     return {k: a[k] - b[k] for k in a if k != "k_mean"}
 
 
-DEFAULT_GROUPS = {"cfg4_6x6_b20": 2, "cfg5_6x6_b40": 2}
+DEFAULT_GROUPS = {"cfg4_6x6_b20": 4, "cfg5_6x6_b40": 2}
 
 
 def run_gpu(args):
@@ -307,7 +307,7 @@ def run_gpu(args):
                     "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak if fp64_peak else None,
                     "traffic": (FLUSH_TRAFFIC_PER_WALKER[cfg["name"]] * (B // G) if cfg["name"] in FLUSH_TRAFFIC_PER_WALKER and
                                 delay == cfg["delay"] else None),
-                    "algorithmic_bytes": 16.0 * dk["sum_k"] / max(dk["proposals"], 1) ** 1 * 0 + 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),
+                    "algorithmic_bytes": 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),   # read + write of N, both spins
                     "peak_source": "cuBLAS DGEMM 8192^3 measured live in this run (FP64 runs at max SM clock: no power cap)",
                     "peak_alt": fp64_alt,
                     "peak_alt_source": f"{peaks['source']} bf16 sustained {peaks['bf16_sustained']:.1f} TF x nominal FP64:bf16 "

@@ -82,6 +82,68 @@ struct DescCandCols {  // G2: Gx (n x m) = N_ext (n x n) * gxC (n x m)
     return true;
   }
 };
+// Split-K forms of the two S2 GEMMs.  Their outputs are skinny (m = 64 rows or columns), so one CTA per
+// output tile leaves most of the 148 x 4 CTA slots empty (config 4 with two stream groups: 232 CTAs);
+// the contraction index is cut into S chunks, every chunk writes its partial product to `skbuf`, and
+// k_splitk_reduce adds the partials in a fixed order (deterministic, unlike atomics).
+__device__ __forceinline__ int sk_chunk(int K, int S) { return (((K + S - 1) / S) + 15) & ~15; }
+struct DescCandRowsSK {
+  DevCtx c; int S;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0 || st.k == 0) return false;
+    const int ch = sk_chunk(st.k, S), kb = s * ch;
+    if (kb >= st.k) return false;
+    const double* N = c.N(w, sp, st.n_cur);
+    d.M = st.m; d.N = st.k; d.K = (st.k - kb < ch) ? st.k - kb : ch;
+    d.A = c.Bm + ((size_t)w * 2 + sp) * (size_t)c.ldm * c.cap + (size_t)kb * c.ldm; d.lda = c.ldm;
+    d.B = N + kb; d.ldb = c.ld;
+    d.C = c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride; d.ldc = c.ldm;
+    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = 1.0; d.beta = 0.0;
+    return true;
+  }
+};
+struct DescCandColsSK {
+  DevCtx c; int S;
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0) return false;
+    const int n = st.k + st.m;
+    const int ch = sk_chunk(n, S), kb = s * ch;
+    if (kb >= n) return false;
+    d.M = n; d.N = st.m; d.K = (n - kb < ch) ? n - kb : ch;
+    d.A = c.N(w, sp, st.n_cur) + (size_t)kb * c.ld; d.lda = c.ld;
+    d.B = c.gxC + (size_t)w * c.ld * c.mmax + kb; d.ldb = c.ld;
+    d.C = c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride; d.ldc = c.ld;
+    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = 1.0; d.beta = 0.0;
+    return true;
+  }
+};
+// which = 0: candidate rows -> N_ext[k:k+m, 0:k];  which = 1: candidate columns -> Gx (n x m)
+__global__ void k_splitk_reduce(DevCtx c, int S, int which) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int m = st.m, k = st.k;
+  if (m == 0 || (which == 0 && k == 0)) return;
+  const int n = k + m;
+  const int rows = which == 0 ? m : n, cols = which == 0 ? k : m;
+  const int K = which == 0 ? k : n, ldp = which == 0 ? c.ldm : c.ld;
+  const int nvalid = (K + sk_chunk(K, S) - 1) / sk_chunk(K, S);
+  const double* part = c.skbuf + ((size_t)w * 2 + sp) * kMaxSplitK * c.skstride;
+  double* out = which == 0 ? c.N(w, sp, st.n_cur) + k : c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
+  const size_t total = (size_t)rows * cols;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % rows), j = (int)(idx / rows);
+    const size_t o = (size_t)j * ldp + i;
+    double v = part[o];
+    for (int s = 1; s < nvalid; ++s) v += part[(size_t)s * c.skstride + o];
+    out[(size_t)j * c.ld + i] = v;
+  }
+}
 struct DescUSinv {  // G3: Ut (k' x r) = U (k' x r) * S^-1 (r x r)
   DevCtx c;
   __device__ bool operator()(int prob, GemmDesc& d) const {
@@ -187,6 +249,12 @@ struct ctaux_ctx {
   bool sinv_smem;
   int propose_smem;
   bool small_tiles;
+  cudaStream_t hi;    // internal high-priority stream for the serial S3 kernel (forked from / joined to `stream`
+                      // with events): when several contexts share the GPU its few CTAs must not queue behind
+                      // thousands of GEMM CTAs of the other contexts
+  cudaEvent_t ev_fork, ev_join;
+  int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
+                      // kernels stride over their tiles, so a stale hint costs balance, never correctness)
   bool persist;       // large k and few problems: persistent GEMM kernel (gemm_persist.cuh)
   // timing
   bool timing;
@@ -201,7 +269,7 @@ namespace {
 
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
-      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, total;
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -225,6 +293,10 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   d.ld = round_up(d.cap, 8);
   d.ldm = round_up(mmax, 8);
   d.ldr = round_up(p->delay, 8);
+  {
+    const size_t a = (size_t)d.ldm * d.cap, b = (size_t)d.ld * d.mmax;
+    d.skstride = a > b ? a : b;
+  }
   d.log_capacity = p->log_capacity;
   d.beta = p->beta; d.K = p->K; d.tau_scale = (double)p->n_tau / p->beta;
   // Eq. (25): cosh(gamma) = 1 + U beta Ncorr / (2K)
@@ -265,6 +337,7 @@ Layout make_layout(const DevCtx& d) {
   L.perm = take(B * 2 * d.ld * 4);
   L.detsign = take(B * 2 * 4);
   L.seeds = take(B * 8);
+  L.skbuf = take(d.max_k > 512 ? B * 2 * kMaxSplitK * d.skstride * 8 : 0);
   L.total = o;
   return L;
 }
@@ -278,7 +351,8 @@ struct Scoped {
   ctaux_ctx* x;
   int cls;
   size_t idx;
-  Scoped(ctaux_ctx* x_, int cls_) : x(x_), cls(cls_), idx(0) {
+  cudaStream_t st;
+  Scoped(ctaux_ctx* x_, int cls_, cudaStream_t st_ = nullptr) : x(x_), cls(cls_), idx(0), st(st_ ? st_ : x_->stream) {
     if (!x->timing) return;
     if (x->ev_used + 2 > x->ev_pool.size()) {
       for (int i = 0; i < 2; ++i) {
@@ -291,11 +365,11 @@ struct Scoped {
     idx = x->ev_used;
     x->ev_class[idx / 2] = cls;
     x->ev_used += 2;
-    cudaEventRecord(x->ev_pool[idx], x->stream);
+    cudaEventRecord(x->ev_pool[idx], st);
   }
   ~Scoped() {
     if (!x->timing) return;
-    cudaEventRecord(x->ev_pool[idx + 1], x->stream);
+    cudaEventRecord(x->ev_pool[idx + 1], st);
   }
 };
 void harvest_timing(ctaux_ctx* x) {  // call after a stream synchronise
@@ -325,6 +399,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
   harvest_timing(x);
   int kmax = 0;
   for (int w = 0; w < d.B; ++w) kmax = h[w].k > kmax ? h[w].k : kmax;
+  x->k_hint = kmax;
   if (set_sign) {
     std::vector<int> ones(d.B * 2, 1);
     CU_CHECK(cudaMemcpyAsync(x->detsign, ones.data(), sizeof(int) * d.B * 2, cudaMemcpyHostToDevice, s));
@@ -379,13 +454,16 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
 
 // one block step for all walkers: S1/S2 prep, S2 GEMMs, S3 proposals, S4 flush
 int enqueue_block_step(ctaux_ctx* x) {
-  const DevCtx& d = x->d;
+  DevCtx d = x->d;
   cudaStream_t s = x->stream;
   const int P = d.B * 2;
+  // grids are sized for the live order (hint + one block of growth), not for the capacity
+  const int kh = x->k_hint + d.delay < d.max_k ? x->k_hint + d.delay : d.max_k;
+  const int kcap = kh + d.mmax;
   {
     Scoped t(x, C_PREP);
     k_prep_window<<<d.B, 1024, 0, s>>>(d);
-    k_prep_fill<<<dim3(grid_for((size_t)d.cap * d.mmax, 256, 256), d.B), 256, 0, s>>>(d);
+    k_prep_fill<<<dim3(grid_for((size_t)kcap * d.mmax, 256, 256), d.B), 256, 0, s>>>(d);
     tick(x, C_PREP); tick(x, C_PREP);
   }
   {
@@ -395,32 +473,57 @@ int enqueue_block_step(ctaux_ctx* x) {
       e1 = launch_persist<1>(DescCandRows{d}, P, s);
       e2 = launch_persist<0>(DescCandCols{d}, P, s);
     } else if (x->small_tiles) {
-      e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
-      e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
+      e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((kh + 63) / 64), P, s);
+      e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (kcap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
-      e1 = launch_gemm<GEMM_Q4>(DescCandRows{d}, (d.mmax + 63) / 64 * ((d.max_k + 63) / 64), P, s);
-      e2 = launch_gemm<GEMM_Q4>(DescCandCols{d}, (d.cap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
+      const int t1 = (d.mmax + 63) / 64 * ((kh + 63) / 64), t2 = (kcap + 63) / 64 * ((d.mmax + 63) / 64);
+      // split-K factor: aim at >= 1.5 waves of the 148 x 4 CTA slots, chunks of at least 128
+      int S = (6 * sm_count() + P * t1 - 1) / (P * t1);
+      if (S > kMaxSplitK) S = kMaxSplitK;
+      while (S > 1 && kh / S < 128) --S;
+      if (S <= 1) {
+        e1 = launch_gemm<GEMM_Q4>(DescCandRows{d}, t1, P, s);
+        e2 = launch_gemm<GEMM_Q4>(DescCandCols{d}, t2, P, s);
+      } else {
+        const int rb = grid_for((size_t)kcap * d.mmax, 256, 128);
+        e1 = launch_gemm<GEMM_Q4>(DescCandRowsSK{d, S}, t1, P * S, s);
+        k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 0);
+        e2 = launch_gemm<GEMM_Q4>(DescCandColsSK{d, S}, t2, P * S, s);
+        k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 1);
+        tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
+      }
     }
     CU_CHECK(e1); CU_CHECK(e2);
     tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
   }
   {
-    Scoped t(x, C_PROPOSE);
-    if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, s>>>(d);
-    else k_propose<false><<<d.B, kPropThreads, x->propose_smem, s>>>(d);
-    tick(x, C_PROPOSE);
+    cudaStream_t ps = x->hi ? x->hi : s;
+    if (x->hi) {
+      CU_CHECK(cudaEventRecord(x->ev_fork, s));
+      CU_CHECK(cudaStreamWaitEvent(x->hi, x->ev_fork, 0));
+    }
+    {
+      Scoped t(x, C_PROPOSE, ps);
+      if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      else k_propose<false><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      tick(x, C_PROPOSE);
+    }
+    if (x->hi) {
+      CU_CHECK(cudaEventRecord(x->ev_join, x->hi));
+      CU_CHECK(cudaStreamWaitEvent(s, x->ev_join, 0));
+    }
   }
   {
     Scoped t(x, C_UV);
-    k_build_uv<<<dim3(grid_for((size_t)d.max_k * d.delay, 256, 512), P), 256, 0, s>>>(d);
+    k_build_uv<<<dim3(grid_for((size_t)kh * d.delay, 256, 512), P), 256, 0, s>>>(d);
     tick(x, C_UV);
   }
   {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
     if (x->persist) e3 = launch_persist<0>(DescUSinv{d}, P, s);
-    else if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
-    else e3 = launch_gemm<GEMM_Q4>(DescUSinv{d}, (d.max_k + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    else if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    else e3 = launch_gemm<GEMM_Q4>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
   }
@@ -430,10 +533,10 @@ int enqueue_block_step(ctaux_ctx* x) {
     if (x->persist) {
       e4 = launch_persist<0>(DescFlush{d}, P, s);
     } else if (x->small_tiles) {
-      const int tl = (d.max_k + 63) / 64;
+      const int tl = (kh + 63) / 64;
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
-      const int tl = (d.max_k + 63) / 64;
+      const int tl = (kh + 63) / 64;
       e4 = launch_gemm<GEMM_Q5>(DescFlush{d}, tl * tl, P, s);  // L2 prefetch of C0 measured: no gain
     }
     CU_CHECK(e4);
@@ -457,9 +560,10 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
       int rc = enqueue_block_step(x);
       if (rc) return rc;
     }
-    CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(cudaStreamSynchronize(s));
     harvest_timing(x);
+    if (x->host_flag[1] > 0) x->k_hint = x->host_flag[1];
     if (x->host_flag[0] <= 0) break;
   }
   // errors raised inside kernels
@@ -519,11 +623,13 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   d.J = (int32_t*)(base + L.J); d.rowmap = (int32_t*)(base + L.rowmap);
   d.log = (LogEntry*)(base + L.log); d.n_active = (int32_t*)(base + L.n_active);
   d.colbuf = (double*)(base + L.colbuf); d.rowbuf = (double*)(base + L.rowbuf); d.perm = (int32_t*)(base + L.perm);
+  d.skbuf = (double*)(base + L.skbuf);
   x->detsign = (int*)(base + L.detsign);
   x->seeds_d = (uint64_t*)(base + L.seeds);
   d.g00 = -prm->g0_table[0];
   x->d = d;
   x->have_state = false;
+  x->k_hint = d.max_k;
   x->sweeps_since_rebuild = 0;
   x->launches = 0;
   x->timing = false;
@@ -558,6 +664,18 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     delete x;
     return CTAUX_ECUDA;
   }
+  x->hi = nullptr; x->ev_fork = nullptr; x->ev_join = nullptr;
+  {
+    int lo = 0, hi = 0;
+    if (cudaDeviceGetStreamPriorityRange(&lo, &hi) == cudaSuccess && hi < lo &&
+        cudaStreamCreateWithPriority(&x->hi, cudaStreamNonBlocking, hi) == cudaSuccess) {
+      if (cudaEventCreateWithFlags(&x->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&x->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaStreamDestroy(x->hi);
+        x->hi = nullptr;
+      }
+    }
+  }
   x->small_tiles = d.max_k <= 512;
   // The persistent kernel (gemm_persist.cuh) hides the C0 latency of the flush but its main loop is slower
   // than two independent 8-warp CTAs per SM (profiles/r1_gemm_variants.md); off until that is fixed.
@@ -570,6 +688,7 @@ void ctaux_destroy(ctaux_ctx* x) {
   if (!x) return;
   cudaStreamSynchronize(x->stream);
   for (cudaEvent_t e : x->ev_pool) cudaEventDestroy(e);
+  if (x->hi) { cudaStreamSynchronize(x->hi); cudaStreamDestroy(x->hi); cudaEventDestroy(x->ev_fork); cudaEventDestroy(x->ev_join); }
   if (x->host_flag) cudaFreeHost(x->host_flag);
   delete x;
 }

@@ -75,7 +75,7 @@ __global__ void k_build_A(DevCtx c, int into_other) {
 // Start of a ctaux_sweep chunk.
 __global__ void k_begin_sweeps(DevCtx c, int n_sweeps) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  if (w == 0) *c.n_active = c.B;
+  if (w == 0) { c.n_active[0] = c.B; c.n_active[1] = 0; }
   if (w >= c.B) return;
   c.ws[w].sweeps_left = n_sweeps;
   c.ws[w].props_left = 0;
@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(1024) k_prep_window(DevCtx c) {
   __shared__ int s_win;
   const int tid = threadIdx.x;
   if (!st.active || st.status) {
-    if (tid == 0) { st.m = 0; st.win = 0; st.r = 0; st.n_src = st.n_cur; }
+    if (tid == 0) { st.m = 0; st.win = 0; st.r = 0; st.n_src = st.n_cur; atomicMax(c.n_active + 1, st.k); }
     return;
   }
   const int k = st.k;
@@ -518,6 +518,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);
     st.flops_usinv += 2.0 * (2.0 * (double)kcur * r * r);
     if (status) st.status = status;
+    atomicMax(c.n_active + 1, kcur);   // largest live order, mirrored to the host at every poll (grid sizing)
     if (finished || status) {
       st.active = 0;
       atomicSub(c.n_active, 1);

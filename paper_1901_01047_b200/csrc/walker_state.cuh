@@ -7,6 +7,7 @@
 namespace ctaux {
 
 constexpr int kMaxDelay = 256;
+constexpr int kMaxSplitK = 8;
 
 struct LogEntry {  // == ctaux_log_entry
   uint64_t p;
@@ -64,6 +65,8 @@ struct DevCtx {
   double* Bm;           // [B][2][ldm*cap]   candidate rows  g(c,j)(E_j-1), m x k col-major
   double* gxC;          // [B][ld*mmax]      g_ext[:, C], n x m col-major (spin independent)
   double* Gx;           // [B][2][ld*mmax]   N_ext * g_ext[:, C]
+  double* skbuf;        // [B][2][kMaxSplitK][skstride]  split-K partial products of the S2 GEMMs
+  size_t skstride;      // max(ldm*cap, ld*mmax)
   double* Um;           // [B][2][ld*delay]  U = X[:, J]
   double* Ut;           // [B][2][ld*delay]  U * S^-1
   double* Vt;           // [B][2][ldr*ld]    rows J of N_ext, r x k' col-major
