@@ -80,6 +80,11 @@ typedef struct ctaux_params {
                               random initial configuration).  0 = library default (100: ends ~1.5% of
                               the blocks early in equilibrium); < 0 or inf = off.  Chain-neutral: only where blocks
                               end.                                                                    */
+  int32_t fused_small;     /* small-k path: 0 = automatic (used when both N_sigma of a walker fit one SM's
+                              shared memory, max_k <= ~100), 1 = require it (CTAUX_ECAPACITY if it does not
+                              fit), -1 = never.  The fused kernel runs whole sweeps of a walker in one launch
+                              with N in shared memory and applies every accepted move at once (delay and
+                              cand_window are ignored there: they are chain-neutral knobs).              */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */

@@ -15,6 +15,7 @@
 #include "gemm_persist.cuh"
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
+#include "walker_fused.cuh"
 
 using namespace ctaux;
 
@@ -253,6 +254,8 @@ struct ctaux_ctx {
                       // with events): when several contexts share the GPU its few CTAs must not queue behind
                       // thousands of GEMM CTAs of the other contexts
   cudaEvent_t ev_fork, ev_join;
+  bool fused;         // small-k path: whole sweeps in k_walk_fused (walker_fused.cuh)
+  int fused_smem, fcap;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
   bool persist;       // large k and few problems: persistent GEMM kernel (gemm_persist.cuh)
@@ -549,8 +552,32 @@ int enqueue_block_step(ctaux_ctx* x) {
 int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
-  k_begin_sweeps<<<(d.B + 127) / 128, 128, 0, s>>>(d, n_sweeps);
-  tick(x, C_OTHER);
+  bool resume = false;   // true: walkers spilled by the fused kernel continue on the delayed path
+  if (x->fused) {
+    CU_CHECK(cudaMemsetAsync(d.n_active, 0, 2 * sizeof(int), s));
+    {
+      Scoped t(x, C_PROPOSE);
+      k_walk_fused<<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
+      tick(x, C_PROPOSE);
+    }
+    CU_CHECK(cudaGetLastError());
+    CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(cudaStreamSynchronize(s));
+    harvest_timing(x);
+    if (x->host_flag[0] <= 0) {
+      std::vector<WalkerState> hf(d.B);
+      CU_CHECK(cudaMemcpy(hf.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+      for (int w = 0; w < d.B; ++w)
+        if (hf[w].status) return hf[w].status;
+      return CTAUX_OK;
+    }
+    resume = true;
+    x->k_hint = d.max_k;
+  }
+  if (!resume) {
+    k_begin_sweeps<<<(d.B + 127) / 128, 128, 0, s>>>(d, n_sweeps);
+    tick(x, C_OTHER);
+  }
   const int steps_per_poll = 8;
   // every block consumes at least one proposal and a sweep has at most max(16, max_k) of them
   const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + steps_per_poll;
@@ -663,6 +690,25 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (x->host_flag) cudaFreeHost(x->host_flag);
     delete x;
     return CTAUX_ECUDA;
+  }
+  {
+    // shared-memory capacity of the fused path: all of max_k if it fits, else up to 104 slots when the
+    // configured capacity is only a little larger (walkers that fluctuate above it spill to the delayed path)
+    int fcap = d.max_k;
+    while (fcap > 8 && fused_smem_layout(fcap).total > max_smem) fcap -= 4;
+    const bool fits = fused_smem_layout(fcap).total <= max_smem && fcap <= 256 && 4 * fcap >= 3 * d.max_k;
+    if (prm->fused_small > 0 && !fits) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_ECAPACITY; }
+    x->fused = prm->fused_small >= 0 && fits;
+    x->fcap = fcap;
+    const int need = fused_smem_layout(fcap).total;
+    x->fused_smem = need;
+    if (x->fused) {
+      static int fused_attr_max = 0;
+      if (need > fused_attr_max) {
+        if (cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, need) != cudaSuccess) x->fused = false;
+        else fused_attr_max = need;
+      }
+    }
   }
   x->hi = nullptr; x->ev_fork = nullptr; x->ev_join = nullptr;
   {

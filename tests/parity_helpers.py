@@ -79,7 +79,7 @@ def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
 
 
 def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, init_k=None, seeds=None,
-                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL):
+                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0):
     """reset + n_sweeps on both sides, compare logs, configurations, N, sign, counters."""
     from paper_1901_01047_b200 import Walkers
     table = table_for(cfg)
@@ -90,7 +90,7 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
                 delay=cfg["delay"] if delay is None else delay, n_walkers=n_walkers, init_k=init_k,
                 max_k=cfg["max_k"] if max_k is None else max_k,
                 rebuild_every=cfg["rebuild_every"] if rebuild_every is None else rebuild_every,
-                log_capacity=cap, cand_window=cand_window)
+                log_capacity=cap, cand_window=cand_window, fused_small=fused)
     W.reset(seeds)
     W.sweep(n_sweeps)
     orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k)

@@ -87,17 +87,32 @@ def test_reset_builds_inverse(ci, nw):
             assert np.linalg.norm(res) / np.sqrt(k) < 1e-10
 
 
-def test_config1_full_lockstep_T0():
+# fused = 1: the single-kernel small-k path (walker_fused.cuh, what configs 1-2 run by default);
+# fused = -1: the delayed-block path (S2 GEMMs, S3 over the Gamma block, S4 flush) the large configs run.
+@pytest.mark.parametrize("fused", [1, -1])
+def test_config1_full_lockstep_T0(fused):
     """Config 1 in full (200 warm-up + 1000 sweeps, 1 walker, delay 8) against brute force T0."""
     cfg = get_config(0)
-    W, orcs, worst = full_parity(cfg, 1, cfg["warmup_sweeps"] + cfg["sweeps"], T0)
+    W, orcs, worst = full_parity(cfg, 1, cfg["warmup_sweeps"] + cfg["sweeps"], T0, fused=fused)
     assert W.get_stats(0)["rebuilds"] == 120
 
 
-def test_config2_batched_walkers_T0_prefix_and_T1():
+@pytest.mark.parametrize("fused", [1, -1])
+def test_config2_batched_walkers_T0_prefix_and_T1(fused):
     cfg = get_config(1)
-    full_parity(cfg, 16, 12, T0)          # brute force on a prefix, 16 walkers
-    full_parity(cfg, 256, 40, T1)         # all 256 walkers, rank-1 oracle
+    full_parity(cfg, 16, 12, T0, fused=fused)          # brute force on a prefix, 16 walkers
+    full_parity(cfg, 256, 40, T1, fused=fused)         # all 256 walkers, rank-1 oracle
+
+
+def test_config2_fused_without_rebuild_N_1e10():
+    """The fused path's incrementally updated N (rank-1 updates in shared memory, no rebuild) from the
+    equilibrated state of an oracle chain: 32 walkers x 15 sweeps."""
+    cfg = get_config(1)
+    table = table_for(cfg)
+    o = OracleWalker.from_config(cfg, table, 0, T1)
+    o.reset(cfg["init_k"])
+    o.sweep(60)
+    parity_from_state(cfg, (o.config(), o.next_id, o.p), walker_seeds(32), 15, T1, fused_small=1)
 
 
 def test_config3_T1():
@@ -119,19 +134,20 @@ def test_config3_thermalised_start_N_1e10():
 def test_chain_independent_of_delay_rebuild_window(delay, rebuild, cand):
     """Q18-Q20: delay, rebuild cadence and the candidate window are performance knobs only."""
     cfg = get_config(1)
-    full_parity(cfg, 4, 10, T1, delay=delay, rebuild_every=rebuild, cand_window=cand)
+    full_parity(cfg, 4, 10, T1, delay=delay, rebuild_every=rebuild, cand_window=cand, fused=-1)
 
 
-def test_sweep_calls_continue_the_chain():
+@pytest.mark.parametrize("fused", [1, -1])
+def test_sweep_calls_continue_the_chain(fused):
     cfg = get_config(1)
     table = table_for(cfg)
     pkg = _pkg()
     seeds = walker_seeds(3, first=100)
-    a = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000)
+    a = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000, fused_small=fused)
     a.reset(seeds)
     for n in (1, 2, 3):
         a.sweep(n)
-    b = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000)
+    b = pkg.Walkers.from_config(cfg, table, n_walkers=3, log_capacity=4000, fused_small=fused)
     b.reset(seeds)
     b.sweep(6)
     for w in range(3):
@@ -141,15 +157,17 @@ def test_sweep_calls_continue_the_chain():
         assert a.get_stats(w)["proposals"] == b.get_stats(w)["proposals"]
 
 
-def test_empty_start_and_tiny_cluster_edge_cases():
+@pytest.mark.parametrize("fused", [1, -1])
+def test_empty_start_and_tiny_cluster_edge_cases(fused):
     """Degenerate cases: empty initial configuration (removals on k=0 are rejected), 1x1 cluster."""
     cfg = get_config(0)
-    full_parity(cfg, 3, 30, T0, init_k=0)
+    full_parity(cfg, 3, 30, T0, init_k=0, fused=fused)
     atom = dict(cfg, name="atom", Lx=1, Ly=1, mu=0.0)
-    full_parity(atom, 2, 30, T0, init_k=0)
+    full_parity(atom, 2, 30, T0, init_k=0, fused=fused)
 
 
-def test_set_state_resumes_an_oracle_chain():
+@pytest.mark.parametrize("fused", [1, -1])
+def test_set_state_resumes_an_oracle_chain(fused):
     """ctaux_set_state: continue on the device from a configuration produced by the oracle."""
     cfg = get_config(1)
     table = table_for(cfg)
@@ -159,7 +177,7 @@ def test_set_state_resumes_an_oracle_chain():
     c0, nid, p0 = o.config(), o.next_id, o.p
     o.clear_log()
     o.sweep(4)
-    W = _pkg().Walkers.from_config(cfg, table, n_walkers=1, log_capacity=2000)
+    W = _pkg().Walkers.from_config(cfg, table, n_walkers=1, log_capacity=2000, fused_small=fused)
     W.set_state([9], [c0], [nid], [p0])
     W.sweep(4)
     compare_logs(W.get_log(0), o.log(), "resumed")
@@ -167,15 +185,35 @@ def test_set_state_resumes_an_oracle_chain():
     compare_N(W, 0, o, "resumed")
 
 
-def test_capacity_error_is_loud():
+@pytest.mark.parametrize("fused", [1, -1])
+def test_capacity_error_is_loud(fused):
     cfg = get_config(1)
     table = table_for(cfg)
     pkg = _pkg()
     W = pkg.Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table, delay=8, n_walkers=2,
-                    init_k=5, max_k=12)
+                    init_k=5, max_k=12, fused_small=fused)
     W.reset(walker_seeds(2))
     with pytest.raises(pkg.CtauxError) as ei:
         W.sweep(50)
+    assert ei.value.code == -2
+
+
+def test_fused_path_spills_to_the_delayed_path():
+    """2x2 cluster at beta = 18: <k> ~ 110 sits at the shared-memory capacity of the fused kernel (116 slots
+    for max_k = 150), so walkers keep crossing it: they spill to the delayed-block path mid-sweep and come
+    back at the next call.  Same chain, bit for bit."""
+    cfg = dict(get_config(1), name="cfg2_beta18", beta=18.0, max_k=150, init_k=74, rebuild_every=4)
+    W, orcs, worst = full_parity(cfg, 8, 16, T1, fused=1, n_tol=N_TOL_THERMALISING)
+    st = [W.get_stats(w) for w in range(8)]
+    assert sum(x["flushes"] for x in st) > 0, "no walker ever spilled: the test does not reach the capacity"
+    assert max(o.k for o in orcs) > 100
+
+
+def test_fused_path_refuses_what_does_not_fit():
+    cfg = get_config(2)                      # max_k 384: 2 x 384^2 x 8 B does not fit one SM
+    pkg = _pkg()
+    with pytest.raises(pkg.CtauxError) as ei:
+        pkg.Walkers.from_config(cfg, table_for(cfg), n_walkers=1, fused_small=1)
     assert ei.value.code == -2
 
 
