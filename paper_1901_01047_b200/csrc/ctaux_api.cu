@@ -16,6 +16,7 @@
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
 #include "walker_fused.cuh"
+#include "walker_propose_cl.cuh"
 
 using namespace ctaux;
 
@@ -254,6 +255,9 @@ struct ctaux_ctx {
                       // with events): when several contexts share the GPU its few CTAs must not queue behind
                       // thousands of GEMM CTAs of the other contexts
   cudaEvent_t ev_fork, ev_join;
+  int cluster_mode;   // 0: k_propose (one CTA per walker); 1 / 2: k_propose_cl (2-CTA cluster per walker) with
+                      // S^-1 in shared memory / in L2 -- used when S^-1 of both spins does not fit one CTA
+  int cluster_smem;
   bool fused;         // small-k path: whole sweeps in k_walk_fused (walker_fused.cuh)
   int fused_smem, fcap;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
@@ -507,7 +511,9 @@ int enqueue_block_step(ctaux_ctx* x) {
     }
     {
       Scoped t(x, C_PROPOSE, ps);
-      if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      if (x->cluster_mode == 1) k_propose_cl<true><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+      else if (x->cluster_mode == 2) k_propose_cl<false><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+      else if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
       else k_propose<false><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
       tick(x, C_PROPOSE);
     }
@@ -708,6 +714,18 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
         if (cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, need) != cudaSuccess) x->fused = false;
         else fused_attr_max = need;
       }
+    }
+  }
+  x->cluster_mode = 0; x->cluster_smem = 0;
+  if (!x->sinv_smem) {
+    ProposeClSmem Lc = propose_cl_smem_layout(d.cap, d.delay, d.winmax, true);
+    int mode = 1;
+    if (Lc.total > max_smem) { Lc = propose_cl_smem_layout(d.cap, d.delay, d.winmax, false); mode = 2; }
+    if (Lc.total <= max_smem) {
+      cudaError_t ec = mode == 1 ? cudaFuncSetAttribute(k_propose_cl<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lc.total)
+                                 : cudaFuncSetAttribute(k_propose_cl<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lc.total);
+      if (ec == cudaSuccess) { x->cluster_mode = mode; x->cluster_smem = Lc.total; }
+      else cudaGetLastError();
     }
   }
   x->hi = nullptr; x->ev_fork = nullptr; x->ev_join = nullptr;

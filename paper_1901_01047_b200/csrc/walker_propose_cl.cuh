@@ -1,0 +1,349 @@
+// S3 for large delays (delay > ~100: S^-1 of both spins no longer fits one SM's shared memory):
+// the same serial Metropolis chain as k_propose (walker_kernels.cuh), run by a thread-block CLUSTER of
+// two CTAs per walker, one per spin.  Each CTA keeps the S^-1 of its own spin (132 KB at delay 128) in
+// its own shared memory (or in L2 when even that does not fit: delay 256), evaluates its spin's
+// determinant ratio with 512 threads (4 lanes per row of S^-1), and the two CTAs exchange their
+// per-proposal scalars through distributed shared memory with ONE cluster barrier per proposal.  All
+// bookkeeping (live list, J, counters) is replicated, so both CTAs take identical decisions.
+// PAPER.md:226-228 (submatrix updates), BASELINE.json config 5 (delay 128 and 256).
+#pragma once
+#include <cooperative_groups.h>
+
+#include "walker_kernels.cuh"
+
+namespace ctaux {
+
+constexpr int kClThreads = 512;
+
+struct ProposeClSmem {
+  int sinv, scol, srow, tv, tpv, red, snn, xch, live0, live1, spin, J, jpos, prop, total;
+};
+__host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
+  ProposeClSmem L;
+  int o = 0;
+  const int lds = delay | 1;
+  L.sinv = o; o += sinv_smem ? lds * delay * 8 : 0;
+  L.scol = o; o += delay * 8;
+  L.srow = o; o += delay * 8;
+  L.tv = o; o += delay * 8;
+  L.tpv = o; o += delay * 8;
+  L.red = o; o += 2 * 16 * 8;
+  L.snn = o; o += 2 * 8;
+  L.xch = o; o += 2 * 2 * 4 * 8;      // [parity][spin][stil, ampnum, -, -]
+  L.prop = o; o += winmax * 16;
+  L.live0 = o; o += cap * 4;
+  L.live1 = o; o += cap * 4;
+  L.J = o; o += delay * 4;
+  L.jpos = o; o += (winmax + 1) * 4;
+  L.spin = o; o += (cap + 15) / 16 * 16;
+  L.total = o;
+  return L;
+}
+
+template <bool sinv_smem>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_propose_cl(DevCtx c) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  extern __shared__ __align__(16) unsigned char smcl[];
+  const int w = blockIdx.x >> 1, sp = (int)cluster.block_rank(), tid = threadIdx.x;
+  WalkerState& st = c.ws[w];
+  if (!st.active || st.status || st.win == 0) return;   // identical in both CTAs of the cluster
+  const ProposeClSmem L = propose_cl_smem_layout(c.cap, c.delay, c.winmax, sinv_smem);
+  const int lds = sinv_smem ? (c.delay | 1) : c.ldr;
+  double* Sv = sinv_smem ? reinterpret_cast<double*>(smcl + L.sinv)
+                         : (c.Sinv + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.delay);
+  double* scol = reinterpret_cast<double*>(smcl + L.scol);
+  double* srow = reinterpret_cast<double*>(smcl + L.srow);
+  double* tv = reinterpret_cast<double*>(smcl + L.tv);
+  double* tpv = reinterpret_cast<double*>(smcl + L.tpv);
+  double* red = reinterpret_cast<double*>(smcl + L.red);    // [16] dot, [16] sum of magnitudes
+  double* snn2 = reinterpret_cast<double*>(smcl + L.snn);   // [2 parities]
+  double* xch = reinterpret_cast<double*>(smcl + L.xch);
+  double* xch_peer = cluster.map_shared_rank(xch, sp ^ 1);
+  PropInfo* prop = reinterpret_cast<PropInfo*>(smcl + L.prop);
+  int* live = reinterpret_cast<int*>(smcl + L.live0);
+  int* live_alt = reinterpret_cast<int*>(smcl + L.live1);
+  int* Js = reinterpret_cast<int*>(smcl + L.J);
+  int* jpos = reinterpret_cast<int*>(smcl + L.jpos);
+  signed char* spin_s = reinterpret_cast<signed char*>(smcl + L.spin);
+
+  const int k0 = st.k, m = st.m, win = st.win, n = k0 + m;
+  const int cfg_old = st.cfg_cur;
+  const size_t off_old = c.cfg_off(w, cfg_old), off_new = c.cfg_off(w, cfg_old ^ 1);
+  const double* Ncur = c.N(w, sp, st.n_cur);
+  const double* Gx = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
+  const int ld = c.ld;
+  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
+  // everything read from the walker state BEFORE the first cluster barrier; rank 0 alone writes it at the end
+  int kcur = k0, r = 0, len = k0;
+  int props_left = st.props_left, sweeps_left = st.sweeps_left;
+  uint64_t next_id = st.next_id, p = st.p;
+  int sign = st.sign, status = 0;
+  int64_t acc_ins = 0, acc_rem = 0, sweeps_done = 0;
+  double min_margin = st.min_margin, sum_k = 0.0;
+  int64_t log_count = st.log_count;
+  const int n_cur0 = st.n_cur;
+  bool finished = false;
+  int guard_end = 0;
+  double errlvl = 1.0;
+
+  for (int i = tid; i < n; i += kClThreads) spin_s[i] = (signed char)c.cfg_spin[off_old + i];
+  for (int i = tid; i < k0; i += kClThreads) live[i] = i;
+  for (int i = tid; i < win; i += kClThreads) prop[i] = c.prop[(size_t)w * c.winmax + i];
+  for (int i = tid; i <= c.winmax; i += kClThreads) jpos[i] = -1;
+  cluster.sync();
+
+  auto X = [&](int i, int j) -> double {
+    const double dlt = (i == j) ? 1.0 : 0.0;
+    if (j < k0) {
+      const bool em = ((sp == 0) == (spin_s[j] > 0));
+      return (dlt - Ncur[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
+    }
+    return dlt - Gx[(size_t)(j - k0) * ld + i];
+  };
+  // publish this spin's two scalars to both CTAs, one cluster barrier, read both spins' values
+  int xpar = 0;
+  auto exchange = [&](double v0, double v1, double (&o0)[2], double (&o1)[2]) {
+    if (tid == 0) {
+      double* mine = xch + (xpar * 2 + sp) * 4;
+      double* theirs = xch_peer + (xpar * 2 + sp) * 4;
+      mine[0] = v0; mine[1] = v1;
+      theirs[0] = v0; theirs[1] = v1;
+    }
+    cluster.sync();
+    o0[0] = xch[(xpar * 2 + 0) * 4]; o0[1] = xch[(xpar * 2 + 0) * 4 + 1];
+    o1[0] = xch[(xpar * 2 + 1) * 4]; o1[1] = xch[(xpar * 2 + 1) * 4 + 1];
+    xpar ^= 1;
+  };
+
+  const int role = tid >> 8, rl = tid & 255;   // role 0: s_col and t; role 1: s_row and t'
+  const int row4 = rl >> 2, q4 = rl & 3;       // 64 rows per pass, 4 lanes per row
+  const unsigned quad_mask = 0xFu << (tid & 28);   // the 4 lanes of a row leave the row loop together
+
+  for (int i = 0; i < win; ++i) {
+    if (props_left == 0) {
+      if (sweeps_left == 0) { finished = true; break; }
+      --sweeps_left;
+      props_left = kcur > 16 ? kcur : 16;
+    }
+    const PropInfo pi = prop[i];
+    const int type = (int)(pi.type_cand & 1u);
+    int slot = -1, j = -1;
+    double pref = 0.0;
+    if (type == 0) {
+      slot = k0 + (int)(pi.type_cand >> 1);
+      pref = c.K / (double)(kcur + 1);
+    } else if (kcur > 0) {
+      j = (int)(((uint64_t)pi.w1 * (uint64_t)kcur) >> 32);
+      slot = live[j];
+      pref = (double)kcur / c.K;
+    }
+    bool accept = false;
+    double R = 0.0, stil_own = 1.0, amp = 1.0;
+    const bool down = (type == 1 && slot >= k0);
+    int apos = -1;
+    if (down) {
+      // removal of a vertex inserted earlier in this block: the buffered insertion is taken out
+      apos = jpos[slot - k0];
+      const int s = spin_s[slot];
+      const double sa_own = Sv[apos + (size_t)apos * lds];
+      double o0[2], o1[2];
+      exchange(sa_own, 0.0, o0, o1);
+      R = pref * ((o0[0] / (c.E(0, s) - 1.0)) * (o1[0] / (c.E(1, s) - 1.0)));
+      accept = pi.u < fabs(R);
+      stil_own = sa_own;
+    } else if (slot >= 0) {
+      const int s = spin_s[slot];
+      const double E0 = c.E(0, s), E1 = c.E(1, s);
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (1.0 - E0);
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (1.0 - E1);
+      const double dE_own = sp == 0 ? dE0 : dE1;
+      for (int a = rl; a < r; a += 256) {
+        const int ja = Js[a];
+        if (role == 0) scol[a] = X(ja, slot);
+        else srow[a] = X(slot, ja);
+      }
+      double* snn = snn2 + (i & 1);
+      if (tid == 0) {
+        if (slot < k0) *snn = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
+        else *snn = 1.0 / dE_own + X(slot, slot);
+      }
+      __syncthreads();
+      double part = 0.0, apart = 0.0;
+      for (int a = row4; a < r; a += 64) {
+        double s0 = 0.0, s1 = 0.0;
+        int b = q4;
+        if (role == 0) {
+          const double* Sa = Sv + a;
+          for (; b + 4 < r; b += 8) { s0 += Sa[(size_t)b * lds] * scol[b]; s1 += Sa[(size_t)(b + 4) * lds] * scol[b + 4]; }
+          if (b < r) s0 += Sa[(size_t)b * lds] * scol[b];
+        } else {
+          const double* Sa = Sv + (size_t)a * lds;
+          for (; b + 4 < r; b += 8) { s0 += srow[b] * Sa[b]; s1 += srow[b + 4] * Sa[b + 4]; }
+          if (b < r) s0 += srow[b] * Sa[b];
+        }
+        double t = s0 + s1;
+        t += __shfl_xor_sync(quad_mask, t, 1);
+        t += __shfl_xor_sync(quad_mask, t, 2);
+        if (q4 == 0) {
+          if (role == 0) { tv[a] = t; part += srow[a] * t; apart += fabs(srow[a] * t); }
+          else tpv[a] = t;
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        part += __shfl_xor_sync(0xffffffffu, part, o);
+        apart += __shfl_xor_sync(0xffffffffu, apart, o);
+      }
+      if ((tid & 31) == 0) { red[tid >> 5] = part; red[16 + (tid >> 5)] = apart; }
+      __syncthreads();
+      double dot = 0.0, adot = 0.0;
+#pragma unroll
+      for (int q = 0; q < 8; ++q) { dot += red[q]; adot += red[16 + q]; }   // role-1 warps (8..15) hold zeros
+      const double stil = *snn - dot;
+      double o0[2], o1[2];
+      exchange(stil, fabs(*snn) + adot, o0, o1);
+      const double stil0 = o0[0], stil1 = o1[0];
+      {
+        const double amp0 = o0[1] / fmax(fabs(stil0), 1e-300);
+        const double amp1 = o1[1] / fmax(fabs(stil1), 1e-300);
+        amp = fmax(amp0, amp1);
+        if (r > 0 && amp * errlvl > c.guard_amp) { guard_end = 1; break; }
+      }
+      stil_own = stil;
+      R = pref * ((dE0 * stil0) * (dE1 * stil1));
+      accept = pi.u < fabs(R);
+    }
+    if (tid == 0 && sp == 0 && log_count < (int64_t)c.log_capacity) {
+      LogEntry e;
+      e.p = p; e.type = type;
+      e.arg = (type == 0) ? c.cfg_site[off_old + slot] : j;
+      e.tau = (type == 0) ? c.cfg_tau[off_old + slot] : 0.0;
+      e.spin = (type == 0) ? (int)spin_s[slot] : 0;
+      e.accepted = accept ? 1 : 0;
+      e.R = R; e.u = pi.u;
+      c.log[(size_t)w * c.log_capacity + log_count] = e;
+    }
+    ++log_count;
+    if (slot >= 0) {
+      const double aR = fabs(R);
+      const double mg = fabs(pi.u - aR) / fmax(aR, 1e-300);
+      if (mg < min_margin) min_margin = mg;
+    }
+    sum_k += (double)kcur;
+    if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }
+    if (accept && down) {
+      const double inv = 1.0 / stil_own;
+      for (int a = tid; a < r; a += kClThreads) {
+        tv[a] = Sv[a + (size_t)apos * lds];
+        tpv[a] = Sv[apos + (size_t)a * lds];
+      }
+      __syncthreads();
+      for (int a = tid & 63; a < r; a += 64) {
+        const double ta = tv[a] * inv;
+        double* Sa = Sv + a;
+        for (int b = tid >> 6; b < r; b += 8) Sa[(size_t)b * lds] -= ta * tpv[b];
+      }
+      __syncthreads();
+      const int last = r - 1;
+      if (apos != last) {
+        for (int b = tid; b < r; b += kClThreads) Sv[apos + (size_t)b * lds] = Sv[last + (size_t)b * lds];
+        __syncthreads();
+        for (int a = tid; a < last; a += kClThreads) Sv[a + (size_t)apos * lds] = Sv[a + (size_t)last * lds];
+      }
+      if (tid == 0) {
+        jpos[slot - k0] = -1;
+        if (apos != last) {
+          const int moved = Js[last];
+          Js[apos] = moved;
+          if (moved >= k0) jpos[moved - k0] = apos;
+        }
+      }
+      for (int idx = tid; idx < len - 1; idx += kClThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
+      int* t = live; live = live_alt; live_alt = t;
+      --len; --kcur; ++acc_rem;
+      if (R < 0.0) sign = -sign;
+      --r;
+    } else if (accept) {
+      const double inv = 1.0 / stil_own;
+      for (int a = tid & 63; a < r; a += 64) {
+        const double ta = tv[a] * inv;
+        double* Sa = Sv + a;
+        for (int b = tid >> 6; b < r; b += 8) Sa[(size_t)b * lds] += ta * tpv[b];
+      }
+      for (int a = tid; a < r; a += kClThreads) {
+        Sv[a + (size_t)r * lds] = -tv[a] * inv;
+        Sv[r + (size_t)a * lds] = -tpv[a] * inv;
+      }
+      if (tid == 0) { Sv[r + (size_t)r * lds] = inv; Js[r] = slot; }
+      errlvl = fmax(errlvl, amp);
+      if (type == 0) {
+        if (tid == 0) {
+          live[len] = slot; jpos[slot - k0] = r;
+          if (sp == 0) c.cfg_id[off_old + slot] = next_id;
+        }
+        ++len; ++kcur; ++next_id; ++acc_ins;
+      } else {
+        for (int idx = tid; idx < len - 1; idx += kClThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
+        int* t = live; live = live_alt; live_alt = t;
+        --len; --kcur; ++acc_rem;
+      }
+      if (R < 0.0) sign = -sign;
+      ++r;
+    }
+    if (accept) __syncthreads();
+    --props_left; ++p;
+    if (props_left == 0) ++sweeps_done;
+    if (r == c.delay) break;
+  }
+  __syncthreads();
+  if (props_left == 0 && sweeps_left == 0) finished = true;
+
+  // ---- write back.  Each CTA: its own S^-1.  Rank 0: list, maps, scalars.
+  if (sinv_smem) {
+    double* Sg = c.Sinv + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.delay;
+    for (int a = tid & 63; a < r; a += 64)
+      for (int b = tid >> 6; b < r; b += 8) Sg[a + (size_t)b * c.ldr] = Sv[a + (size_t)b * lds];
+  }
+  cluster.sync();   // both CTAs are past every read of the walker state and of cfg_id before rank 0 rewrites them
+  if (sp == 0) {
+    int* rowmap = c.rowmap + (size_t)w * c.cap;
+    for (int i = tid; i < kcur; i += kClThreads) {
+      const int sl = live[i];
+      rowmap[i] = sl;
+      c.cfg_site[off_new + i] = c.cfg_site[off_old + sl];
+      c.cfg_tau[off_new + i] = c.cfg_tau[off_old + sl];
+      c.cfg_spin[off_new + i] = c.cfg_spin[off_old + sl];
+      c.cfg_id[off_new + i] = c.cfg_id[off_old + sl];
+    }
+    for (int a = tid; a < r; a += kClThreads) c.J[(size_t)w * c.delay + a] = Js[a];
+    if (tid == 0) {
+      st.k_new = kcur;
+      st.k = kcur;
+      st.m = k0;
+      st.cfg_cur = cfg_old ^ 1;
+      st.r = r;
+      st.n_src = n_cur0;
+      st.n_cur = r > 0 ? (n_cur0 ^ 1) : n_cur0;
+      st.next_id = next_id; st.p = p; st.sign = sign;
+      st.sweeps_left = sweeps_left; st.props_left = props_left;
+      st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
+      st.blocks += 1;
+      st.guard_ends += guard_end;
+      if (r > 0) { st.flushes += 1; st.sum_rank += r; }
+      st.log_count = log_count;
+      st.min_margin = min_margin; st.sum_k += sum_k;
+      st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
+      st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);
+      st.flops_usinv += 2.0 * (2.0 * (double)kcur * r * r);
+      if (status) st.status = status;
+      atomicMax(c.n_active + 1, kcur);
+      if (finished || status) {
+        st.active = 0;
+        atomicSub(c.n_active, 1);
+      }
+    }
+  }
+}
+
+}  // namespace ctaux

@@ -130,7 +130,9 @@ def test_config3_thermalised_start_N_1e10():
     assert sum(W.get_stats(w)["flushes"] for w in range(16)) > 500
 
 
-@pytest.mark.parametrize("delay,rebuild,cand", [(1, 0, 0), (8, 0, 3), (64, 3, 0), (16, 1, 40), (256, 0, 0)])
+# delay 128 / 256: the two-CTA cluster form of the S3 kernel (S^-1 of one spin per CTA in shared memory / in L2)
+@pytest.mark.parametrize("delay,rebuild,cand", [(1, 0, 0), (8, 0, 3), (64, 3, 0), (16, 1, 40), (128, 0, 0), (256, 0, 0),
+                                                (100, 0, 0)])
 def test_chain_independent_of_delay_rebuild_window(delay, rebuild, cand):
     """Q18-Q20: delay, rebuild cadence and the candidate window are performance knobs only."""
     cfg = get_config(1)
@@ -230,3 +232,12 @@ def test_config4_thermalised_start_N_1e10():
     oracle-thermalised configuration: 4 seeds x 1 sweep without rebuild, logs bit-exact, N within 1e-10."""
     cfg = get_config(3)
     parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(4), 1, T1)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("delay", [128, 256])
+def test_config4_thermalised_start_cluster_kernel(delay):
+    """Same start, delay 128 / 256 (config 5's delays): the S3 kernel runs as a two-CTA cluster per walker."""
+    cfg = get_config(3)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1, delay=delay)
+    assert max(W.get_stats(w)["sum_rank"] / max(W.get_stats(w)["flushes"], 1) for w in range(2)) > 0.5 * delay
