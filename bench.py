@@ -317,6 +317,10 @@ def run_gpu(args):
                     "launches": fl["launches"], "mean_rank": dk["sum_rank"] / max(dk["flushes"], 1),
                     "walkers_per_launch": B // G,
                     "timed": "kernel pass after the timed region: one more step, groups one after the other"}
+        if fl["launches"] == 0:   # fused small-k path: no flush GEMM exists; the walker is one latency-bound kernel
+            roofline = {"kernel": "k_walk_fused (whole sweeps in one kernel, N in shared memory; rank-1 updates)",
+                        "bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None, "traffic": None,
+                        "note": "dependent-latency bound chain (one CTA per walker): no roofline applies; see DESIGN.md section 9"}
         steps_ms = {k: v["ms"] for k, v in tim.items()}
         other = {"cand_gemm_tflops": dk["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
                  "rebuild_tflops": dk["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}

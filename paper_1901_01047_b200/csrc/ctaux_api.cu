@@ -546,7 +546,7 @@ int enqueue_block_step(ctaux_ctx* x) {
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
       const int tl = (kh + 63) / 64;
-      e4 = launch_gemm<GEMM_Q5>(DescFlush{d}, tl * tl, P, s);  // L2 prefetch of C0 measured: no gain
+      e4 = launch_gemm<GEMM_Q5>(DescFlush{d}, tl * tl, P, s);  // measured, no gain: L2 prefetch of C0; 2-8 tiles per CTA
     }
     CU_CHECK(e4);
     tick(x, C_FLUSH_GEMM);
