@@ -223,7 +223,7 @@ def diff(a, b):
     return {k: a[k] - b[k] for k in a if k != "k_mean"}
 
 
-DEFAULT_GROUPS = {"cfg4_6x6_b20": 4, "cfg5_6x6_b40": 2}
+DEFAULT_GROUPS = {"cfg3_4x4_b10": 4, "cfg4_6x6_b20": 4, "cfg5_6x6_b40": 2}
 
 
 def run_gpu(args):

@@ -255,6 +255,8 @@ struct ctaux_ctx {
                       // with events): when several contexts share the GPU its few CTAs must not queue behind
                       // thousands of GEMM CTAs of the other contexts
   cudaEvent_t ev_fork, ev_join;
+  bool lu_cluster;    // S5 panel factorisation on an 8-CTA cluster per matrix (large k)
+  int lu_cluster_smem;
   int cluster_mode;   // 0: k_propose (one CTA per walker); 1 / 2: k_propose_cl (2-CTA cluster per walker) with
                       // S^-1 in shared memory / in L2 -- used when S^-1 of both spins does not fit one CTA
   int cluster_smem;
@@ -433,7 +435,12 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     for (int j0 = 0; j0 < kmax; j0 += kLuNb) {  // factorisation + forward substitution
       Scoped t(x, C_REBUILD);
       const int j1 = j0 + kLuNb < kmax ? j0 + kLuNb : kmax;
-      k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, set_sign ? x->detsign : nullptr);
+      if (x->lu_cluster) {
+        const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
+        k_lu_panel_cl<<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, set_sign ? x->detsign : nullptr, rl_cap);
+      } else {
+        k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, set_sign ? x->detsign : nullptr);
+      }
       k_lu_swap<<<dim3(cb, P), 128, 0, s>>>(d, j0);
       k_lu_trsm<<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
       tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
@@ -713,6 +720,18 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       if (need > fused_attr_max) {
         if (cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, need) != cudaSuccess) x->fused = false;
         else fused_attr_max = need;
+      }
+    }
+  }
+  x->lu_cluster = false; x->lu_cluster_smem = 0;
+  if (d.max_k > 512) {
+    const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
+    const int need = (rl_cap * kLuPad + 2 * kLuNb + kLuCl) * 8 + kLuCl * 4 + 64;
+    if (need <= max_smem) {
+      if (cudaFuncSetAttribute(k_lu_panel_cl, cudaFuncAttributeMaxDynamicSharedMemorySize, need) == cudaSuccess) {
+        x->lu_cluster = true; x->lu_cluster_smem = need;
+      } else {
+        cudaGetLastError();
       }
     }
   }

@@ -15,6 +15,8 @@
 //   GEMM              : X[0:j0, :] -= U[0:j0, j0:j1] X[j0:j1, :]
 // The trailing updates run on the DMMA GEMM tiles of gemm_dmma.cuh.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "gemm_dmma.cuh"
 #include "walker_state.cuh"
 
@@ -103,6 +105,133 @@ __global__ void __launch_bounds__(1024) k_lu_panel(DevCtx c, int j0, int* detsig
       }
     }
     __syncthreads();
+  }
+}
+
+// Panel factorisation spread over a thread-block CLUSTER of 8 CTAs per matrix (large k): the rows j0..k of the
+// panel are dealt out in 8 contiguous slabs, each held in its CTA's shared memory for the whole panel, so the
+// kLuNb column steps run out of shared memory instead of streaming the panel through one SM's L2 port
+// (k_lu_panel: 200-600 us per panel at k = 1300-3600).  Per column: local pivot search, candidates exchanged
+// through distributed shared memory (cluster barrier), pivot row broadcast + row interchange (cluster barrier),
+// local elimination.  Same pivot choice as k_lu_panel (largest magnitude, smallest row index on ties).
+constexpr int kLuCl = 8;
+constexpr int kLuClThreads = 512;
+constexpr int kLuPad = kLuNb + 1;
+
+__global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
+    k_lu_panel_cl(DevCtx c, int j0, int* detsign, int rl_cap) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  extern __shared__ __align__(16) double lsm[];
+  const int prob = blockIdx.x / kLuCl, rank = (int)cluster.block_rank();
+  const int w = prob >> 1, sp = prob & 1;
+  WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (j0 >= k) return;                       // identical for all CTAs of the cluster
+  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+  const int nb = j1 - j0;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
+  const int ld = c.ld, tid = threadIdx.x;
+  const int rows = k - j0;
+  const int R = (rows + kLuCl - 1) / kLuCl;  // rows per CTA (<= rl_cap)
+  const int r0 = j0 + rank * R;              // first global row of this slab
+  int nloc = k - r0; if (nloc > R) nloc = R; if (nloc < 0) nloc = 0;
+  double* A = lsm;                           // [rl_cap][kLuPad] row-major: A[i*kLuPad + cc]
+  double* prow = lsm + (size_t)rl_cap * kLuPad;         // [kLuNb] pivot row of the current column
+  double* swp = prow + kLuNb;                          // [kLuNb] row `col` travelling to the pivot's slot
+  double* cval = swp + kLuNb;                          // [kLuCl] candidates
+  int* cidx = reinterpret_cast<int*>(cval + kLuCl);    // [kLuCl]
+  __shared__ double s_val[kLuClThreads / 32];
+  __shared__ int s_idx[kLuClThreads / 32];
+
+  for (int idx = tid; idx < nloc * nb; idx += kLuClThreads) {
+    const int i = idx % nloc, cc = idx / nloc;
+    A[i * kLuPad + cc] = F[(size_t)(j0 + cc) * ld + r0 + i];
+  }
+  cluster.sync();
+
+  for (int cc = 0; cc < nb; ++cc) {
+    const int col = j0 + cc;
+    // 1. local pivot candidate over the local rows with global index >= col
+    double best = -1.0;
+    int bi = 0x7fffffff;
+    for (int i = tid; i < nloc; i += kLuClThreads) {
+      const int gi = r0 + i;
+      if (gi >= col) {
+        const double v = fabs(A[i * kLuPad + cc]);
+        if (v > best || (v == best && gi < bi)) { best = v; bi = gi; }
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+    }
+    if ((tid & 31) == 0) { s_val[tid >> 5] = best; s_idx[tid >> 5] = bi; }
+    __syncthreads();
+    if (tid < kLuCl) {   // thread q publishes this CTA's candidate to CTA q
+      double b = s_val[0];
+      int ix = s_idx[0];
+      for (int q = 1; q < kLuClThreads / 32; ++q)
+        if (s_val[q] > b || (s_val[q] == b && s_idx[q] < ix)) { b = s_val[q]; ix = s_idx[q]; }
+      double* rv = cluster.map_shared_rank(cval, tid);
+      int* ri = cluster.map_shared_rank(cidx, tid);
+      rv[rank] = b; ri[rank] = ix;
+    }
+    cluster.sync();
+    // 2. global pivot
+    double pb = cval[0];
+    int pr = cidx[0];
+#pragma unroll
+    for (int q = 1; q < kLuCl; ++q)
+      if (cval[q] > pb || (cval[q] == pb && cidx[q] < pr)) { pb = cval[q]; pr = cidx[q]; }
+    const int qp = (pr - j0) / R, qc = (col - j0) / R;   // owners of the pivot row and of row `col`
+    if (rank == 0 && tid == 0) {
+      ipiv[col] = pr;
+      if (!(pb > 0.0)) st.status = -4;  // CTAUX_ESINGULAR
+    }
+    // 3. pivot row to everybody; row `col` to the pivot's owner
+    if (rank == qp && tid < kLuCl * kLuNb) {
+      const int q = tid / kLuNb, x = tid % kLuNb;
+      double* rp = cluster.map_shared_rank(prow, q);
+      rp[x] = x < nb ? A[(pr - r0) * kLuPad + x] : 0.0;
+    }
+    if (rank == qc && pr != col && tid >= kLuCl * kLuNb && tid < kLuCl * kLuNb + kLuNb) {
+      const int x = tid - kLuCl * kLuNb;
+      double* rs = cluster.map_shared_rank(swp, qp);
+      rs[x] = x < nb ? A[(col - r0) * kLuPad + x] : 0.0;
+    }
+    cluster.sync();
+    if (pr != col) {
+      if (rank == qp && tid < nb) A[(pr - r0) * kLuPad + tid] = swp[tid];
+      if (rank == qc && tid < nb) A[(col - r0) * kLuPad + tid] = prow[tid];
+    }
+    if (rank == 0 && tid == 0 && detsign) {
+      int sg = detsign[w * 2 + sp];
+      if (pr != col) sg = -sg;
+      if (prow[cc] < 0.0) sg = -sg;
+      detsign[w * 2 + sp] = sg;
+    }
+    __syncthreads();
+    // 4. elimination of the local rows below `col`
+    const double piv = prow[cc];
+    if (piv != 0.0) {
+      for (int i = tid; i < nloc; i += kLuClThreads) {
+        if (r0 + i > col) {
+          double* Ai = A + i * kLuPad;
+          const double l = Ai[cc] / piv;
+          Ai[cc] = l;
+          for (int x = cc + 1; x < nb; ++x) Ai[x] -= l * prow[x];
+        }
+      }
+    }
+    __syncthreads();
+  }
+  for (int idx = tid; idx < nloc * nb; idx += kLuClThreads) {
+    const int i = idx % nloc, cc = idx / nloc;
+    F[(size_t)(j0 + cc) * ld + r0 + i] = A[i * kLuPad + cc];
   }
 }
 

@@ -89,6 +89,15 @@ def test_reset_builds_inverse(ci, nw):
 
 # fused = 1: the single-kernel small-k path (walker_fused.cuh, what configs 1-2 run by default);
 # fused = -1: the delayed-block path (S2 GEMMs, S3 over the Gamma block, S4 flush) the large configs run.
+def test_rebuild_large_k_kernels_at_small_size():
+    """max_k > 512 selects the large-k kernels (64x64 4-warp GEMM tiles, split-K, the 8-CTA cluster LU panel):
+    S1 + S5 and a few sweeps against the oracle on config 3 with the capacity raised to 600."""
+    cfg = dict(get_config(2), max_k=600)
+    full_parity(cfg, 3, 10, T1)           # ends on a rebuild: N fresh from the cluster LU
+    W, orcs, worst = full_parity(cfg, 2, 0, T0)   # reset only: direct inverse of the random start
+    assert worst < 1e-10
+
+
 @pytest.mark.parametrize("fused", [1, -1])
 def test_config1_full_lockstep_T0(fused):
     """Config 1 in full (200 warm-up + 1000 sweeps, 1 walker, delay 8) against brute force T0."""
