@@ -250,3 +250,32 @@ def test_config4_thermalised_start_cluster_kernel(delay):
     cfg = get_config(3)
     W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1, delay=delay)
     assert max(W.get_stats(w)["sum_rank"] / max(W.get_stats(w)["flushes"], 1) for w in range(2)) > 0.5 * delay
+
+
+def test_error_codes_through_the_abi():
+    """Calls that are not valid fail with their CTAUX_E* code and leave the process alive."""
+    pkg = _pkg()
+    cfg = get_config(0)
+    table = table_for(cfg)
+    W = pkg.Walkers.from_config(cfg, table)
+    with pytest.raises(pkg.CtauxError) as ei:
+        W.sweep(1)                       # sweep before reset
+    assert ei.value.code == -5
+    with pytest.raises(pkg.CtauxError) as ei:
+        W.rebuild()
+    assert ei.value.code == -5
+    W.reset([3])
+    W.sweep(2)
+    L = pkg.load_library()
+    import ctypes as C
+    k = C.c_int32(0)
+    assert L.ctaux_get_config(W._h, 5, C.byref(k), None, None, None, None, 0) == -1      # walker out of range
+    assert L.ctaux_get_config(W._h, 0, C.byref(k), None, None, None, None, 0) == 0 and k.value == W.get_stats(0)["k"]
+    buf = np.zeros(4, np.int32)
+    assert L.ctaux_get_config(W._h, 0, C.byref(k), None, buf.ctypes.data, None, None, 1) == (-2 if k.value > 1 else 0)
+    assert L.ctaux_get_N(W._h, 0, 2, buf.ctypes.data, 64) == -1                             # spin out of range
+    assert L.ctaux_get_N(W._h, 0, 0, buf.ctypes.data, 0) == (-1 if k.value > 0 else 0)      # ld < k
+    W.close()
+    with pytest.raises(pkg.CtauxError) as ei:   # invalid parameters are refused before anything is allocated
+        pkg.Walkers(2, 2, 2.0, 4.0, 1.0, table, delay=300, n_walkers=1, init_k=1, max_k=64)
+    assert ei.value.code == -1
