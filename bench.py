@@ -324,6 +324,11 @@ def run_gpu(args):
         steps_ms = {k: v["ms"] for k, v in tim.items()}
         other = {"cand_gemm_tflops": dk["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
                  "rebuild_tflops": dk["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}
+        cand_tf = other["cand_gemm_tflops"]
+        roofline_s2 = {"kernel": "gemm_grouped_kernel<DescCandRows/Cols[SK]> (S2 candidate products, the largest share of a "
+                                 "large-k step; ncu: DMMA pipe 81 % busy, profiles/r1_v4_kernels_full.md)",
+                       "bound": "tensor", "achieved": cand_tf, "peak": fp64_peak, "unit": "TFLOP/s",
+                       "frac": cand_tf / fp64_peak if fp64_peak else None}
         out = {"metric": METRIC, "value": acc_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -336,7 +341,7 @@ def run_gpu(args):
                "mean_k_over_proposals": d["sum_k"] / max(d["proposals"], 1),
                "acceptance": acc / max(d["proposals"], 1),
                "blocks": int(d["blocks"]), "guard_ends": int(d["guard_ends"]),
-               "gpu_launches": int(l1 - l0), "roofline": roofline, "kernel_pass_ms_by_class": steps_ms, "gemm": other}
+               "gpu_launches": int(l1 - l0), "roofline": roofline, "roofline_s2": roofline_s2, "kernel_pass_ms_by_class": steps_ms, "gemm": other}
         out["clocks"] = clk.summary()
     return W, cfg, table, out, (rank, world, local)
 
