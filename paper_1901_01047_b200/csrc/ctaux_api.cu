@@ -553,7 +553,21 @@ int enqueue_block_step(ctaux_ctx* x) {
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
       const int tl = (kh + 63) / 64;
-      e4 = launch_gemm<GEMM_Q5>(DescFlush{d}, tl * tl, P, s);  // measured, no gain: L2 prefetch of C0; 2-8 tiles per CTA
+      // measured, no gain: L2 prefetch of C0; 2-8 tiles per CTA.  Gain: compaction-map loads issued before the descriptor.
+      {
+        using Cfg = GemmCfg<64, 64, 2, 2, 2>;
+        auto kern = gemm_flush_kernel<GEMM_Q5, DescFlush>;
+        static bool configured = false;
+        e4 = cudaSuccess;
+        if (!configured) {
+          e4 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+          configured = e4 == cudaSuccess;
+        }
+        if (e4 == cudaSuccess) {
+          kern<<<dim3(tl * tl, P), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(DescFlush{d}, d.rowmap, d.cap, tl);
+          e4 = cudaGetLastError();
+        }
+      }
     }
     CU_CHECK(e4);
     tick(x, C_FLUSH_GEMM);

@@ -61,8 +61,9 @@ struct GemmCfg {
 };
 
 // One CTA computes one BM x BN tile of one problem.
-template <int BM, int BN, int WM, int WN, int STAGES>
-__device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int tile_n, double* smem) {
+template <int BM, int BN, int WM, int WN, int STAGES, bool PRE = false>
+__device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int tile_n, double* smem,
+                                          const int* pre_srow = nullptr, const int* pre_scol = nullptr) {
   using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
   constexpr int BK = Cfg::BK, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
   constexpr int TM = Cfg::TM, TN = Cfg::TN, THREADS = Cfg::THREADS;
@@ -81,14 +82,16 @@ __device__ __forceinline__ void gemm_tile(const GemmDesc& d, int tile_m, int til
 #pragma unroll
   for (int i = 0; i < TM; ++i) {
     crow[i] = m0 + wm * (TM * 8) + i * 8 + g;
-    srow[i] = (d.rowmap && crow[i] < M) ? d.rowmap[crow[i]] : crow[i];
+    if (PRE) srow[i] = pre_srow[i];
+    else srow[i] = (d.rowmap && crow[i] < M) ? d.rowmap[crow[i]] : crow[i];
   }
 #pragma unroll
   for (int j = 0; j < TN; ++j)
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       ccol[j][h] = n0 + wn * (TN * 8) + j * 8 + 2 * q + h;
-      scol[j][h] = (d.colmap && ccol[j][h] < N) ? d.colmap[ccol[j][h]] : ccol[j][h];
+      if (PRE) scol[j][h] = pre_scol[j * 2 + h];
+      else scol[j][h] = (d.colmap && ccol[j][h] < N) ? d.colmap[ccol[j][h]] : ccol[j][h];
     }
   const int nk = (K + BK - 1) / BK;
 
@@ -247,6 +250,34 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn
     gemm_tile<BM, BN, WM, WN, STAGES>(d, t % tm, t / tm, smem_gemm);
     __syncthreads();
   }
+}
+
+// Flush form of the grouped kernel: the tile -> (tile_m, tile_n) mapping uses a host-side tile count `tmax`
+// instead of the problem's own size, so every CTA can issue the loads of its compaction-map entries
+// (map of problem p at maps + (p >> 1) * map_stride, rows and columns alike) BEFORE the device-side descriptor
+// has arrived: the dependent chain  descriptor -> maps -> C0  loses one L2 round trip per CTA.
+// Tiles beyond the live size exit; the map array has at least tmax * BM entries.
+template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class DescFn>
+__global__ void __launch_bounds__(WM * WN * 32, MINB)
+    gemm_flush_kernel(DescFn fn, const int* maps, int map_stride, int tmax) {
+  extern __shared__ __align__(16) double smem_gemm[];
+  using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
+  constexpr int TM = Cfg::TM, TN = Cfg::TN;
+  const int tile_m = blockIdx.x % tmax, tile_n = blockIdx.x / tmax;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int wm = warp % WM, wn = warp / WM, g = lane >> 2, q = lane & 3;
+  const int* map = maps + (size_t)(blockIdx.y >> 1) * map_stride;
+  int psrow[TM], pscol[TN * 2];
+#pragma unroll
+  for (int i = 0; i < TM; ++i) psrow[i] = __ldg(map + tile_m * BM + wm * (TM * 8) + i * 8 + g);
+#pragma unroll
+  for (int j = 0; j < TN; ++j)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) pscol[j * 2 + h] = __ldg(map + tile_n * BN + wn * (TN * 8) + j * 8 + 2 * q + h);
+  GemmDesc d;
+  if (!fn(blockIdx.y, d)) return;
+  if (tile_m * BM >= d.M || tile_n * BN >= d.N) return;
+  gemm_tile<BM, BN, WM, WN, STAGES, true>(d, tile_m, tile_n, smem_gemm, psrow, pscol);
 }
 
 }  // namespace ctaux
