@@ -154,6 +154,14 @@ int ctaux_get_config(ctaux_ctx* ctx, int32_t walker, int32_t* k, uint64_t* id, i
  * into a HOST buffer, rows/columns in list order.  This is the incrementally updated matrix. */
 int ctaux_get_N(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N, int32_t ld);
 
+/* Batched read-out (one synchronisation for the whole context).  k: HOST [n_walkers]; id / site / tau / spin:
+ * HOST [n_walkers][max_k] (walker w at offset w*max_k, list order), any of them may be NULL. */
+int ctaux_get_config_all(ctaux_ctx* ctx, int32_t* k, uint64_t* id, int32_t* site, double* tau, int8_t* spin);
+
+/* Every N_sigma of the context into one HOST buffer: matrix (w, spin) is k_w x k_w, column-major with leading
+ * dimension k_w, at offset (2*w + spin) * max_k * max_k doubles.  `N` should be pinned for full PCIe rate. */
+int ctaux_get_N_all(ctaux_ctx* ctx, double* N);
+
 /* Same matrix, copied device-to-device into a DEVICE buffer (no host staging). */
 int ctaux_get_N_device(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N_dev, int32_t ld);
 

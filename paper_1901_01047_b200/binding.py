@@ -40,7 +40,7 @@ class _Stats(C.Structure):
 
 
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
-           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_N", "ctaux_get_N_device", "ctaux_get_stats",
+           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats",
            "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_dgemm_ex", "ctaux_debug_philox"]
 
@@ -70,6 +70,8 @@ def load_library():
     L.ctaux_rebuild.argtypes = [vp]
     L.ctaux_get_config.argtypes = [vp, i32, C.POINTER(i32), vp, vp, vp, vp, i32]
     L.ctaux_get_N.argtypes = [vp, i32, i32, vp, i32]
+    L.ctaux_get_config_all.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.ctaux_get_N_all.argtypes = [vp, vp]
     L.ctaux_get_N_device.argtypes = [vp, i32, i32, vp, i32]
     L.ctaux_get_stats.argtypes = [vp, i32, C.POINTER(_Stats)]
     L.ctaux_get_log.restype = i64
@@ -205,13 +207,43 @@ class Walkers:
         return dict(id=ids[:n].copy(), site=site[:n].copy(), tau=tau[:n].copy(), spin=spin[:n].copy())
 
     def get_N(self, w, spin):
-        """k x k numpy array (row index = first index), list order."""
+        """k x k numpy array (row index = first index, Fortran order), list order.  The device-to-host copy
+        lands in a pinned staging buffer (full PCIe rate) and is copied out once."""
         st = self.get_stats(w)
         k = st["k"]
-        buf = np.zeros((k, k), np.float64, order="F")
-        if k:
-            _check(self._L.ctaux_get_N(self._h, w, spin, buf.ctypes.data, k), "ctaux_get_N")
-        return np.ascontiguousarray(buf)
+        if not k:
+            return np.zeros((0, 0), np.float64)
+        if getattr(self, "_pin", None) is None:
+            self._pin = self._torch.empty(self.max_k * self.max_k, dtype=self._torch.float64, pin_memory=True)
+        stage = self._pin[:k * k].numpy()
+        _check(self._L.ctaux_get_N(self._h, w, spin, stage.ctypes.data, k), "ctaux_get_N")
+        return stage.reshape((k, k), order="F").copy(order="F")
+
+    def get_config_all(self):
+        """Configurations of all walkers with one synchronisation: list of dicts (id, site, tau, spin)."""
+        B, mk = self.n_walkers, self.max_k
+        k = np.zeros(B, np.int32)
+        ids, site = np.zeros((B, mk), np.uint64), np.zeros((B, mk), np.int32)
+        tau, spin = np.zeros((B, mk), np.float64), np.zeros((B, mk), np.int8)
+        _check(self._L.ctaux_get_config_all(self._h, k.ctypes.data, ids.ctypes.data, site.ctypes.data,
+                                            tau.ctypes.data, spin.ctypes.data), "ctaux_get_config_all")
+        return [dict(id=ids[w, :k[w]].copy(), site=site[w, :k[w]].copy(), tau=tau[w, :k[w]].copy(),
+                     spin=spin[w, :k[w]].copy()) for w in range(B)]
+
+    def get_N_all(self, ks):
+        """All N_sigma through one pinned buffer and one call: list of (N_up, N_down) views (Fortran order) into
+        a pinned staging tensor that the next get_N_all overwrites."""
+        B, mk = self.n_walkers, self.max_k
+        if getattr(self, "_pin_all", None) is None:
+            self._pin_all = self._torch.empty(B * 2 * mk * mk, dtype=self._torch.float64, pin_memory=True)
+        flat = self._pin_all.numpy()
+        _check(self._L.ctaux_get_N_all(self._h, flat.ctypes.data), "ctaux_get_N_all")
+        out = []
+        for w in range(B):
+            k = int(ks[w])
+            out.append(tuple(flat[(2 * w + s) * mk * mk:(2 * w + s) * mk * mk + k * k].reshape((k, k), order="F")
+                             for s in range(2)))
+        return out
 
     def get_N_device(self, w, spin):
         torch = self._torch
@@ -314,6 +346,24 @@ class WalkerGroups:
 
     def launch_count(self):
         return sum(W.launch_count() for W in self.groups)
+
+    def fetch_all(self, with_N=True):
+        """(configs, stats, N) of every walker in job order, the groups read out concurrently (one host thread
+        and one pinned staging buffer per group).  N[w] = (N_up, N_down) or None."""
+        cfgs = [None] * self.n_walkers
+        stats = [None] * self.n_walkers
+        Ns = [None] * self.n_walkers
+
+        def one(W, g):
+            lo = g * self.per
+            cfgs[lo:lo + self.per] = W.get_config_all()
+            for i in range(self.per):
+                stats[lo + i] = W.get_stats(i)
+            if with_N:
+                Ns[lo:lo + self.per] = W.get_N_all([len(c["site"]) for c in cfgs[lo:lo + self.per]])
+
+        self._each(one)
+        return cfgs, stats, Ns
 
     def timing_enable(self, on=True):
         for W in self.groups:

@@ -911,6 +911,49 @@ int ctaux_get_N_device(ctaux_ctx* x, int32_t w, int32_t sp, double* N, int32_t l
   return get_N_impl(x, w, sp, N, ld, cudaMemcpyDeviceToDevice);
 }
 
+int ctaux_get_config_all(ctaux_ctx* x, int32_t* k, uint64_t* id, int32_t* site, double* tau, int8_t* spin) {
+  if (!x || !k) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  std::vector<WalkerState> h(d.B);
+  CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+  std::vector<int32_t> tmp(spin ? d.max_k : 0);
+  for (int w = 0; w < d.B; ++w) {
+    const int kw = h[w].k;
+    k[w] = kw;
+    if (kw == 0) continue;
+    const size_t off = ((size_t)w * 2 + h[w].cfg_cur) * d.cap, dst = (size_t)w * d.max_k;
+    if (id) CU_CHECK(cudaMemcpyAsync(id + dst, d.cfg_id + off, 8 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
+    if (site) CU_CHECK(cudaMemcpyAsync(site + dst, d.cfg_site + off, 4 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
+    if (tau) CU_CHECK(cudaMemcpyAsync(tau + dst, d.cfg_tau + off, 8 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
+    if (spin) {
+      CU_CHECK(cudaMemcpy(tmp.data(), d.cfg_spin + off, 4 * (size_t)kw, cudaMemcpyDeviceToHost));
+      for (int i = 0; i < kw; ++i) spin[dst + i] = (int8_t)tmp[i];
+    }
+  }
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  return CTAUX_OK;
+}
+
+int ctaux_get_N_all(ctaux_ctx* x, double* N) {
+  if (!x || !N) return CTAUX_EINVAL;
+  const DevCtx& d = x->d;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  std::vector<WalkerState> h(d.B);
+  CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+  for (int w = 0; w < d.B; ++w) {
+    const int kw = h[w].k;
+    if (kw == 0) continue;
+    for (int sp = 0; sp < 2; ++sp) {
+      const double* src = d.Nbuf + (((size_t)w * 2 + sp) * 2 + h[w].n_cur) * (size_t)d.ld * d.ld;
+      double* dst = N + ((size_t)w * 2 + sp) * (size_t)d.max_k * d.max_k;
+      CU_CHECK(cudaMemcpy2DAsync(dst, (size_t)kw * 8, src, (size_t)d.ld * 8, (size_t)kw * 8, kw, cudaMemcpyDeviceToHost, x->stream));
+    }
+  }
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  return CTAUX_OK;
+}
+
 int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   if (!x || w < 0 || w >= x->d.B || !out) return CTAUX_EINVAL;
   CU_CHECK(cudaStreamSynchronize(x->stream));

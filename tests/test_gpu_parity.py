@@ -279,3 +279,20 @@ def test_error_codes_through_the_abi():
     with pytest.raises(pkg.CtauxError) as ei:   # invalid parameters are refused before anything is allocated
         pkg.Walkers(2, 2, 2.0, 4.0, 1.0, table, delay=300, n_walkers=1, init_k=1, max_k=64)
     assert ei.value.code == -1
+
+
+def test_batched_readout_equals_per_walker_readout():
+    pkg = _pkg()
+    cfg = get_config(1)
+    W = pkg.Walkers.from_config(cfg, table_for(cfg), n_walkers=5)
+    W.reset(walker_seeds(5, first=7))
+    W.sweep(3)
+    cfgs = W.get_config_all()
+    Ns = W.get_N_all([len(c["site"]) for c in cfgs])
+    for w in range(5):
+        one = W.get_config(w)
+        for f in one:
+            assert one[f].tobytes() == cfgs[w][f].tobytes()
+        for s in range(2):
+            assert np.array_equal(W.get_N(w, s), Ns[w][s])
+    W.close()
