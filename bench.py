@@ -250,6 +250,8 @@ def run_gpu(args):
     # replicas only: rank r runs its own walkers with disjoint seeds
     seeds = rank_seeds(rank, B)
     fp64_dgemm = measure_fp64_peak(dev) if rank == 0 else 0.0
+    from paper_1901_01047_b200 import probe_fp64
+    fp64_dmma = probe_fp64(0) if rank == 0 else 0.0
     W = WalkerGroups(G, B, lambda g, nb, stream: Walkers.from_config(
         cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream))
     W.reset(seeds)
@@ -309,6 +311,7 @@ def run_gpu(args):
                                 delay == cfg["delay"] else None),
                     "algorithmic_bytes": 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),   # read + write of N, both spins
                     "peak_source": "cuBLAS DGEMM 8192^3 measured live in this run (FP64 runs at max SM clock: no power cap)",
+                    "peak_dmma_issue_rate": fp64_dmma,
                     "peak_alt": fp64_alt,
                     "peak_alt_source": f"{peaks['source']} bf16 sustained {peaks['bf16_sustained']:.1f} TF x nominal FP64:bf16 "
                                        f"{NOMINAL_FP64_TFLOPS:g}:{NOMINAL_BF16_TFLOPS:g}",

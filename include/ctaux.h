@@ -201,6 +201,11 @@ int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, 
                    int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc,
                    int32_t kernel);
 
+/* Measurement helper: issue-rate peak of the FP64 pipes on the current device, TFLOP/s.  which = 0: DMMA.8x8x4
+ * (mma.sync m8n8k4 f64, the tensor path the GEMM tiles use), 1: DFMA.  One CTA of 256 threads per SM x 2,
+ * 16 independent accumulators per warp / thread, CUDA events.  The roofline ceiling beside cuBLAS DGEMM. */
+int ctaux_probe_fp64(int32_t which, double* tflops);
+
 /* Debug / pin helper: Philox4x32-10 evaluated ON THE DEVICE for n (counter, key) pairs.
  * ctr: HOST [n][4], key: HOST [n][2], out: HOST [n][4]. */
 int ctaux_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int32_t n);

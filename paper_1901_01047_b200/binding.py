@@ -42,7 +42,7 @@ class _Stats(C.Structure):
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats",
            "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
-           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_dgemm_ex", "ctaux_debug_philox"]
+           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_dgemm_ex", "ctaux_probe_fp64", "ctaux_debug_philox"]
 
 _lib = None
 
@@ -87,6 +87,7 @@ def load_library():
     L.ctaux_last_cuda_error.restype = C.c_char_p
     L.ctaux_dgemm.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32]
     L.ctaux_dgemm_ex.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32]
+    L.ctaux_probe_fp64.argtypes = [i32, C.POINTER(C.c_double)]
     L.ctaux_debug_philox.argtypes = [vp, vp, vp, i32]
     _lib = L
     return L
@@ -420,6 +421,14 @@ def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, kernel=0):
     _check(L.ctaux_dgemm_ex(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
                             C_out.data_ptr(), ld(C_out), kernel), "ctaux_dgemm_ex")
     return C_out
+
+
+def probe_fp64(which=0):
+    """Issue-rate peak of the FP64 tensor (0: DMMA.8x8x4) or vector (1: DFMA) pipe, TFLOP/s."""
+    L = load_library()
+    v = C.c_double(0.0)
+    _check(L.ctaux_probe_fp64(which, C.byref(v)), "ctaux_probe_fp64")
+    return v.value
 
 
 def debug_philox(ctr, key):

@@ -491,8 +491,8 @@ int enqueue_block_step(ctaux_ctx* x) {
       e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (kcap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
       const int t1 = (d.mmax + 63) / 64 * ((kh + 63) / 64), t2 = (kcap + 63) / 64 * ((d.mmax + 63) / 64);
-      // split-K factor: aim at >= 1.5 waves of the 148 x 4 CTA slots, chunks of at least 128
-      int S = (6 * sm_count() + P * t1 - 1) / (P * t1);
+      // split-K factor: aim at >= 3 waves of the 148 x 4 CTA slots (measured optimum), chunks of at least 128
+      int S = (12 * sm_count() + P * t1 - 1) / (P * t1);
       if (S > kMaxSplitK) S = kMaxSplitK;
       while (S > 1 && kh / S < 128) --S;
       if (S <= 1) {
@@ -1037,6 +1037,64 @@ int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, 
     default: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st, 4 * sm_count()); break;  // 8: with L2 prefetch of C0
   }
   CU_CHECK(e);
+  return CTAUX_OK;
+}
+
+}  // extern "C" (interrupted for two probe kernels)
+
+namespace {
+__global__ void k_probe_dmma(double* out, int iters) {
+  double acc[16][2];
+  for (int i = 0; i < 16; ++i) { acc[i][0] = threadIdx.x; acc[i][1] = i; }
+  const double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) dmma884(acc[i][0], acc[i][1], a, b);
+  }
+  double s = 0;
+  for (int i = 0; i < 16; ++i) s += acc[i][0] + acc[i][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void k_probe_dfma(double* out, int iters) {
+  double acc[16];
+  for (int i = 0; i < 16; ++i) acc[i] = threadIdx.x + i;
+  const double a = 1.0 + threadIdx.x * 1e-9, b = 1e-9;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc[i] = fma(acc[i], a, b);
+  }
+  double s = 0;
+  for (int i = 0; i < 16; ++i) s += acc[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+extern "C" {
+
+int ctaux_probe_fp64(int32_t which, double* tflops) {
+  if (!tflops || which < 0 || which > 1) return CTAUX_EINVAL;
+  const int blocks = 2 * sm_count(), threads = 256, iters = 20000;
+  double* out = nullptr;
+  CU_CHECK(cudaMalloc((void**)&out, (size_t)blocks * threads * 8));
+  cudaEvent_t e0, e1;
+  CU_CHECK(cudaEventCreate(&e0));
+  CU_CHECK(cudaEventCreate(&e1));
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {   // first repetition = warm-up
+    cudaEventRecord(e0);
+    if (which == 0) k_probe_dmma<<<blocks, threads>>>(out, iters);
+    else k_probe_dfma<<<blocks, threads>>>(out, iters);
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = which == 0 ? (double)blocks * (threads / 32) * iters * 16.0 * 512.0   // m8n8k4 = 512 flop
+                                 : (double)blocks * threads * iters * 16.0 * 2.0;
+    if (rep > 0 && ms > 0.f && fl / ms / 1e9 > best) best = fl / ms / 1e9;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+  CU_CHECK(cudaGetLastError());
+  *tflops = best;
   return CTAUX_OK;
 }
 
