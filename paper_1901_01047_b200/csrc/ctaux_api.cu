@@ -495,6 +495,7 @@ int enqueue_block_step(ctaux_ctx* x) {
       int S = (12 * sm_count() + P * t1 - 1) / (P * t1);
       if (S > kMaxSplitK) S = kMaxSplitK;
       while (S > 1 && kh / S < 128) --S;
+      if (d.max_k <= 512) S = 1;   // the split-K scratch exists only for the large configurations
       if (S <= 1) {
         e1 = launch_gemm<GEMM_Q4>(DescCandRows{d}, t1, P, s);
         e2 = launch_gemm<GEMM_Q4>(DescCandCols{d}, t2, P, s);
@@ -773,7 +774,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       }
     }
   }
-  x->small_tiles = d.max_k <= 512;
+  x->small_tiles = d.max_k <= 512;   // (64x64 / 4-warp tiles on config 3, k = 245: measured, no gain)
   // The persistent kernel (gemm_persist.cuh) hides the C0 latency of the flush but its main loop is slower
   // than two independent 8-warp CTAs per SM (profiles/r1_gemm_variants.md); off until that is fixed.
   x->persist = false && !x->small_tiles && 2 * d.B <= kPMaxProblems;
