@@ -375,7 +375,7 @@ def run_e2e(W, cfg, B, S, steps, rank):
     dt = time.perf_counter() - t0
     return {"value": acc / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d / steps), "d2h_bytes_per_step": int(d2h / steps),
             "steps": steps, "ms_per_step": 1e3 * dt / steps,
-            "what": "ctaux_set_state(host arrays) + ctaux_sweep + ctaux_get_config/get_N to host, every step"}
+            "what": "ctaux_set_state(host arrays) + ctaux_sweep + ctaux_get_config_all/get_N_all to pinned host buffers, every step"}
 
 
 def main():
