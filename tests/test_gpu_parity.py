@@ -296,3 +296,33 @@ def test_batched_readout_equals_per_walker_readout():
         for s in range(2):
             assert np.array_equal(W.get_N(w, s), Ns[w][s])
     W.close()
+
+
+@pytest.mark.parametrize("fused", [1, -1])
+def test_walker_groups_run_the_same_chains(fused):
+    """WalkerGroups (walkers split over contexts / streams / host threads) against one context: identical
+    configurations, counters and N for every walker; batched fetch_all equals the per-walker getters."""
+    pkg = _pkg()
+    cfg = get_config(1)
+    table = table_for(cfg)
+    B, G, ns = 6, 3, 7
+    seeds = walker_seeds(B, first=40)
+    one = pkg.Walkers.from_config(cfg, table, n_walkers=B, fused_small=fused)
+    one.reset(seeds)
+    one.sweep(ns)
+    grp = pkg.WalkerGroups(G, B, lambda g, nb, stream: pkg.Walkers.from_config(cfg, table, n_walkers=nb, stream=stream,
+                                                                                 fused_small=fused))
+    grp.reset(seeds)
+    grp.sweep(3)
+    grp.sweep(ns - 3)
+    cfgs, stats, Ns = grp.fetch_all()
+    for w in range(B):
+        compare_configs(cfgs[w], one.get_config(w), f"group walker {w}")
+        s1 = one.get_stats(w)
+        for f in ("k", "proposals", "next_id", "sign", "acc_ins", "acc_rem", "sweeps"):
+            assert stats[w][f] == s1[f], (w, f)
+        for s in range(2):
+            assert frob_rel(Ns[w][s], one.get_N(w, s)) < 1e-10
+            assert np.array_equal(Ns[w][s], grp.get_N(w, s))
+    grp.close()
+    one.close()
