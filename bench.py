@@ -253,7 +253,8 @@ def run_gpu(args):
     from paper_1901_01047_b200 import probe_fp64
     fp64_dmma = probe_fp64(0) if rank == 0 else 0.0
     W = WalkerGroups(G, B, lambda g, nb, stream: Walkers.from_config(
-        cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream))
+        cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream,
+        rebuild_mode=args.rebuild_mode))
     W.reset(seeds)
     stream = torch.cuda.current_stream()
 
@@ -337,7 +338,7 @@ def run_gpu(args):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
                           "K": cfg["K"], "walkers_per_gpu": B, "stream_groups": G, "delay": delay, "sweeps_per_step": S,
-                          "rebuild_every": S, "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
+                          "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh", "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
                           "working set fits L2 (latency-bound chain; no flush between steps)",
                           "parallelism": "replicas only"},
                "proposals_per_s": props_all / (ms_max * 1e-3), "k_mean": s1["k_mean"],
@@ -389,6 +390,8 @@ def main():
     ap.add_argument("--delay", type=int, default=0)
     ap.add_argument("--sweeps-per-step", type=int, default=0)
     ap.add_argument("--groups", type=int, default=0, help="stream groups the walkers are split over (0 = per-config default)")
+    ap.add_argument("--rebuild-mode", type=int, default=0, choices=[0, 1],
+                    help="periodic rebuild: 0 = from-scratch LU (default, BASELINE.json), 1 = Newton-Schulz refresh (two GEMMs)")
     ap.add_argument("--cand-window", type=int, default=0, help="insertion candidates pre-expanded per block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

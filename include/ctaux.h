@@ -85,6 +85,12 @@ typedef struct ctaux_params {
                               fit), -1 = never.  The fused kernel runs whole sweeps of a walker in one launch
                               with N in shared memory and applies every accepted move at once (delay and
                               cand_window are ignored there: they are chain-neutral knobs).              */
+  int32_t rebuild_mode;    /* periodic rebuild of N: 0 = from scratch, blocked LU with partial pivoting (the default and
+                              what ctaux_reset / ctaux_set_state / ctaux_rebuild always do); 1 = refresh by one
+                              Newton-Schulz step N <- N (2 - A N) with A rebuilt from the configuration -- two dense
+                              FP64 GEMMs instead of the latency-bound LU; quadratic, so an N that has drifted to
+                              1e-9 comes back to rounding level.  Falls back to LU when max|A N - 1| > 1e-4.
+                              Chain-neutral like every rebuild.  Needs one more k x k buffer per matrix.     */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */

@@ -278,7 +278,7 @@ namespace {
 
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
-      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, total;
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -306,6 +306,7 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
     const size_t a = (size_t)d.ldm * d.cap, b = (size_t)d.ld * d.mmax;
     d.skstride = a > b ? a : b;
   }
+  d.Tbuf = p->rebuild_mode == 1 ? reinterpret_cast<double*>(1) : nullptr;   // flag for make_layout; set for real in create
   d.log_capacity = p->log_capacity;
   d.beta = p->beta; d.K = p->K; d.tau_scale = (double)p->n_tau / p->beta;
   // Eq. (25): cosh(gamma) = 1 + U beta Ncorr / (2K)
@@ -347,6 +348,8 @@ Layout make_layout(const DevCtx& d) {
   L.detsign = take(B * 2 * 4);
   L.seeds = take(B * 8);
   L.skbuf = take(d.max_k > 512 ? B * 2 * kMaxSplitK * d.skstride * 8 : 0);
+  L.Tbuf = take(d.Tbuf ? B * 2 * (size_t)d.ld * d.ld * 8 : 0);   // d.Tbuf != null here only flags rebuild_mode 1
+  L.resid = take(B * 2 * 8);
   L.total = o;
   return L;
 }
@@ -409,6 +412,40 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
   int kmax = 0;
   for (int w = 0; w < d.B; ++w) kmax = h[w].k > kmax ? h[w].k : kmax;
   x->k_hint = kmax;
+  if (d.Tbuf && !set_sign && count && kmax > 0) {
+    // rebuild_mode 1: Newton-Schulz refresh, two GEMMs; falls back to the LU below when A N is not close to 1
+    const int P = d.B * 2;
+    const int gb = grid_for((size_t)kmax * kmax, 256, 1024);
+    const int t64 = ((kmax + 63) / 64) * ((kmax + 63) / 64);
+    {
+      Scoped t(x, C_REBUILD);
+      CU_CHECK(cudaMemsetAsync(d.resid, 0, sizeof(unsigned long long) * P, s));
+      k_build_A<<<dim3(gb, P), 256, 0, s>>>(d, 1);
+      cudaError_t e = x->small_tiles ? launch_gemm<GEMM_SMALL>(DescNS{d, 0}, t64, P, s) : launch_gemm<GEMM_Q4>(DescNS{d, 0}, t64, P, s);
+      CU_CHECK(e);
+      k_ns_resid<<<dim3(gb > 256 ? 256 : gb, P), 256, 0, s>>>(d);
+      tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
+    }
+    std::vector<unsigned long long> hr(P);
+    CU_CHECK(cudaMemcpyAsync(hr.data(), d.resid, sizeof(unsigned long long) * P, cudaMemcpyDeviceToHost, s));
+    CU_CHECK(cudaStreamSynchronize(s));
+    harvest_timing(x);
+    double worst = 0.0;
+    for (int q = 0; q < P; ++q) { double v; memcpy(&v, &hr[q], 8); worst = v > worst ? v : worst; }
+    if (worst < 1e-4) {
+      {
+        Scoped t(x, C_REBUILD);
+        cudaError_t e = x->small_tiles ? launch_gemm<GEMM_SMALL>(DescNS{d, 1}, t64, P, s) : launch_gemm<GEMM_Q4>(DescNS{d, 1}, t64, P, s);
+        CU_CHECK(e);
+        k_ns_flip<<<(d.B + 127) / 128, 128, 0, s>>>(d);
+        tick(x, C_REBUILD); tick(x, C_OTHER);
+      }
+      CU_CHECK(cudaGetLastError());
+      CU_CHECK(cudaStreamSynchronize(s));
+      harvest_timing(x);
+      return CTAUX_OK;
+    }
+  }
   if (set_sign) {
     std::vector<int> ones(d.B * 2, 1);
     CU_CHECK(cudaMemcpyAsync(x->detsign, ones.data(), sizeof(int) * d.B * 2, cudaMemcpyHostToDevice, s));
@@ -679,6 +716,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   d.log = (LogEntry*)(base + L.log); d.n_active = (int32_t*)(base + L.n_active);
   d.colbuf = (double*)(base + L.colbuf); d.rowbuf = (double*)(base + L.rowbuf); d.perm = (int32_t*)(base + L.perm);
   d.skbuf = (double*)(base + L.skbuf);
+  d.Tbuf = prm->rebuild_mode == 1 ? (double*)(base + L.Tbuf) : nullptr;
+  d.resid = (unsigned long long*)(base + L.resid);
   x->detsign = (int*)(base + L.detsign);
   x->seeds_d = (uint64_t*)(base + L.seeds);
   d.g00 = -prm->g0_table[0];

@@ -354,4 +354,56 @@ struct DescLU {
   }
 };
 
+// ---- rebuild_mode 1: Newton-Schulz refresh  N <- N (2 - A N) = 2 N - N (A N)
+// A_sigma is built (k_build_A) into the spare N buffer; T = A N goes to Tbuf; the new N overwrites A.
+struct DescNS {
+  DevCtx c;
+  int stage;  // 0: T = A * N;  1: N_new = 2 N - N * T
+  __device__ bool operator()(int prob, GemmDesc& d) const {
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    const int k = st.k;
+    if (k == 0) return false;
+    double* Ncur = c.N(w, sp, st.n_cur);
+    double* Oth = c.N(w, sp, st.n_cur ^ 1);
+    double* T = c.Tbuf + ((size_t)w * 2 + sp) * (size_t)c.ld * c.ld;
+    d.M = k; d.N = k; d.K = k;
+    d.lda = c.ld; d.ldb = c.ld; d.ldc = c.ld; d.ldc0 = c.ld;
+    d.rowmap = nullptr; d.colmap = nullptr;
+    if (stage == 0) {
+      d.A = Oth; d.B = Ncur; d.C = T; d.C0 = nullptr; d.alpha = 1.0; d.beta = 0.0;
+    } else {
+      d.A = Ncur; d.B = T; d.C = Oth; d.C0 = Ncur; d.alpha = -1.0; d.beta = 2.0;
+    }
+    return true;
+  }
+};
+
+__global__ void k_ns_resid(DevCtx c) {   // resid[prob] = max |T - 1|
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const int k = c.ws[w].k;
+  const double* T = c.Tbuf + ((size_t)w * 2 + sp) * (size_t)c.ld * c.ld;
+  double mx = 0.0;
+  const size_t total = (size_t)k * k;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % k), j = (int)(idx / k);
+    const double v = fabs(T[(size_t)j * c.ld + i] - (i == j ? 1.0 : 0.0));
+    mx = v > mx ? v : mx;   // NaN never wins here; it is caught below
+    if (!(v == v)) mx = 1e300;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(c.resid + blockIdx.y, (unsigned long long)__double_as_longlong(mx));
+}
+
+__global__ void k_ns_flip(DevCtx c) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.B) return;
+  WalkerState& st = c.ws[w];
+  if (st.k > 0) st.n_cur ^= 1;
+  st.n_src = st.n_cur;
+  st.rebuilds += 1;
+  st.flops_rebuild += 2.0 * 4.0 * (double)st.k * st.k * st.k;   // two k^3 GEMMs per spin
+}
+
 }  // namespace ctaux

@@ -65,6 +65,8 @@ struct DevCtx {
   double* Bm;           // [B][2][ldm*cap]   candidate rows  g(c,j)(E_j-1), m x k col-major
   double* gxC;          // [B][ld*mmax]      g_ext[:, C], n x m col-major (spin independent)
   double* Gx;           // [B][2][ld*mmax]   N_ext * g_ext[:, C]
+  double* Tbuf;         // [B][2][ld*ld]  A*N of the Newton-Schulz refresh (rebuild_mode 1), else null
+  unsigned long long* resid;  // [B*2]  max |A N - 1| per matrix as the bit pattern of a non-negative double
   double* skbuf;        // [B][2][kMaxSplitK][skstride]  split-K partial products of the S2 GEMMs
   size_t skstride;      // max(ldm*cap, ld*mmax)
   double* Um;           // [B][2][ld*delay]  U = X[:, J]

@@ -79,7 +79,7 @@ def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
 
 
 def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, init_k=None, seeds=None,
-                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0):
+                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0, rebuild_mode=0):
     """reset + n_sweeps on both sides, compare logs, configurations, N, sign, counters."""
     from paper_1901_01047_b200 import Walkers
     table = table_for(cfg)
@@ -90,7 +90,7 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
                 delay=cfg["delay"] if delay is None else delay, n_walkers=n_walkers, init_k=init_k,
                 max_k=cfg["max_k"] if max_k is None else max_k,
                 rebuild_every=cfg["rebuild_every"] if rebuild_every is None else rebuild_every,
-                log_capacity=cap, cand_window=cand_window, fused_small=fused)
+                log_capacity=cap, cand_window=cand_window, fused_small=fused, rebuild_mode=rebuild_mode)
     W.reset(seeds)
     W.sweep(n_sweeps)
     orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k)
@@ -130,7 +130,8 @@ def load_thermalised(name, seed=0):
     return cfg, int(meta["next_id"]), int(meta["p"])
 
 
-def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay=None, tol=N_FROB_TOL, **kw):
+def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay=None, tol=N_FROB_TOL,
+                      rebuild_every=0, **kw):
     """Both sides start from the SAME given configuration (a thermalised, well-conditioned one), each
     walker with its own seed; no rebuild on the device, so N is the incrementally updated matrix after
     n_sweeps sweeps (or the oracle runs n_proposals single proposals and the device log is compared on
@@ -142,7 +143,7 @@ def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay
     cap = int(max(n_sweeps, 1) * max(cfg["max_k"], 16) + 64)
     W = Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table,
                 delay=cfg["delay"] if delay is None else delay, n_walkers=nw, init_k=0, max_k=cfg["max_k"],
-                rebuild_every=0, log_capacity=cap, **kw)
+                rebuild_every=rebuild_every, log_capacity=cap, **kw)
     W.set_state(seeds, [c0] * nw, [next_id] * nw, [p0] * nw)
 
     def one(seed):

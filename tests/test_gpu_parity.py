@@ -326,3 +326,30 @@ def test_walker_groups_run_the_same_chains(fused):
             assert np.array_equal(Ns[w][s], grp.get_N(w, s))
     grp.close()
     one.close()
+
+
+@pytest.mark.parametrize("fused", [1, -1])
+def test_newton_schulz_refresh_config2(fused):
+    """rebuild_mode 1: the periodic rebuild is one Newton-Schulz step N <- N (2 - A N) (two GEMMs) instead of the
+    LU.  Same chain; N right after a refresh within 1e-10 of the oracle's direct inverse."""
+    cfg = get_config(1)
+    W, orcs, worst = full_parity(cfg, 16, 20, T1, fused=fused, rebuild_mode=1, rebuild_every=5)
+    assert all(W.get_stats(w)["rebuilds"] == 4 for w in range(16))
+    full_parity(cfg, 4, 12, T0, fused=fused, rebuild_mode=1, rebuild_every=1)
+
+
+def test_newton_schulz_refresh_config3_and_large_k_kernels():
+    cfg = get_config(2)
+    full_parity(cfg, 8, 10, T1, rebuild_mode=1, rebuild_every=5, n_tol=1e-10)
+    big = dict(cfg, max_k=600)
+    full_parity(big, 2, 6, T1, rebuild_mode=1, rebuild_every=3)
+
+
+@pytest.mark.slow
+def test_newton_schulz_refresh_config4_thermalised():
+    """Config 4 at full size from the thermalised start: 2 sweeps with a refresh after each; the refreshed N
+    against the oracle's from-scratch inverse."""
+    cfg = get_config(3)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 2, T1,
+                                       rebuild_every=1, rebuild_mode=1)
+    assert all(W.get_stats(w)["rebuilds"] == 2 for w in range(2))
