@@ -34,6 +34,9 @@
 //   Q16 sweep = max(16, k at sweep start) proposals       (convention: parity unpinned)
 //   Q17 init_k Philox-drawn vertices accepted unconditionally (convention: parity unpinned)
 //   Q29 uniform integers by multiply-shift (w * range) >> 32 (convention: parity unpinned)
+//   NEXT-1 (off by default, orc_set_flips): auxiliary-spin flip as a third move, type = (w6*3)>>32, vertex at list
+//       position (w1*k)>>32, R = prod_sigma det A'/det A.  Pinned by the Fock-space trace ratio, T1 == T0, and the
+//       atomic-limit <k> with flips on; the word -> move mapping is a convention (parity unpinned).
 // Pins (tests/test_oracle_*.py): closed-form table values, Fock-space trace = det A,
 // one-vertex closed form, U->0 Poisson law, atomic-limit <k>, reversibility,
 // permutation / spin symmetry, Philox against cuRAND's host generator, T1 == T0.
@@ -186,6 +189,11 @@ struct Walker {
   uint64_t p = 0;
   int sign = 1;
   int mode = 0;  // 0 = T0, 1 = T1
+  int flips = 0; // 1: auxiliary-spin FLIP as a third move (Fig. 5 (c)->(d)); SURVEY NEXT-1.
+                 //    move type = (w6 * 3) >> 32: 0 insert, 1 remove, 2 flip, 1/3 each (w6 = reserved word wB[2]);
+                 //    flip: vertex at list position (w1 * k) >> 32, s -> -s, R = prod_sigma det A'/det A
+                 //    (symmetric proposal, no prefactor); k = 0: rejected.  0 (default): the two-move chain.
+  int64_t acc_flip = 0;
   std::vector<LogEntry> log;
   int64_t acc_ins = 0, acc_rem = 0;
   double min_margin = INFINITY;
@@ -292,7 +300,7 @@ struct Walker {
     refresh_det();
     sign = sd[0] * sd[1];
     log.clear();
-    acc_ins = acc_rem = 0;
+    acc_ins = acc_rem = 0; acc_flip = 0;
     min_margin = INFINITY;
   }
 
@@ -369,6 +377,29 @@ struct Walker {
     const int k = (int)L.size();
     return N[0][(size_t)j * k + j] * N[1][(size_t)j * k + j];
   }
+  // flip of vertex j changes column j of A only: A' = A + dE (e_j - g_{.j}) e_j^T, dE = E'_j - E_j, and
+  // N (e_j - g_{.j}) = (e_j - N_{.j}) / (E_j - 1)  (from N A = 1), so per spin
+  //   det A'/det A = 1 + dE (1 - N_jj)/(E_j - 1),   N' = N - (dE / ratio) x_j N_{j.},  x_j[i] = (delta_ij - N_ij)/(E_j - 1)
+  double ratio_flip_T1(int j, double r[2]) const {
+    const int k = (int)L.size();
+    for (int s = 0; s < 2; ++s) {
+      const double Eo = E(s, L[j].spin), En = E(s, -L[j].spin);
+      r[s] = 1.0 + (En - Eo) * (1.0 - N[s][(size_t)j * k + j]) / (Eo - 1.0);
+    }
+    return r[0] * r[1];
+  }
+  void apply_flip_T1(int j, const double r[2]) {
+    const int k = (int)L.size();
+    for (int s = 0; s < 2; ++s) {
+      const double Eo = E(s, L[j].spin), En = E(s, -L[j].spin);
+      const double f = (En - Eo) / r[s] / (Eo - 1.0);
+      std::vector<double>& Nm = N[s];
+      std::vector<double> x(k), row(k);
+      for (int i = 0; i < k; ++i) { x[i] = ((i == j) ? 1.0 : 0.0) - Nm[(size_t)i * k + j]; row[i] = Nm[(size_t)j * k + i]; }
+      for (int a = 0; a < k; ++a)
+        for (int b = 0; b < k; ++b) Nm[(size_t)a * k + b] -= f * x[a] * row[b];
+    }
+  }
   void apply_rem_T1(int j) {
     const int k = (int)L.size();  // size BEFORE the removal
     for (int s = 0; s < 2; ++s) {
@@ -401,7 +432,7 @@ struct Walker {
     LogEntry e;
     std::memset(&e, 0, sizeof(e));
     e.p = p;
-    e.type = (int32_t)(wA[0] & 1u);
+    e.type = flips ? (int32_t)(((uint64_t)wB[2] * 3u) >> 32) : (int32_t)(wA[0] & 1u);
     e.u = unif53(wB[0], wB[1]);
     double R = 0.0;
     if (mode == 1 && !N_valid) refresh_N();
@@ -425,6 +456,30 @@ struct Walker {
         L.push_back(v);
         det_valid = false;
         ++acc_ins;
+      }
+    } else if (e.type == 2) {
+      if (k == 0) {
+        e.arg = -1;
+        R = 0.0;
+        e.accepted = 0;
+      } else {
+        const int j = (int)(((uint64_t)wA[1] * (uint64_t)k) >> 32);
+        e.arg = j;
+        double r[2] = {1.0, 1.0};
+        if (mode == 0) {
+          std::vector<Vertex> Ln(L);
+          Ln[j].spin = -Ln[j].spin;
+          R = ratio_T0(Ln);
+        } else {
+          R = ratio_flip_T1(j, r);
+        }
+        e.accepted = (e.u < std::fabs(R)) ? 1 : 0;
+        if (e.accepted) {
+          if (mode == 1) apply_flip_T1(j, r);
+          L[j].spin = -L[j].spin;
+          det_valid = false;
+          ++acc_flip;
+        }
       }
     } else {
       if (k == 0) {
@@ -456,7 +511,7 @@ struct Walker {
     e.R = R;
     const double aR = std::fabs(R);
     const double margin = std::fabs(e.u - aR) / std::max(aR, 1e-300);
-    if (!(e.type == 1 && k == 0) && margin < min_margin) min_margin = margin;
+    if (!(e.type != 0 && k == 0) && margin < min_margin) min_margin = margin;
     log.push_back(e);
     ++p;
   }
@@ -495,6 +550,8 @@ void* orc_create(int Lx, int Ly, double beta, double U, double K, int M, const d
 }
 void orc_destroy(void* h) { delete (Walker*)h; }
 void orc_reset(void* h, int init_k) { ((Walker*)h)->reset(init_k); }
+void orc_set_flips(void* h, int on) { ((Walker*)h)->flips = on ? 1 : 0; }
+int64_t orc_acc_flip(void* h) { return ((Walker*)h)->acc_flip; }
 void orc_set_mode(void* h, int mode) { Walker* w = (Walker*)h; w->mode = mode; w->N_valid = false; w->det_valid = false; }
 
 // Start from a given configuration (list order), proposal counter and next id.
@@ -512,6 +569,7 @@ void orc_set_state(void* h, int k, const uint64_t* id, const int32_t* site, cons
   w->sign = w->sd[0] * w->sd[1];
   w->log.clear();
   w->acc_ins = w->acc_rem = 0;
+  w->acc_flip = 0;
   w->min_margin = INFINITY;
 }
 void orc_sweep(void* h, int n_sweeps) { ((Walker*)h)->sweep(n_sweeps); }

@@ -43,6 +43,9 @@ def lib():
         L.orc_destroy.argtypes = [vp]
         L.orc_reset.argtypes = [vp, i32]
         L.orc_set_mode.argtypes = [vp, i32]
+        L.orc_set_flips.argtypes = [vp, i32]
+        L.orc_acc_flip.restype = i64
+        L.orc_acc_flip.argtypes = [vp]
         L.orc_set_state.argtypes = [vp, i32, vp, vp, vp, vp, u64, u64]
         L.orc_sweep.argtypes = [vp, i32]
         L.orc_propose.argtypes = [vp, i64]
@@ -109,6 +112,12 @@ class OracleWalker:
 
     def set_mode(self, mode):
         lib().orc_set_mode(self._h, mode)
+
+    def set_flips(self, on=True):
+        """Enable the auxiliary-spin flip as a third move.  Default: off."""
+        lib().orc_set_flips(self._h, 1 if on else 0)
+
+    acc_flip = property(lambda s: lib().orc_acc_flip(s._h))
 
     def set_state(self, site, tau, spin, ids=None, next_id=None, p=0):
         site = np.ascontiguousarray(site, dtype=np.int32)

@@ -433,3 +433,98 @@ def test_sweep_length_and_counter_continuity():
     e.reset(0)
     e.sweep(1)
     assert e.p == 16
+
+
+# ----------------------------------------------------------------------------- NEXT-1: auxiliary-spin flips
+def test_flip_ratio_equals_ratio_of_fock_space_traces():
+    """A flip multiplies the weight by prod_sigma det A'_sigma / det A_sigma (Fig. 5 (c)->(d)).
+    The logged ratio of the oracle's first flip proposal, against the ratio of the two Fock-space traces of
+    Eq. (27) evaluated literally (independent of every matrix formula in the oracle)."""
+    Lx = Ly = 2
+    beta, U, K, M, mu = 2.0, 4.0, 1.0, 512, -0.3
+    T = g0_table(Lx, Ly, beta, mu, M)
+    rng = np.random.default_rng(7)
+    checked = 0
+    for seed in range(40):
+        nv = int(rng.integers(1, 5))
+        sites = rng.integers(0, 4, nv).astype(np.int32)
+        taus = rng.choice(np.arange(1, M), nv, replace=False) * beta / M
+        spins = rng.choice([-1, 1], nv).astype(np.int8)
+        for mode in (T0, T1):
+            w = OracleWalker(Lx, Ly, beta, U, K, T, seed, mode)
+            w.set_flips(True)
+            w.set_state(sites, taus, spins)
+            w.propose(1)
+            e = w.log()[0]
+            if e["type"] != 2:
+                continue
+            j = int(e["arg"])
+            gamma = math.log(w.exp_gamma)
+            flipped = spins.copy()
+            flipped[j] = -flipped[j]
+            want = 1.0
+            for sigma in (+1, -1):
+                num = _fock_trace(Lx, Ly, beta, mu, sites, taus, [-gamma * sigma * int(s) for s in flipped])
+                den = _fock_trace(Lx, Ly, beta, mu, sites, taus, [-gamma * sigma * int(s) for s in spins])
+                want *= num / den
+            assert abs(e["R"] / want - 1) < 1e-9, (seed, mode, e["R"], want)
+            assert e["accepted"] == (1 if e["u"] < abs(e["R"]) else 0)
+            checked += 1
+    assert checked >= 10
+
+
+@pytest.mark.parametrize("ci,sweeps", [(0, 60), (1, 6)])
+def test_flips_T1_equals_T0(ci, sweeps):
+    """With flips enabled the rank-1 oracle (column-change formula) reproduces brute force decision for decision."""
+    cfg = get_config(ci)
+    table = table_for(cfg)
+    out = []
+    for mode in (T0, T1):
+        w = OracleWalker.from_config(cfg, table, 11, mode)
+        w.set_flips(True)
+        w.reset(cfg["init_k"])
+        w.sweep(sweeps)
+        out.append((w.log(), w.config(), w.acc_flip, w.sign, w.N(0), w.N(1)))
+    a, b = out
+    assert a[2] == b[2] > 0 and a[3] == b[3]
+    for f in ("p", "type", "arg", "tau", "spin", "accepted", "u"):
+        assert a[0][f].tobytes() == b[0][f].tobytes(), f
+    assert set(np.unique(a[0]["type"])) == {0, 1, 2}
+    assert np.max(np.abs(a[0]["R"] - b[0]["R"]) / np.maximum(np.abs(a[0]["R"]), 1e-300)) < 1e-8
+    for f in a[1]:
+        assert a[1][f].tobytes() == b[1][f].tobytes()
+    # flipping twice is the identity on the weight: R_1 * R_2 = 1 (brute force, T0)
+    cfg1 = a[1]
+    w = OracleWalker.from_config(cfg, table, 0, T0)
+    w.set_state(cfg1["site"], cfg1["tau"], cfg1["spin"])
+    l0 = [w.logdet(s) for s in range(2)]
+    sp = cfg1["spin"].copy()
+    sp[0] = -sp[0]
+    w.set_state(cfg1["site"], cfg1["tau"], sp)
+    l1 = [w.logdet(s) for s in range(2)]
+    r12 = math.exp(sum(x[0] for x in l1) - sum(x[0] for x in l0))
+    r21 = math.exp(sum(x[0] for x in l0) - sum(x[0] for x in l1))
+    assert abs(r12 * r21 - 1) < 1e-12
+
+
+def test_flips_keep_the_stationary_distribution():
+    """Adding a valid move must not change the stationary law: atomic limit <k> (pin P6) with flips on, and the
+    auxiliary spins stay unpolarised on average."""
+    beta, U, K = 2.0, 4.0, 1.0
+    want = K + (beta * U / 2) / (1 + math.exp(-beta * U / 2))
+    T = atomic_limit_table(64)
+    means, acc = [], 0
+    for seed in range(8):
+        w = OracleWalker(1, 1, beta, U, K, T, seed, T1)
+        w.set_flips(True)
+        w.reset(5)
+        w.propose(150000)
+        log = w.log()
+        dk = log["accepted"] * np.where(log["type"] == 0, 1, np.where(log["type"] == 1, -1, 0))
+        k_before = 5 + np.concatenate([[0], np.cumsum(dk)[:-1]])
+        means.append(k_before[5000:].mean())
+        acc += w.acc_flip
+    means = np.array(means)
+    err = means.std(ddof=1) / math.sqrt(len(means))
+    assert acc > 1000
+    assert abs(means.mean() - want) < max(4 * err, 0.02), (means.mean(), err, want)
