@@ -207,7 +207,7 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------
 def total_stats(W, n_walkers):
     keys = ("proposals", "acc_ins", "acc_rem", "flops_cand", "flops_flush", "flops_usinv", "flops_rebuild",
-            "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds", "guard_ends")
+            "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds", "guard_ends", "acc_flip")
     tot = {k: 0.0 for k in keys}
     ks = []
     for w in range(n_walkers):
@@ -254,7 +254,7 @@ def run_gpu(args):
     fp64_dmma = probe_fp64(0) if rank == 0 else 0.0
     W = WalkerGroups(G, B, lambda g, nb, stream: Walkers.from_config(
         cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream,
-        rebuild_mode=args.rebuild_mode))
+        rebuild_mode=args.rebuild_mode, flip_moves=args.flips))
     W.reset(seeds)
     stream = torch.cuda.current_stream()
 
@@ -282,7 +282,7 @@ def run_gpu(args):
     s1 = total_stats(W, B)
     l1 = W.launch_count()
     d = diff(s1, s0)
-    acc = d["acc_ins"] + d["acc_rem"]
+    acc = d["acc_ins"] + d["acc_rem"] + d["acc_flip"]
     # ---- kernel pass: the same step once more, per-class CUDA events on the launching streams; with
     # several groups they run one after the other here, so that each kernel is timed alone
     W.timing_enable(True)
@@ -338,7 +338,8 @@ def run_gpu(args):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
                           "K": cfg["K"], "walkers_per_gpu": B, "stream_groups": G, "delay": delay, "sweeps_per_step": S,
-                          "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh", "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
+                          "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh",
+                          "moves": "insert/remove/flip" if args.flips else "insert/remove", "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
                           "working set fits L2 (latency-bound chain; no flush between steps)",
                           "parallelism": "replicas only"},
                "proposals_per_s": props_all / (ms_max * 1e-3), "k_mean": s1["k_mean"],
@@ -368,7 +369,7 @@ def run_e2e(W, cfg, B, S, steps, rank):
         W.sweep(S)
         cfgs, new_stats, Ns = W.fetch_all(with_N=True)
         for st in new_stats:
-            acc += st["acc_ins"] + st["acc_rem"]      # counters restart at set_state
+            acc += st["acc_ins"] + st["acc_rem"] + st["acc_flip"]      # counters restart at set_state
             d2h += st["k"] * (8 + 4 + 8 + 1) + 2 * st["k"] * st["k"] * 8
         del Ns
         stats = new_stats
@@ -392,6 +393,8 @@ def main():
     ap.add_argument("--groups", type=int, default=0, help="stream groups the walkers are split over (0 = per-config default)")
     ap.add_argument("--rebuild-mode", type=int, default=0, choices=[0, 1],
                     help="periodic rebuild: 0 = from-scratch LU (default, BASELINE.json), 1 = Newton-Schulz refresh (two GEMMs)")
+    ap.add_argument("--flips", type=int, default=0, choices=[0, 1],
+                    help="1: auxiliary-spin flip as a third move (SURVEY NEXT-1; a different chain than BASELINE.json's)")
     ap.add_argument("--cand-window", type=int, default=0, help="insertion candidates pre-expanded per block")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

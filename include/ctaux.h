@@ -91,6 +91,10 @@ typedef struct ctaux_params {
                               FP64 GEMMs instead of the latency-bound LU; quadratic, so an N that has drifted to
                               1e-9 comes back to rounding level.  Falls back to LU when max|A N - 1| > 1e-4.
                               Chain-neutral like every rebuild.  Needs one more k x k buffer per matrix.     */
+  int32_t flip_moves;      /* 1: auxiliary-spin FLIP as a third move (Fig. 5 (c)->(d)): move type =
+                              (w6 * 3) >> 32 (0 insert, 1 remove, 2 flip), flip of the vertex at list position
+                              (w1 * k) >> 32, R = prod_sigma det A'/det A.  0 (default): the two-move chain of
+                              BASELINE.json.  This DOES change the chain (it is a different sampler).          */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */
@@ -112,13 +116,14 @@ typedef struct ctaux_stats {
   double sum_k;            /* sum over proposals of k before the proposal (for <k>)                   */
   double flops_usinv;      /* S4: 2*k'*r*r (U * S^-1), both spins                                     */
   int64_t guard_ends;      /* blocks ended early by the numerical guard (ctaux_params.guard_amp)      */
+  int64_t acc_flip;        /* accepted auxiliary-spin flips since reset (flip_moves = 1)              */
 } ctaux_stats;
 
 /* One entry of the decision log (48 bytes). */
 typedef struct ctaux_log_entry {
   uint64_t p;              /* proposal counter                                                        */
-  int32_t type;            /* 0 insert, 1 remove                                                      */
-  int32_t arg;             /* insert: site; remove: list position j (-1 when k == 0)                  */
+  int32_t type;            /* 0 insert, 1 remove, 2 flip                                              */
+  int32_t arg;             /* insert: site; remove / flip: list position j (-1 when k == 0)           */
   double tau;              /* insert: proposed tau; remove: 0                                         */
   int32_t spin;            /* insert: proposed auxiliary spin; remove: 0                              */
   int32_t accepted;        /* 1 iff u < |R|                                                           */

@@ -26,7 +26,7 @@ class _Params(C.Structure):
                 ("delay", C.c_int32), ("n_walkers", C.c_int32), ("init_k", C.c_int32),
                 ("max_k", C.c_int32), ("rebuild_every", C.c_int32), ("log_capacity", C.c_int32),
                 ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
-                ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32)]
+                ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32), ("flip_moves", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -36,7 +36,7 @@ class _Stats(C.Structure):
                 ("k", C.c_int32), ("sign", C.c_int32), ("flops_cand", C.c_double),
                 ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
                 ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double),
-                ("guard_ends", C.c_int64)]
+                ("guard_ends", C.c_int64), ("acc_flip", C.c_int64)]
 
 
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
@@ -112,7 +112,7 @@ class Walkers:
 
     def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
                  rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None,
-                 guard_amp=0.0, fused_small=0, rebuild_mode=0):
+                 guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0):
         import torch
         if not torch.cuda.is_available():
             raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
@@ -132,6 +132,7 @@ class Walkers:
         p.guard_amp = guard_amp
         p.fused_small = fused_small
         p.rebuild_mode = rebuild_mode
+        p.flip_moves = flip_moves
         nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
         if nbytes == 0:
             raise CtauxError(-1, "ctaux_workspace_bytes", "invalid parameters")

@@ -289,6 +289,7 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   memset(&d, 0, sizeof(d));
   d.B = p->n_walkers; d.Lx = p->Lx; d.Ly = p->Ly; d.Nc = p->Lx * p->Ly; d.M = p->n_tau;
   d.max_k = p->max_k; d.delay = p->delay;
+  d.flips = p->flip_moves ? 1 : 0;
   // candidates pre-expanded per block: about delay / (2 * acceptance * 1/2) = delay at the ~50 % acceptance of the
   // paper-shaped workloads; kept a multiple of the 64-row GEMM tile for the large-delay configurations
   int mmax = p->cand_window > 0 ? p->cand_window : (p->delay >= 64 ? p->delay : p->delay + p->delay / 4 + 8);
@@ -1005,7 +1006,7 @@ int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   out->k = st.k; out->sign = st.sign;
   out->flops_cand = st.flops_cand; out->flops_flush = st.flops_flush; out->flops_rebuild = st.flops_rebuild;
   out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
-  out->guard_ends = st.guard_ends;
+  out->guard_ends = st.guard_ends; out->acc_flip = st.acc_flip;
   return CTAUX_OK;
 }
 

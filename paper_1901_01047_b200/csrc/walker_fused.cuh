@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
   int nfree = cap - k, hi = k;   // hi: slots in use are < hi
   uint64_t p = st.p, next_id = st.next_id;
   int sign = st.sign, status = 0, spill_sweeps = -1, spill_props = 0;
-  int64_t acc_ins = 0, acc_rem = 0, log_count = st.log_count;
+  int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, log_count = st.log_count;
   double min_margin = st.min_margin, sum_k = 0.0;
   int sweeps_done = 0;
   const double em1p = c.egm - 1.0, em1m = c.egp - 1.0;   // E - 1 for sigma*s = +1 / -1
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
       uint32_t wa[4], wb[4];
       philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 0u, 1u, st.key0, st.key1, wa);
       philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 1u, 1u, st.key0, st.key1, wb);
-      const int type = (int)(wa[0] & 1u);
+      const int type = c.flips ? (int)(((uint64_t)wb[2] * 3u) >> 32) : (int)(wa[0] & 1u);
       const double uu = unif53(wb[0], wb[1]);
       double R = 0.0;
       bool accept = false;
@@ -227,7 +227,45 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
           if (slot >= hi) hi = slot + 1;
           if (R < 0.0) sign = -sign;
         }
-      } else if (k > 0) {
+      } else if (type == 2 && k > 0) {
+        // ---------------------------------------------------------------- auxiliary-spin flip
+        // column j of A changes by dE = E(-s) - E(s):  det A'/det A = 1 + dE (1 - N_jj)/(E - 1),
+        // N' = N - (dE / ratio) x N_{j.},  x_a = (delta_aj - N_aj)/(E - 1)   (from N A = 1)
+        j = (int)(((uint64_t)wa[1] * (uint64_t)k) >> 32);
+        arg = j;
+        slot = live[j];
+        const int so = spin_s[slot];
+        const double eo0 = so > 0 ? em1p : em1m, en0 = so > 0 ? em1m : em1p;   // spin up: E(s) - 1, E(-s) - 1
+        const double eo1 = so > 0 ? em1m : em1p, en1 = so > 0 ? em1p : em1m;   // spin down
+        const double n0 = Nup[slot + slot * lds], n1 = Ndn[slot + slot * lds];
+        const double r0 = 1.0 + (en0 - eo0) * (1.0 - n0) / eo0;
+        const double r1 = 1.0 + (en1 - eo1) * (1.0 - n1) / eo1;
+        R = r0 * r1;
+        accept = uu < fabs(R);
+        if (accept) {
+          const double f = sp == 0 ? (en0 - eo0) / (r0 * eo0) : (en1 - eo1) / (r1 * eo1);
+          for (int a = lt; a < hi; a += kFusedGroup) {
+            uv[a] = ((a == slot) ? 1.0 : 0.0) - N[a + slot * lds];
+            wv[a] = N[slot + a * lds];
+          }
+          __syncthreads();
+          if (hi <= 64) {
+            const int a = lt & 63;
+            if (a < hi) {
+              const double ua = uv[a] * f;
+              for (int b = lt >> 6; b < hi; b += 2) N[a + b * lds] -= ua * wv[b];
+            }
+          } else {
+            for (int a = lt; a < hi; a += kFusedGroup) {
+              const double ua = uv[a] * f;
+              for (int b = 0; b < hi; ++b) N[a + b * lds] -= ua * wv[b];
+            }
+          }
+          if (tid == 0) spin_s[slot] = (signed char)(-so);
+          ++acc_flip;
+          if (R < 0.0) sign = -sign;
+        }
+      } else if (type == 1 && k > 0) {
         // ---------------------------------------------------------------- removal
         j = (int)(((uint64_t)wa[1] * (uint64_t)k) >> 32);
         arg = j;
@@ -275,7 +313,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         const double mg = fabs(uu - aR) / fmax(aR, 1e-300);
         if (mg < min_margin) min_margin = mg;
       }
-      sum_k += (double)(k - (accept ? (type == 0 ? 1 : -1) : 0));   // k before the proposal
+      sum_k += (double)(k - (accept ? (type == 0 ? 1 : (type == 1 ? -1 : 0)) : 0));   // k before the proposal
       ++p;
       __syncthreads();
       if (status) break;
@@ -301,7 +339,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
   if (tid == 0) {
     st.k = k; st.k_new = k; st.r = 0; st.m = 0; st.n_src = st.n_cur;
     st.next_id = next_id; st.p = p; st.sign = sign;
-    st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
+    st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.acc_flip += acc_flip; st.sweeps += sweeps_done;
     st.blocks += sweeps_done; st.log_count = log_count;
     st.min_margin = min_margin; st.sum_k += sum_k;
     st.sweeps_left = 0; st.props_left = 0; st.active = 0;

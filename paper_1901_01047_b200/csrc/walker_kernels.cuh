@@ -104,7 +104,8 @@ __global__ void __launch_bounds__(1024) k_prep_window(DevCtx c) {
     philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 0u, 1u, st.key0, st.key1, wa);
     philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 1u, 1u, st.key0, st.key1, wb);
   }
-  const int is_ins = (in && (wa[0] & 1u) == 0u) ? 1 : 0;
+  const uint32_t mtype = c.flips ? (uint32_t)(((uint64_t)wb[2] * 3u) >> 32) : (wa[0] & 1u);
+  const int is_ins = (in && mtype == 0u) ? 1 : 0;
   // inclusive scan of is_ins over the CTA
   s_scan[tid] = is_ins;
   if (tid == 0) s_win = c.winmax;
@@ -123,7 +124,7 @@ __global__ void __launch_bounds__(1024) k_prep_window(DevCtx c) {
   const int win = s_win;
   if (in && tid < win) {
     PropInfo pi;
-    pi.type_cand = (wa[0] & 1u) | ((uint32_t)(is_ins ? cand : 0) << 1);
+    pi.type_cand = mtype | ((uint32_t)(is_ins ? cand : 0) << 2);
     pi.w1 = wa[1];
     pi.u = unif53(wb[0], wb[1]);
     c.prop[(size_t)w * c.winmax + tid] = pi;
@@ -200,7 +201,7 @@ constexpr int kGroup = kPropThreads / 2;  // threads per spin
 
 struct ProposeSmem {
   // byte offsets into dynamic shared memory
-  int sinv, scol, srow, tv, tpv, red, snn, live0, live1, spin, J, jpos, prop, total;
+  int sinv, scol, srow, tv, tpv, red, snn, live0, live1, spin, J, jpos, prop, flip, total;
 };
 
 __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
@@ -220,6 +221,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.J = o; o += delay * 4;
   L.jpos = o; o += (winmax + 1) * 4;
   L.spin = o; o += (cap + 15) / 16 * 16;
+  L.flip = o; o += (cap + 15) / 16 * 16;
   L.total = o;
   return L;
 }
@@ -249,6 +251,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   int* Js = reinterpret_cast<int*>(smraw + L.J);
   int* jpos = reinterpret_cast<int*>(smraw + L.jpos);  // candidate index -> position in J (-1: not buffered)
   signed char* spin_s = reinterpret_cast<signed char*>(smraw + L.spin);
+  signed char* flipped = reinterpret_cast<signed char*>(smraw + L.flip);   // 1: block-start vertex flipped in this block
 
   const int k0 = st.k, m = st.m, win = st.win, n = k0 + m;
   const int cfg_old = st.cfg_cur;
@@ -259,7 +262,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
 
   for (int i = tid; i < n; i += kPropThreads) spin_s[i] = (signed char)c.cfg_spin[off_old + i];
-  for (int i = tid; i < k0; i += kPropThreads) live[i] = i;
+  for (int i = tid; i < k0; i += kPropThreads) { live[i] = i; flipped[i] = 0; }
   for (int i = tid; i < win; i += kPropThreads) prop[i] = c.prop[(size_t)w * c.winmax + i];
   for (int i = tid; i <= c.winmax; i += kPropThreads) jpos[i] = -1;
   __syncthreads();
@@ -277,7 +280,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   int props_left = st.props_left, sweeps_left = st.sweeps_left;
   uint64_t next_id = st.next_id, p = st.p;
   int sign = st.sign, status = 0, consumed = 0;
-  int64_t acc_ins = 0, acc_rem = 0, sweeps_done = 0;
+  int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, sweeps_done = 0;
   double min_margin = st.min_margin, sum_k = 0.0;
   int64_t log_count = st.log_count;
   bool finished = false;
@@ -291,16 +294,20 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       props_left = kcur > 16 ? kcur : 16;
     }
     const PropInfo pi = prop[i];
-    const int type = (int)(pi.type_cand & 1u);
+    const int type = (int)(pi.type_cand & 3u);
     int slot = -1, j = -1;
     double pref = 0.0;
     if (type == 0) {
-      slot = k0 + (int)(pi.type_cand >> 1);
+      slot = k0 + (int)(pi.type_cand >> 2);
       pref = c.K / (double)(kcur + 1);
     } else if (kcur > 0) {
       j = (int)(((uint64_t)pi.w1 * (uint64_t)kcur) >> 32);
       slot = live[j];
-      pref = (double)kcur / c.K;
+      pref = type == 1 ? (double)kcur / c.K : 1.0;
+      // A vertex already changed in this block (flipped, or inserted and now to be flipped) is not touched a
+      // second time inside the block: the block is flushed BEFORE this proposal, which then meets an untouched
+      // vertex (exact; the insert-then-remove pair keeps its own in-block treatment below).
+      if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
     double R = 0.0, stil_own = 1.0, amp = 1.0;
@@ -319,8 +326,9 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     } else if (slot >= 0) {
       const int s = spin_s[slot];
       const double E0 = c.E(0, s), E1 = c.E(1, s);
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (1.0 - E0);
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (1.0 - E1);
+      // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
       // thread roles inside a spin group of 128: half 0 builds s_col and t = S^-1 s_col (and the dot
       // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass
@@ -334,7 +342,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       if (lt == 0) {
         // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
         // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
-        if (slot < k0) snn[sp] = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
+        if (slot < k0 && type == 1) snn[sp] = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
         else snn[sp] = 1.0 / dE_own + X(slot, slot);
       }
       __syncthreads();
@@ -464,6 +472,9 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       if (type == 0) {
         if (tid == 0) { live[len] = slot; c.cfg_id[off_old + slot] = next_id; jpos[slot - k0] = r; }
         ++len; ++kcur; ++next_id; ++acc_ins;
+      } else if (type == 2) {
+        if (tid == 0) flipped[slot] = 1;     // the vertex stays in the list; its spin changes at write-back
+        ++acc_flip;
       } else {
         for (int idx = tid; idx < len - 1; idx += kPropThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
         int* t = live; live = live_alt; live_alt = t;
@@ -487,7 +498,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     rowmap[i] = sl;
     c.cfg_site[off_new + i] = c.cfg_site[off_old + sl];
     c.cfg_tau[off_new + i] = c.cfg_tau[off_old + sl];
-    c.cfg_spin[off_new + i] = c.cfg_spin[off_old + sl];
+    c.cfg_spin[off_new + i] = (sl < k0 && flipped[sl]) ? -c.cfg_spin[off_old + sl] : c.cfg_spin[off_old + sl];
     c.cfg_id[off_new + i] = c.cfg_id[off_old + sl];
   }
   if (sinv_smem) {
@@ -508,9 +519,9 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     if (r > 0) st.n_cur ^= 1;
     st.next_id = next_id; st.p = p; st.sign = sign;
     st.sweeps_left = sweeps_left; st.props_left = props_left;
-    st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
+    st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.acc_flip += acc_flip; st.sweeps += sweeps_done;
     st.blocks += 1;
-    st.guard_ends += guard_end;
+    st.guard_ends += guard_end != 0;
     if (r > 0) { st.flushes += 1; st.sum_rank += r; }
     st.log_count = log_count;
     st.min_margin = min_margin; st.sum_k += sum_k;

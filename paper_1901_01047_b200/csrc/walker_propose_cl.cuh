@@ -16,7 +16,7 @@ namespace ctaux {
 constexpr int kClThreads = 512;
 
 struct ProposeClSmem {
-  int sinv, scol, srow, tv, tpv, red, snn, xch, live0, live1, spin, J, jpos, prop, total;
+  int sinv, scol, srow, tv, tpv, red, snn, xch, live0, live1, spin, J, jpos, prop, flip, total;
 };
 __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
   ProposeClSmem L;
@@ -36,6 +36,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.J = o; o += delay * 4;
   L.jpos = o; o += (winmax + 1) * 4;
   L.spin = o; o += (cap + 15) / 16 * 16;
+  L.flip = o; o += (cap + 15) / 16 * 16;
   L.total = o;
   return L;
 }
@@ -66,6 +67,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   int* Js = reinterpret_cast<int*>(smcl + L.J);
   int* jpos = reinterpret_cast<int*>(smcl + L.jpos);
   signed char* spin_s = reinterpret_cast<signed char*>(smcl + L.spin);
+  signed char* flipped = reinterpret_cast<signed char*>(smcl + L.flip);   // 1: block-start vertex flipped in this block
 
   const int k0 = st.k, m = st.m, win = st.win, n = k0 + m;
   const int cfg_old = st.cfg_cur;
@@ -79,7 +81,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   int props_left = st.props_left, sweeps_left = st.sweeps_left;
   uint64_t next_id = st.next_id, p = st.p;
   int sign = st.sign, status = 0;
-  int64_t acc_ins = 0, acc_rem = 0, sweeps_done = 0;
+  int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, sweeps_done = 0;
   double min_margin = st.min_margin, sum_k = 0.0;
   int64_t log_count = st.log_count;
   const int n_cur0 = st.n_cur;
@@ -88,7 +90,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   double errlvl = 1.0;
 
   for (int i = tid; i < n; i += kClThreads) spin_s[i] = (signed char)c.cfg_spin[off_old + i];
-  for (int i = tid; i < k0; i += kClThreads) live[i] = i;
+  for (int i = tid; i < k0; i += kClThreads) { live[i] = i; flipped[i] = 0; }
   for (int i = tid; i < win; i += kClThreads) prop[i] = c.prop[(size_t)w * c.winmax + i];
   for (int i = tid; i <= c.winmax; i += kClThreads) jpos[i] = -1;
   cluster.sync();
@@ -127,16 +129,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       props_left = kcur > 16 ? kcur : 16;
     }
     const PropInfo pi = prop[i];
-    const int type = (int)(pi.type_cand & 1u);
+    const int type = (int)(pi.type_cand & 3u);
     int slot = -1, j = -1;
     double pref = 0.0;
     if (type == 0) {
-      slot = k0 + (int)(pi.type_cand >> 1);
+      slot = k0 + (int)(pi.type_cand >> 2);
       pref = c.K / (double)(kcur + 1);
     } else if (kcur > 0) {
       j = (int)(((uint64_t)pi.w1 * (uint64_t)kcur) >> 32);
       slot = live[j];
-      pref = (double)kcur / c.K;
+      pref = type == 1 ? (double)kcur / c.K : 1.0;
+      // A vertex already changed in this block (flipped, or inserted and now to be flipped) is not touched a
+      // second time inside the block: the block is flushed BEFORE this proposal, which then meets an untouched
+      // vertex (exact; the insert-then-remove pair keeps its own in-block treatment below).
+      if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
     double R = 0.0, stil_own = 1.0, amp = 1.0;
@@ -155,8 +161,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
     } else if (slot >= 0) {
       const int s = spin_s[slot];
       const double E0 = c.E(0, s), E1 = c.E(1, s);
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (1.0 - E0);
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (1.0 - E1);
+      // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
       for (int a = rl; a < r; a += 256) {
         const int ja = Js[a];
@@ -165,7 +172,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       }
       double* snn = snn2 + (i & 1);
       if (tid == 0) {
-        if (slot < k0) *snn = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
+        if (slot < k0 && type == 1) *snn = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
         else *snn = 1.0 / dE_own + X(slot, slot);
       }
       __syncthreads();
@@ -283,6 +290,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
           if (sp == 0) c.cfg_id[off_old + slot] = next_id;
         }
         ++len; ++kcur; ++next_id; ++acc_ins;
+      } else if (type == 2) {
+        if (tid == 0) flipped[slot] = 1;     // the vertex stays in the list; its spin changes at write-back
+        ++acc_flip;
       } else {
         for (int idx = tid; idx < len - 1; idx += kClThreads) live_alt[idx] = live[idx + (idx >= j ? 1 : 0)];
         int* t = live; live = live_alt; live_alt = t;
@@ -313,7 +323,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       rowmap[i] = sl;
       c.cfg_site[off_new + i] = c.cfg_site[off_old + sl];
       c.cfg_tau[off_new + i] = c.cfg_tau[off_old + sl];
-      c.cfg_spin[off_new + i] = c.cfg_spin[off_old + sl];
+      c.cfg_spin[off_new + i] = (sl < k0 && flipped[sl]) ? -c.cfg_spin[off_old + sl] : c.cfg_spin[off_old + sl];
       c.cfg_id[off_new + i] = c.cfg_id[off_old + sl];
     }
     for (int a = tid; a < r; a += kClThreads) c.J[(size_t)w * c.delay + a] = Js[a];
@@ -327,9 +337,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       st.n_cur = r > 0 ? (n_cur0 ^ 1) : n_cur0;
       st.next_id = next_id; st.p = p; st.sign = sign;
       st.sweeps_left = sweeps_left; st.props_left = props_left;
-      st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.sweeps += sweeps_done;
+      st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.acc_flip += acc_flip; st.sweeps += sweeps_done;
       st.blocks += 1;
-      st.guard_ends += guard_end;
+      st.guard_ends += guard_end != 0;
       if (r > 0) { st.flushes += 1; st.sum_rank += r; }
       st.log_count = log_count;
       st.min_margin = min_margin; st.sum_k += sum_k;

@@ -18,7 +18,7 @@ struct LogEntry {  // == ctaux_log_entry
 };
 
 struct PropInfo {  // one pre-expanded proposal of the current window (16 bytes)
-  uint32_t type_cand;  // bit0: type (0 insert, 1 remove); bits 1..: candidate index (inserts)
+  uint32_t type_cand;  // bits 0-1: type (0 insert, 1 remove, 2 flip); bits 2..: candidate index (inserts)
   uint32_t w1;         // word used for the removal index
   double u;            // uniform for the Metropolis test
 };
@@ -41,13 +41,14 @@ struct WalkerState {
   int32_t active;  // 1 while the walker still has proposals to do in this sweep call
   int32_t pad0;
   // statistics
-  int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count, guard_ends;
+  int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count, guard_ends, acc_flip;
   double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k, flops_usinv;
 };
 
 // Everything a kernel needs: passed by value (fits the 4 KB parameter space easily).
 struct DevCtx {
   int B, Lx, Ly, Nc, M;
+  int flips;   // 1: spin flip as a third move (ctaux_params.flip_moves)
   int max_k, mmax, winmax, delay;
   int cap;   // max_k + mmax : extended slots
   int ld;    // leading dimension of every N / Gx / U buffer (cap rounded up to 8)

@@ -24,11 +24,13 @@ R_ATOL = 1e-8
 N_FROB_TOL = 1e-10     # BASELINE.json north_star: relative Frobenius error of N
 
 
-def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None):
+def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None, flips=0):
     init_k = cfg["init_k"] if init_k is None else init_k
 
     def one(seed):
         w = OracleWalker.from_config(cfg, table, int(seed), mode)
+        if flips:
+            w.set_flips(True)
         w.reset(init_k)
         w.sweep(n_sweeps)
         return w
@@ -79,7 +81,7 @@ def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
 
 
 def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, init_k=None, seeds=None,
-                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0, rebuild_mode=0):
+                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0, rebuild_mode=0, flips=0):
     """reset + n_sweeps on both sides, compare logs, configurations, N, sign, counters."""
     from paper_1901_01047_b200 import Walkers
     table = table_for(cfg)
@@ -90,10 +92,10 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
                 delay=cfg["delay"] if delay is None else delay, n_walkers=n_walkers, init_k=init_k,
                 max_k=cfg["max_k"] if max_k is None else max_k,
                 rebuild_every=cfg["rebuild_every"] if rebuild_every is None else rebuild_every,
-                log_capacity=cap, cand_window=cand_window, fused_small=fused, rebuild_mode=rebuild_mode)
+                log_capacity=cap, cand_window=cand_window, fused_small=fused, rebuild_mode=rebuild_mode, flip_moves=flips)
     W.reset(seeds)
     W.sweep(n_sweeps)
-    orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k)
+    orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k, flips=flips)
     worst = 0.0
     for w, o in enumerate(orcs):
         what = f"{cfg['name']} walker {w}"
@@ -105,6 +107,7 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
         assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id, what
         assert st["sign"] == o.sign and st["acc_ins"] == o.acc_ins and st["acc_rem"] == o.acc_rem, what
         assert st["sweeps"] == n_sweeps, what
+        assert st["acc_flip"] == o.acc_flip, what
         if check_N:
             errs = compare_N(W, w, o, what, tol=n_tol)
             worst = max([worst] + errs)
@@ -131,7 +134,7 @@ def load_thermalised(name, seed=0):
 
 
 def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay=None, tol=N_FROB_TOL,
-                      rebuild_every=0, **kw):
+                      rebuild_every=0, flips=0, **kw):
     """Both sides start from the SAME given configuration (a thermalised, well-conditioned one), each
     walker with its own seed; no rebuild on the device, so N is the incrementally updated matrix after
     n_sweeps sweeps (or the oracle runs n_proposals single proposals and the device log is compared on
@@ -143,11 +146,13 @@ def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay
     cap = int(max(n_sweeps, 1) * max(cfg["max_k"], 16) + 64)
     W = Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table,
                 delay=cfg["delay"] if delay is None else delay, n_walkers=nw, init_k=0, max_k=cfg["max_k"],
-                rebuild_every=rebuild_every, log_capacity=cap, **kw)
+                rebuild_every=rebuild_every, log_capacity=cap, flip_moves=flips, **kw)
     W.set_state(seeds, [c0] * nw, [next_id] * nw, [p0] * nw)
 
     def one(seed):
         o = OracleWalker.from_config(cfg, table, int(seed), mode)
+        if flips:
+            o.set_flips(True)
         o.set_state(c0["site"], c0["tau"], c0["spin"], c0["id"], next_id, p0)
         if n_proposals is None:
             o.sweep(n_sweeps)

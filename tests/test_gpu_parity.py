@@ -353,3 +353,35 @@ def test_newton_schulz_refresh_config4_thermalised():
     W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 2, T1,
                                        rebuild_every=1, rebuild_mode=1)
     assert all(W.get_stats(w)["rebuilds"] == 2 for w in range(2))
+
+
+# ---------------------------------------------------------------- NEXT-1: auxiliary-spin flips (flip_moves = 1)
+@pytest.mark.parametrize("fused", [1, -1])
+def test_flips_config1_and_2(fused):
+    """Three-move chain (insert / remove / flip) against the oracle: brute force on config 1 and a config-2
+    prefix, rank-1 oracle on 64 walkers; logs, configurations (spins!), counters bit-exact, N within 1e-10."""
+    cfg = get_config(0)
+    W, orcs, worst = full_parity(cfg, 1, 300, T0, fused=fused, flips=1)
+    assert W.get_stats(0)["acc_flip"] > 50
+    cfg = get_config(1)
+    full_parity(cfg, 8, 12, T0, fused=fused, flips=1)
+    full_parity(cfg, 64, 40, T1, fused=fused, flips=1)
+
+
+@pytest.mark.parametrize("delay", [1, 16, 64, 128])
+def test_flips_chain_independent_of_delay(delay):
+    cfg = get_config(1)
+    full_parity(cfg, 4, 10, T1, delay=delay, rebuild_every=0, fused=-1, flips=1)
+
+
+def test_flips_config3_thermalised():
+    cfg = get_config(2)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(8), 6, T1, flips=1)
+    assert sum(W.get_stats(w)["acc_flip"] for w in range(8)) > 100
+
+
+@pytest.mark.slow
+def test_flips_config4_thermalised():
+    cfg = get_config(3)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1, flips=1)
+    assert sum(W.get_stats(w)["acc_flip"] for w in range(2)) > 50
