@@ -40,7 +40,7 @@ FALLBACK_BF16_TFLOPS = 1590.0
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the flush kernel from the committed
 # `ncu --set full` capture of the same launch configuration (profiles/), bytes; None = not captured
-FLUSH_TRAFFIC_PER_WALKER = {"cfg4_6x6_b20": 98.1e6}   # profiles/r1_v3_flush_full.md: 785 MB / 8 walkers
+FLUSH_TRAFFIC_PER_WALKER = {"cfg4_6x6_b20": 97.4e6}   # profiles/r1_v3_flush_full.md (update): 779 MB / 8 walkers
 
 
 def measured_peaks():
@@ -305,7 +305,7 @@ def run_gpu(args):
         fl = tim["flush_gemm"]
         flush_tf = dk["flops_flush"] / (fl["ms"] * 1e-3) / 1e12 if fl["ms"] > 0 else 0.0
         per_launch_flops = dk["flops_flush"] / max(fl["launches"], 1)
-        roofline = {"kernel": "gemm_grouped_kernel<DescFlush> (S4 rank-r flush, DMMA m8n8k4; 64x64 tiles at 5 CTAs/SM "
+        roofline = {"kernel": "gemm_flush_kernel<64,64,2,2,2,5,DescFlush> (S4 rank-r flush, DMMA m8n8k4; 64x64 tiles at 5 CTAs/SM "
                               "for k > 512, 8-warp 64x64 tiles below)", "bound": "tensor",
                     "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak if fp64_peak else None,
                     "traffic": (FLUSH_TRAFFIC_PER_WALKER[cfg["name"]] * (B // G) if cfg["name"] in FLUSH_TRAFFIC_PER_WALKER and
