@@ -257,6 +257,7 @@ struct ctaux_ctx {
   cudaEvent_t ev_fork, ev_join;
   bool lu_cluster;    // S5 panel factorisation on an 8-CTA cluster per matrix (large k)
   int lu_cluster_smem;
+  int lu_nb;          // panel width: 64 with the cluster panel when its slabs fit shared memory, else 32
   int cluster_mode;   // 0: k_propose (one CTA per walker); 1 / 2: k_propose_cl (2-CTA cluster per walker) with
                       // S^-1 in shared memory / in L2 -- used when S^-1 of both spins does not fit one CTA
   int cluster_smem;
@@ -463,31 +464,40 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
       tick(x, C_REBUILD); tick(x, C_REBUILD);
     }
     const int cb = grid_for((size_t)2 * kmax, 128, 64);
+    const int nbw = x->lu_nb;
     auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
-      if (x->persist) return launch_persist<0>(DescLU{d, j0, which}, P, s);
-      if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
-      return launch_gemm<GEMM_Q4>(DescLU{d, j0, which}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
+      if (x->persist) return launch_persist<0>(DescLU{d, j0, which, nbw}, P, s);
+      if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
+      return launch_gemm<GEMM_Q4>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
     };
-    for (int j0 = 0; j0 < kmax; j0 += kLuNb) {  // factorisation + forward substitution
+    for (int j0 = 0; j0 < kmax; j0 += nbw) {  // factorisation + forward substitution
       Scoped t(x, C_REBUILD);
-      const int j1 = j0 + kLuNb < kmax ? j0 + kLuNb : kmax;
+      const int j1 = j0 + nbw < kmax ? j0 + nbw : kmax;
+      int* dsg = set_sign ? x->detsign : nullptr;
       if (x->lu_cluster) {
         const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
-        k_lu_panel_cl<<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, set_sign ? x->detsign : nullptr, rl_cap);
+        if (nbw == 64) k_lu_panel_cl<64><<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, dsg, rl_cap);
+        else k_lu_panel_cl<32><<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, dsg, rl_cap);
       } else {
-        k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, set_sign ? x->detsign : nullptr);
+        k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, dsg);
       }
-      k_lu_swap<<<dim3(cb, P), 128, 0, s>>>(d, j0);
-      k_lu_trsm<<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
+      if (nbw == 64) {
+        k_lu_swap<64><<<dim3(cb, P), 128, 0, s>>>(d, j0);
+        k_lu_trsm<64><<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
+      } else {
+        k_lu_swap<32><<<dim3(cb, P), 128, 0, s>>>(d, j0);
+        k_lu_trsm<32><<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
+      }
       tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
       CU_CHECK(trailing(j0, 0, kmax - j1, kmax - j1));
       CU_CHECK(trailing(j0, 1, kmax - j1, kmax));
     }
-    for (int j0 = (kmax - 1) / kLuNb * kLuNb; j0 >= 0; j0 -= kLuNb) {  // backward substitution
+    for (int j0 = (kmax - 1) / nbw * nbw; j0 >= 0; j0 -= nbw) {  // backward substitution
       Scoped t(x, C_REBUILD);
-      k_lu_trsm<<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
+      if (nbw == 64) k_lu_trsm<64><<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
+      else k_lu_trsm<32><<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
       tick(x, C_REBUILD);
       CU_CHECK(trailing(j0, 2, j0, kmax));
     }
@@ -778,17 +788,17 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       }
     }
   }
-  x->lu_cluster = false; x->lu_cluster_smem = 0;
+  x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
   if (d.max_k > 512) {
     const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
-    const int need = (rl_cap * kLuPad + 2 * kLuNb + kLuCl) * 8 + kLuCl * 4 + 64;
-    if (need <= max_smem) {
-      if (cudaFuncSetAttribute(k_lu_panel_cl, cudaFuncAttributeMaxDynamicSharedMemorySize, need) == cudaSuccess) {
-        x->lu_cluster = true; x->lu_cluster_smem = need;
-      } else {
-        cudaGetLastError();
-      }
+    // panel width 32: width 64 (k_lu_panel_cl<64>, k_lu_trsm<64>) was measured at the same total time -- the rank-64
+    // trailing updates save 17 %, the wider panel and triangular solves cost it again (profiles/r1_v4_kernels_full.md)
+    const int need32 = lu_cl_smem_doubles(rl_cap, 32) * 8 + 64;
+    if (need32 <= max_smem &&
+        cudaFuncSetAttribute(k_lu_panel_cl<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, need32) == cudaSuccess) {
+      x->lu_cluster = true; x->lu_cluster_smem = need32; x->lu_nb = 32;
     }
+    cudaGetLastError();
   }
   x->cluster_mode = 0; x->cluster_smem = 0;
   if (!x->sinv_smem) {   // (measured: for delay <= 64 the cluster form is 20-25 % slower than one CTA per walker)

@@ -116,10 +116,15 @@ __global__ void __launch_bounds__(1024) k_lu_panel(DevCtx c, int j0, int* detsig
 // local elimination.  Same pivot choice as k_lu_panel (largest magnitude, smallest row index on ties).
 constexpr int kLuCl = 8;
 constexpr int kLuClThreads = 512;
-constexpr int kLuPad = kLuNb + 1;
+// dynamic shared memory of k_lu_panel_cl<NB>, in doubles
+__host__ __device__ inline int lu_cl_smem_doubles(int rl_cap, int nbw) {
+  return rl_cap * (nbw + 1) + 2 * kLuCl * (nbw + 2) + 2 * nbw;
+}
 
+template <int NB>   // panel width: 64 when the slabs fit shared memory (config 4), else 32
 __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     k_lu_panel_cl(DevCtx c, int j0, int* detsign, int rl_cap) {
+  constexpr int kLuNb = NB, kLuPad = NB + 1, kLuMsg = NB + 2;   // (shadow the file-level panel width)
   namespace cg = cooperative_groups;
   cg::cluster_group cluster = cg::this_cluster();
   extern __shared__ __align__(16) double lsm[];
@@ -137,13 +142,12 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
   const int R = (rows + kLuCl - 1) / kLuCl;  // rows per CTA (<= rl_cap)
   const int r0 = j0 + rank * R;              // first global row of this slab
   int nloc = k - r0; if (nloc > R) nloc = R; if (nloc < 0) nloc = 0;
-  double* A = lsm;                           // [rl_cap][kLuPad] row-major: A[i*kLuPad + cc]
-  double* prow = lsm + (size_t)rl_cap * kLuPad;         // [kLuNb] pivot row of the current column
-  double* swp = prow + kLuNb;                          // [kLuNb] row `col` travelling to the pivot's slot
-  double* cval = swp + kLuNb;                          // [kLuCl] candidates
-  int* cidx = reinterpret_cast<int*>(cval + kLuCl);    // [kLuCl]
+  double* A = lsm;                                       // [rl_cap][kLuPad] row-major: A[i*kLuPad + cc]
+  double* msg = lsm + (size_t)rl_cap * kLuPad;           // [2 parities][kLuCl senders][kLuMsg]
+  double* rowc = msg + 2 * kLuCl * kLuMsg;               // [2 parities][kLuNb]  row `col` (from its owner)
   __shared__ double s_val[kLuClThreads / 32];
   __shared__ int s_idx[kLuClThreads / 32];
+  __shared__ int s_best;
 
   for (int idx = tid; idx < nloc * nb; idx += kLuClThreads) {
     const int i = idx % nloc, cc = idx / nloc;
@@ -152,7 +156,7 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
   cluster.sync();
 
   for (int cc = 0; cc < nb; ++cc) {
-    const int col = j0 + cc;
+    const int col = j0 + cc, par = cc & 1;
     // 1. local pivot candidate over the local rows with global index >= col
     double best = -1.0;
     int bi = 0x7fffffff;
@@ -171,48 +175,66 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     }
     if ((tid & 31) == 0) { s_val[tid >> 5] = best; s_idx[tid >> 5] = bi; }
     __syncthreads();
-    if (tid < kLuCl) {   // thread q publishes this CTA's candidate to CTA q
+    if (tid == 0) {
       double b = s_val[0];
       int ix = s_idx[0];
       for (int q = 1; q < kLuClThreads / 32; ++q)
         if (s_val[q] > b || (s_val[q] == b && s_idx[q] < ix)) { b = s_val[q]; ix = s_idx[q]; }
-      double* rv = cluster.map_shared_rank(cval, tid);
-      int* ri = cluster.map_shared_rank(cidx, tid);
-      rv[rank] = b; ri[rank] = ix;
+      s_val[0] = b; s_best = ix;
+    }
+    __syncthreads();
+    // 2. ONE message per CTA to every CTA: candidate magnitude, row index and the candidate row itself; the owner
+    //    of row `col` also sends that row (it travels to the pivot's slot).  One cluster barrier per column.
+    {
+      const double b = s_val[0];
+      const int ix = s_best;
+      const bool have = ix != 0x7fffffff;
+      for (int t = tid; t < kLuCl * kLuMsg; t += kLuClThreads) {
+        const int q = t / kLuMsg, x = t % kLuMsg;
+        double* dst = cluster.map_shared_rank(msg, q) + ((size_t)par * kLuCl + rank) * kLuMsg;
+        double v;
+        if (x == 0) v = b;
+        else if (x == 1) v = (double)ix;
+        else v = (have && x - 2 < nb) ? A[(ix - r0) * kLuPad + (x - 2)] : 0.0;
+        dst[x] = v;
+      }
+      const int qc = (col - j0) / R;
+      if (rank == qc) {
+        for (int t = tid; t < kLuCl * kLuNb; t += kLuClThreads) {
+          const int q = t / kLuNb, x = t % kLuNb;
+          double* dst = cluster.map_shared_rank(rowc, q) + (size_t)par * kLuNb;
+          dst[x] = x < nb ? A[(col - r0) * kLuPad + x] : 0.0;
+        }
+      }
     }
     cluster.sync();
-    // 2. global pivot
-    double pb = cval[0];
-    int pr = cidx[0];
+    // 3. everybody picks the same winner
+    const double* mp = msg + (size_t)par * kLuCl * kLuMsg;
+    int qw = 0;
+    double pb = mp[0];
+    int pr = (int)mp[1];
 #pragma unroll
-    for (int q = 1; q < kLuCl; ++q)
-      if (cval[q] > pb || (cval[q] == pb && cidx[q] < pr)) { pb = cval[q]; pr = cidx[q]; }
-    const int qp = (pr - j0) / R, qc = (col - j0) / R;   // owners of the pivot row and of row `col`
+    for (int q = 1; q < kLuCl; ++q) {
+      const double v = mp[q * kLuMsg];
+      const int ix = (int)mp[q * kLuMsg + 1];
+      if (v > pb || (v == pb && ix < pr)) { pb = v; pr = ix; qw = q; }
+    }
+    const double* prow = mp + qw * kLuMsg + 2;      // pivot row (old contents of row pr)
+    const double* crow = rowc + (size_t)par * kLuNb; // old contents of row col
+    const int qp = (pr - j0) / R, qc = (col - j0) / R;
     if (rank == 0 && tid == 0) {
       ipiv[col] = pr;
       if (!(pb > 0.0)) st.status = -4;  // CTAUX_ESINGULAR
+      if (detsign) {
+        int sg = detsign[w * 2 + sp];
+        if (pr != col) sg = -sg;
+        if (prow[cc] < 0.0) sg = -sg;
+        detsign[w * 2 + sp] = sg;
+      }
     }
-    // 3. pivot row to everybody; row `col` to the pivot's owner
-    if (rank == qp && tid < kLuCl * kLuNb) {
-      const int q = tid / kLuNb, x = tid % kLuNb;
-      double* rp = cluster.map_shared_rank(prow, q);
-      rp[x] = x < nb ? A[(pr - r0) * kLuPad + x] : 0.0;
-    }
-    if (rank == qc && pr != col && tid >= kLuCl * kLuNb && tid < kLuCl * kLuNb + kLuNb) {
-      const int x = tid - kLuCl * kLuNb;
-      double* rs = cluster.map_shared_rank(swp, qp);
-      rs[x] = x < nb ? A[(col - r0) * kLuPad + x] : 0.0;
-    }
-    cluster.sync();
     if (pr != col) {
-      if (rank == qp && tid < nb) A[(pr - r0) * kLuPad + tid] = swp[tid];
-      if (rank == qc && tid < nb) A[(col - r0) * kLuPad + tid] = prow[tid];
-    }
-    if (rank == 0 && tid == 0 && detsign) {
-      int sg = detsign[w * 2 + sp];
-      if (pr != col) sg = -sg;
-      if (prow[cc] < 0.0) sg = -sg;
-      detsign[w * 2 + sp] = sg;
+      if (rank == qp && tid < nb) A[(pr - r0) * kLuPad + tid] = crow[tid];
+      if (rank == qc && tid >= 64 && tid < 64 + nb) A[(col - r0) * kLuPad + tid - 64] = prow[tid - 64];
     }
     __syncthreads();
     // 4. elimination of the local rows below `col`
@@ -229,6 +251,7 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     }
     __syncthreads();
   }
+  cluster.sync();   // nobody leaves while a peer may still write into its shared memory
   for (int idx = tid; idx < nloc * nb; idx += kLuClThreads) {
     const int i = idx % nloc, cc = idx / nloc;
     F[(size_t)(j0 + cc) * ld + r0 + i] = A[i * kLuPad + cc];
@@ -236,7 +259,9 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
 }
 
 // one thread per column: apply the panel's interchanges to F (outside the panel) and to X (all columns)
+template <int NB>
 __global__ void k_lu_swap(DevCtx c, int j0) {
+  constexpr int kLuNb = NB;
   const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
   const WalkerState& st = c.ws[w];
   const int k = st.k;
@@ -270,7 +295,9 @@ __global__ void k_lu_swap(DevCtx c, int j0) {
 // Triangular solves with the kLuNb x kLuNb diagonal block, one thread per right-hand-side column.
 //   upper == 0: rows j0..j1 of F (columns >= j1) and of X (all columns)  <-  L11^-1 (unit lower)
 //   upper == 1: rows j0..j1 of X (all columns)                           <-  U11^-1
+template <int NB>
 __global__ void __launch_bounds__(128) k_lu_trsm(DevCtx c, int j0, int upper) {
+  constexpr int kLuNb = NB;
   const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
   const WalkerState& st = c.ws[w];
   const int k = st.k;
@@ -326,12 +353,13 @@ struct DescLU {
   DevCtx c;
   int j0;
   int which;  // 0: F trailing, 1: X forward (rows below the panel), 2: X backward (rows above)
+  int nb;     // panel width
   __device__ bool operator()(int prob, GemmDesc& d) const {
     const int w = prob >> 1, sp = prob & 1;
     const WalkerState& st = c.ws[w];
     const int k = st.k;
     if (j0 >= k) return false;
-    const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+    const int j1 = (j0 + nb < k) ? j0 + nb : k;
     const size_t ld = c.ld;
     double* F = c.N(w, sp, st.n_cur ^ 1);
     double* X = c.N(w, sp, st.n_cur);
