@@ -385,3 +385,25 @@ def test_flips_config4_thermalised():
     cfg = get_config(3)
     W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1, flips=1)
     assert sum(W.get_stats(w)["acc_flip"] for w in range(2)) > 50
+
+
+def test_numerical_guard_is_chain_neutral():
+    """guard_amp only moves block boundaries: off, default and an aggressive setting give the same decisions;
+    the aggressive one ends many more blocks early."""
+    pkg = _pkg()
+    cfg = get_config(1)
+    table = table_for(cfg)
+    seeds = walker_seeds(6, first=200)
+    logs, ends = [], []
+    for ga in (-1.0, 0.0, 5.0):
+        W = pkg.Walkers.from_config(cfg, table, n_walkers=6, fused_small=-1, rebuild_every=0, log_capacity=3000, guard_amp=ga)
+        W.reset(seeds)
+        W.sweep(12)
+        logs.append([W.get_log(w) for w in range(6)])
+        ends.append(sum(W.get_stats(w)["guard_ends"] for w in range(6)))
+        W.close()
+    for w in range(6):
+        for other in (1, 2):
+            for f in ("p", "type", "arg", "tau", "spin", "accepted", "u"):
+                assert logs[0][w][f].tobytes() == logs[other][w][f].tobytes(), (w, other, f)
+    assert ends[0] == 0 and ends[2] > ends[1] >= 0 and ends[2] > 20
