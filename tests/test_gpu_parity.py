@@ -407,3 +407,26 @@ def test_numerical_guard_is_chain_neutral():
             for f in ("p", "type", "arg", "tau", "spin", "accepted", "u"):
                 assert logs[0][w][f].tobytes() == logs[other][w][f].tobytes(), (w, other, f)
     assert ends[0] == 0 and ends[2] > ends[1] >= 0 and ends[2] > 20
+
+
+@pytest.mark.parametrize("flips", [0, 1])
+def test_P6_atomic_limit_mean_order_on_the_device(flips):
+    """Pin P6 evaluated on the DEVICE chain itself (no oracle log involved): Nc = 1, xi = 0,
+    <k> = K + (beta U/2)/(1 + e^{-beta U/2}) = 4.92806, from sum_k / proposals over 128 chains."""
+    import math
+    from ctaux_workloads import atomic_limit_table
+    pkg = _pkg()
+    beta, U, K = 2.0, 4.0, 1.0
+    want = K + (beta * U / 2) / (1 + math.exp(-beta * U / 2))
+    nw = 128
+    W = pkg.Walkers(1, 1, beta, U, K, atomic_limit_table(64), delay=8, n_walkers=nw, init_k=5, max_k=64,
+                    rebuild_every=50, flip_moves=flips)
+    W.reset(walker_seeds(nw, first=1000))
+    W.sweep(300)                                   # thermalise
+    a = [W.get_stats(w) for w in range(nw)]
+    W.sweep(3000)
+    b = [W.get_stats(w) for w in range(nw)]
+    means = np.array([(y["sum_k"] - x["sum_k"]) / (y["proposals"] - x["proposals"]) for x, y in zip(a, b)])
+    err = means.std(ddof=1) / math.sqrt(nw)
+    assert abs(means.mean() - want) < max(4 * err, 0.01), (means.mean(), err, want)
+    W.close()
