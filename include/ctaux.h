@@ -50,7 +50,8 @@ typedef struct ctaux_ctx ctaux_ctx; /* opaque */
 typedef struct ctaux_params {
   int32_t Lx, Ly;          /* periodic cluster, Nc = Lx*Ly, site i = x + Lx*y      */
   double beta;             /* inverse temperature                                      */
-  double U;                /* on-site Hubbard U; N_corr = Nc            */
+  double U;                /* on-site Hubbard U >= 0; N_corr = Nc.  U = 0 (gamma = 0) is
+                              accepted only where the fused small-k path runs (else CTAUX_EINVAL)      */
   double K;                /* CT-AUX expansion parameter K of Eq. (22)            */
   int32_t n_tau;           /* M = number of tau INTERVALS (`sp-time-intervals`);
                               the table has M+1 points per row                                        */

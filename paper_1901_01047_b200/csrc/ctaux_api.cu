@@ -777,6 +777,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     const bool fits = fused_smem_layout(fcap).total <= max_smem && fcap <= 256 && 4 * fcap >= 3 * d.max_k;
     if (prm->fused_small > 0 && !fits) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_ECAPACITY; }
     x->fused = prm->fused_small >= 0 && fits;
+    // U = 0 (gamma = 0, E = 1): the delayed-block formulas divide by E - 1; only the fused path (which never does)
+    // can run this degenerate case -- N stays 1, R_ins = K/(k+1), R_rem = k/K.  Refuse it loudly otherwise.
+    if (d.egp == 1.0 && !x->fused) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_EINVAL; }
     x->fcap = fcap;
     const int need = fused_smem_layout(fcap).total;
     x->fused_smem = need;

@@ -430,3 +430,32 @@ def test_P6_atomic_limit_mean_order_on_the_device(flips):
     err = means.std(ddof=1) / math.sqrt(nw)
     assert abs(means.mean() - want) < max(4 * err, 0.01), (means.mean(), err, want)
     W.close()
+
+
+def test_P5_U_zero_on_the_device():
+    """Degenerate case gamma = 0 (BASELINE.json: "gamma -> 0 leaves N = 1"): the chain is the birth-death process with
+    R_ins = K/(k+1), R_rem = k/K, stationary k ~ Poisson(K): mean = variance = K on the device chains; N = 1; bit-exact
+    against the oracle; the delayed-block path (which divides by E - 1) refuses U = 0 loudly."""
+    pkg = _pkg()
+    K = 1.5
+    cfg = dict(get_config(0), name="U0", U=0.0, K=K, init_k=3)
+    full_parity(cfg, 4, 50, T1, fused=1)
+    table = table_for(cfg)
+    nw = 256
+    W = pkg.Walkers(2, 2, cfg["beta"], 0.0, K, table, delay=8, n_walkers=nw, init_k=3, max_k=64, rebuild_every=0)
+    W.reset(walker_seeds(nw, first=500))
+    W.sweep(50)
+    ks = []
+    for rep in range(40):
+        W.sweep(3)
+        ks += [W.get_stats(w)["k"] for w in range(nw)]
+    ks = np.array(ks, dtype=np.float64)
+    n = ks.size
+    assert abs(ks.mean() - K) < 5 * np.sqrt(K / n) * 3       # autocorrelated samples: generous factor
+    assert abs(ks.var() - K) < 0.15
+    k0 = W.get_stats(0)["k"]
+    assert np.array_equal(W.get_N(0, 0), np.eye(k0)) and np.array_equal(W.get_N(0, 1), np.eye(k0))
+    W.close()
+    with pytest.raises(pkg.CtauxError) as ei:
+        pkg.Walkers(2, 2, cfg["beta"], 0.0, K, table, delay=8, n_walkers=1, init_k=3, max_k=64, fused_small=-1)
+    assert ei.value.code == -1
