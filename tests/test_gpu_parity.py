@@ -459,3 +459,13 @@ def test_P5_U_zero_on_the_device():
     with pytest.raises(pkg.CtauxError) as ei:
         pkg.Walkers(2, 2, cfg["beta"], 0.0, K, table, delay=8, n_walkers=1, init_k=3, max_k=64, fused_small=-1)
     assert ei.value.code == -1
+
+
+@pytest.mark.slow
+def test_config5_thermalised_start_full_size():
+    """Config 5 at full size (6x6, beta 40, k ~ 3600, delay 128: the 2-CTA cluster form of S3, split-K S2 GEMMs,
+    rank-128 flushes) from the oracle-thermalised configuration: one sweep (~3600 proposals, ~30 blocks) of 2
+    seeds, decisions bit-exact, N within 1e-10.  The oracle side costs ~4 min of CPU."""
+    cfg = get_config(4)
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1)
+    assert all(W.get_stats(w)["flushes"] > 10 for w in range(2))
