@@ -466,6 +466,10 @@ def test_config5_thermalised_start_full_size():
     """Config 5 at full size (6x6, beta 40, k ~ 3600, delay 128: the 2-CTA cluster form of S3, split-K S2 GEMMs,
     rank-128 flushes) from the oracle-thermalised configuration: one sweep (~3600 proposals, ~30 blocks) of 2
     seeds, decisions bit-exact, N within 1e-10.  The oracle side costs ~4 min of CPU."""
+    import os
     cfg = get_config(4)
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"thermalised_{cfg['name']}_seed0.txt")
+    if not os.path.exists(golden):
+        pytest.skip("tests/golden/thermalised_cfg5_6x6_b40_seed0.txt not generated (make_thermalised.py, ~1 h of CPU)")
     W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1)
     assert all(W.get_stats(w)["flushes"] > 10 for w in range(2))
