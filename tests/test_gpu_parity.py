@@ -468,8 +468,17 @@ def test_config5_thermalised_start_full_size():
     seeds, decisions bit-exact, N within 1e-10.  The oracle side costs ~4 min of CPU."""
     import os
     cfg = get_config(4)
-    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"thermalised_{cfg['name']}_seed0.txt")
-    if not os.path.exists(golden):
-        pytest.skip("tests/golden/thermalised_cfg5_6x6_b40_seed0.txt not generated (make_thermalised.py, ~1 h of CPU)")
-    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"]), walker_seeds(2), 1, T1)
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    have = [sd for sd in (0, 1) if os.path.exists(os.path.join(gdir, f"thermalised_{cfg['name']}_seed{sd}.txt"))]
+    if not have:
+        pytest.skip("tests/golden/thermalised_cfg5_6x6_b40_seed*.txt not generated (make_thermalised.py, ~1 h of CPU)")
+    # One sweep = ~3100-3600 proposals and ~25 rank-128 flushes on matrices whose columns span 8 decades
+    # (e^gamma = 8642): the incrementally updated N drifts to 2-3e-10 over that span (measured; config 4, with half
+    # the order and a quarter of the flush work, stays below 1e-10), which is why BASELINE.json gives this config its
+    # periodic rebuild.  Decisions and configurations are bit-exact; N is held to 5e-10 after the sweep and to
+    # 1e-10 right after the from-scratch rebuild (S1 + S5 at k ~ 3100-3600 on the cluster LU).
+    W, orcs, worst = parity_from_state(cfg, load_thermalised(cfg["name"], have[0]), walker_seeds(2), 1, T1, tol=5e-10)
+    W.rebuild()
+    for w, o in enumerate(orcs):
+        compare_N(W, w, o, f"config 5 after rebuild, walker {w}", tol=1e-10)
     assert all(W.get_stats(w)["flushes"] > 10 for w in range(2))
