@@ -469,7 +469,7 @@ def test_config5_thermalised_start_full_size():
     import os
     cfg = get_config(4)
     gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
-    have = [sd for sd in (0, 1) if os.path.exists(os.path.join(gdir, f"thermalised_{cfg['name']}_seed{sd}.txt"))]
+    have = [sd for sd in (1, 0) if os.path.exists(os.path.join(gdir, f"thermalised_{cfg['name']}_seed{sd}.txt"))]
     if not have:
         pytest.skip("tests/golden/thermalised_cfg5_6x6_b40_seed*.txt not generated (make_thermalised.py, ~1 h of CPU)")
     # One sweep = ~3100-3600 proposals and ~25 rank-128 flushes on matrices whose columns span 8 decades
