@@ -198,30 +198,6 @@ void ctaux_destroy(ctaux_ctx* ctx);
 const char* ctaux_strerror(int code);
 const char* ctaux_last_cuda_error(void);
 
-/* Stand-alone FP64 GEMM through the library's DMMA tile kernel (the kernel S2/S4/S5 use):
- * C (MxN, ldc) = beta*C + alpha * A (MxK, lda) * B (KxN, ldb), all column-major DEVICE pointers.
- * For measurement and tests. */
-int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
-                int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc);
-
-/* Same, with the kernel chosen explicitly, so that tests and measurements reach every GEMM path:
- * 0 = 128x64 tiles, 8 warps, 2 CTAs/SM;  1 = 64x64 tiles, 8 warps (small-k configurations);
- * 2/3 = persistent kernel, 128x64 / 64x128 tiles, k-step 16 x 4 stages; 4/5 = same, k-step 32 x 3;
- * 6 = 64x64 tiles, 4 warps, 4 CTAs/SM (S2, S5 at large k);  7 = same at 5 CTAs/SM (S4 flush);
- * 8 = kernel 6 with L2 prefetch of the next-wave C0 tile. */
-int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A,
-                   int32_t lda, const double* B, int32_t ldb, double beta, double* C, int32_t ldc,
-                   int32_t kernel);
-
-/* Measurement helper: issue-rate peak of the FP64 pipes on the current device, TFLOP/s.  which = 0: DMMA.8x8x4
- * (mma.sync m8n8k4 f64, the tensor path the GEMM tiles use), 1: DFMA.  One CTA of 256 threads per SM x 2,
- * 16 independent accumulators per warp / thread, CUDA events.  The roofline ceiling beside cuBLAS DGEMM. */
-int ctaux_probe_fp64(int32_t which, double* tflops);
-
-/* Debug / pin helper: Philox4x32-10 evaluated ON THE DEVICE for n (counter, key) pairs.
- * ctr: HOST [n][4], key: HOST [n][2], out: HOST [n][4]. */
-int ctaux_debug_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int32_t n);
-
 #ifdef __cplusplus
 }
 #endif

@@ -39,10 +39,12 @@ class _Stats(C.Structure):
                 ("guard_ends", C.c_int64), ("acc_flip", C.c_int64)]
 
 
+# include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats",
            "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
-           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error", "ctaux_dgemm", "ctaux_dgemm_ex", "ctaux_probe_fp64", "ctaux_debug_philox"]
+           "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
+TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
 
 _lib = None
 
@@ -85,8 +87,7 @@ def load_library():
     L.ctaux_strerror.restype = C.c_char_p
     L.ctaux_strerror.argtypes = [C.c_int]
     L.ctaux_last_cuda_error.restype = C.c_char_p
-    L.ctaux_dgemm.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32]
-    L.ctaux_dgemm_ex.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32]
+    L.ctaux_dgemm.argtypes = [vp, i32, i32, i32, C.c_double, vp, i32, vp, i32, C.c_double, vp, i32, i32]
     L.ctaux_probe_fp64.argtypes = [i32, C.POINTER(C.c_double)]
     L.ctaux_debug_philox.argtypes = [vp, vp, vp, i32]
     _lib = L
@@ -95,7 +96,7 @@ def load_library():
 
 def exported_symbols():
     L = load_library()
-    return {name: hasattr(L, name) for name in EXPORTS}
+    return {name: hasattr(L, name) for name in EXPORTS + TEST_EXPORTS}
 
 
 def _check(rc, what):
@@ -420,8 +421,8 @@ def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, kernel=0):
         assert t.shape[0] <= 1 or t.stride(0) == 1, "column-major operands required"
     ld = lambda t: int(t.stride(1)) if t.shape[1] > 1 else max(2, t.shape[0] + (t.shape[0] & 1))
     s = stream if stream is not None else torch.cuda.current_stream(A.device)
-    _check(L.ctaux_dgemm_ex(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
-                            C_out.data_ptr(), ld(C_out), kernel), "ctaux_dgemm_ex")
+    _check(L.ctaux_dgemm(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
+                         C_out.data_ptr(), ld(C_out), kernel), "ctaux_dgemm")
     return C_out
 
 

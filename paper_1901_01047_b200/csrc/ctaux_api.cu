@@ -2,17 +2,18 @@
 // Every step of the path runs in the kernels of walker_kernels.cuh / gemm_dmma.cuh; the host
 // only enqueues launches and polls the completion flag.
 #include "../../include/ctaux.h"
+#include "../../include/ctaux_testing.h"
 
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <string>
 #include <vector>
 
 #include "gemm_dmma.cuh"
-#include "gemm_persist.cuh"
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
 #include "walker_fused.cuh"
@@ -41,9 +42,7 @@ inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 enum StepClass { C_PREP = 0, C_CAND_GEMM = 1, C_PROPOSE = 2, C_UV = 3, C_FLUSH_GEMM = 4, C_REBUILD = 5, C_OTHER = 6, C_USINV_GEMM = 7, N_CLASS = 8 };
 
 // GEMM tile configurations
-//  big:   128x128x16, 8 warps (2x4), 4 stages  -- flush / candidate columns at large k
-//  small:  64x64x16,  4 warps... (kept at 8 warps: 2x4 -> warp tile 32x16)
-#define GEMM_BIG 128, 64, 4, 2, 4, 2
+//  small:  64x64x16, 8 warps (2x4 -> warp tile 32x16), 4 stages, 2 CTAs/SM -- max_k <= 512
 #define GEMM_SMALL 64, 64, 2, 4, 4, 2
 // large k: 64x64 tiles, 4 warps with 32x32 warp tiles, 2 stages, 4-5 INDEPENDENT CTAs per SM: while one CTA
 // waits for its C0 gather / operands or drains its stores, the others keep the DMMA pipe busy
@@ -182,27 +181,38 @@ struct DescPlain {  // ctaux_dgemm
   __device__ bool operator()(int, GemmDesc& o) const { o = d; return true; }
 };
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (function, device): remember the largest value set
+// per device, under a mutex (contexts are created and driven from several host threads, WalkerGroups).
+struct SmemOptIn {
+  std::mutex mu;
+  int cur[64] = {0};
+  template <class K>
+  cudaError_t ensure(K kern, int bytes) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    std::lock_guard<std::mutex> g(mu);
+    if (bytes <= cur[dev]) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) cur[dev] = bytes;
+    return e;
+  }
+};
+
 template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class Fn>
 cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s, int pf_dist = 0) {
   using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
   auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, MINB, Fn>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+  static SmemOptIn optin;
+  {
+    cudaError_t e = optin.ensure(kern, Cfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   if (tiles_x < 1) tiles_x = 1;
   kern<<<dim3(tiles_x, problems), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(fn, pf_dist);
   return cudaGetLastError();
 }
-
-// persistent kernel (large k): descriptor adaptor that fixes the tile orientation
-template <class F, int WIDE>
-struct PAdapt {
-  F f;
-  __device__ bool operator()(int p, GemmDesc& d, int& wide) const { wide = WIDE; return f(p, d); }
-};
 
 int sm_count() {
   static int n = 0;
@@ -211,29 +221,6 @@ int sm_count() {
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
   }
   return n;
-}
-
-#ifndef CTAUX_PBK
-#define CTAUX_PBK 16
-#define CTAUX_PSTAGES 4
-#endif
-template <int WIDE, int BK, int STAGES, class F>
-cudaError_t launch_persist_cfg(const F& f, int problems, cudaStream_t s) {
-  using Fn = PAdapt<F, WIDE>;
-  auto kern = gemm_persistent_kernel<BK, STAGES, Fn>;
-  constexpr int smem = PCfg<BK, STAGES>::SMEM_BYTES;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  kern<<<sm_count(), kPThreads, smem, s>>>(Fn{f}, problems);
-  return cudaGetLastError();
-}
-template <int WIDE, class F>
-cudaError_t launch_persist(const F& f, int problems, cudaStream_t s) {
-  return launch_persist_cfg<WIDE, CTAUX_PBK, CTAUX_PSTAGES>(f, problems, s);
 }
 
 }  // namespace
@@ -265,7 +252,6 @@ struct ctaux_ctx {
   int fused_smem, fcap;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
-  bool persist;       // large k and few problems: persistent GEMM kernel (gemm_persist.cuh)
   // timing
   bool timing;
   std::vector<cudaEvent_t> ev_pool;
@@ -434,7 +420,8 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     harvest_timing(x);
     double worst = 0.0;
     for (int q = 0; q < P; ++q) { double v; memcpy(&v, &hr[q], 8); worst = v > worst ? v : worst; }
-    if (worst < 1e-4) {
+    // one step squares the residual: accept it only where the refreshed N lands at rounding level (1e-6 -> ~1e-12 k)
+    if (worst < 1e-6) {
       {
         Scoped t(x, C_REBUILD);
         cudaError_t e = x->small_tiles ? launch_gemm<GEMM_SMALL>(DescNS{d, 1}, t64, P, s) : launch_gemm<GEMM_Q4>(DescNS{d, 1}, t64, P, s);
@@ -468,7 +455,6 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
-      if (x->persist) return launch_persist<0>(DescLU{d, j0, which, nbw}, P, s);
       if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
       return launch_gemm<GEMM_Q4>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
     };
@@ -531,10 +517,7 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_CAND_GEMM);
     cudaError_t e1, e2;
-    if (x->persist) {
-      e1 = launch_persist<1>(DescCandRows{d}, P, s);
-      e2 = launch_persist<0>(DescCandCols{d}, P, s);
-    } else if (x->small_tiles) {
+    if (x->small_tiles) {
       e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((kh + 63) / 64), P, s);
       e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (kcap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
     } else {
@@ -586,8 +569,7 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
-    if (x->persist) e3 = launch_persist<0>(DescUSinv{d}, P, s);
-    else if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
     else e3 = launch_gemm<GEMM_Q4>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
@@ -595,9 +577,7 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_FLUSH_GEMM);
     cudaError_t e4;
-    if (x->persist) {
-      e4 = launch_persist<0>(DescFlush{d}, P, s);
-    } else if (x->small_tiles) {
+    if (x->small_tiles) {
       const int tl = (kh + 63) / 64;
       e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
     } else {
@@ -606,12 +586,8 @@ int enqueue_block_step(ctaux_ctx* x) {
       {
         using Cfg = GemmCfg<64, 64, 2, 2, 2>;
         auto kern = gemm_flush_kernel<GEMM_Q5, DescFlush>;
-        static bool configured = false;
-        e4 = cudaSuccess;
-        if (!configured) {
-          e4 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
-          configured = e4 == cudaSuccess;
-        }
+        static SmemOptIn optin;
+        e4 = optin.ensure(kern, Cfg::SMEM_BYTES);
         if (e4 == cudaSuccess) {
           kern<<<dim3(tl * tl, P), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(DescFlush{d}, d.rowmap, d.cap, tl);
           e4 = cudaGetLastError();
@@ -755,13 +731,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     x->sinv_smem = Ls.total <= max_smem;
     if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
     x->propose_smem = Ls.total;
-    if (Ls.total > max_smem) { delete x; return CTAUX_ECAPACITY; }
-    static int propose_attr_max[2] = {0, 0};  // the attribute is per function, shared by all contexts
-    if (Ls.total > propose_attr_max[x->sinv_smem ? 1 : 0]) {
-      e = x->sinv_smem ? cudaFuncSetAttribute(k_propose<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total)
-                       : cudaFuncSetAttribute(k_propose<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Ls.total);
-      if (e == cudaSuccess) propose_attr_max[x->sinv_smem ? 1 : 0] = Ls.total;
-    }
+    if (Ls.total > max_smem) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_ECAPACITY; }
+    static SmemOptIn optin[2];   // the attribute is per function and device, shared by all contexts
+    e = x->sinv_smem ? optin[1].ensure(k_propose<true>, Ls.total) : optin[0].ensure(k_propose<false>, Ls.total);
   }
   if (e != cudaSuccess) {
     g_last_cuda_error = std::string("ctaux_create: ") + cudaGetErrorString(e);
@@ -784,11 +756,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     const int need = fused_smem_layout(fcap).total;
     x->fused_smem = need;
     if (x->fused) {
-      static int fused_attr_max = 0;
-      if (need > fused_attr_max) {
-        if (cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, need) != cudaSuccess) x->fused = false;
-        else fused_attr_max = need;
-      }
+      static SmemOptIn optin;
+      if (optin.ensure(k_walk_fused, need) != cudaSuccess) x->fused = false;
     }
   }
   x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
@@ -797,8 +766,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     // panel width 32: width 64 (k_lu_panel_cl<64>, k_lu_trsm<64>) was measured at the same total time -- the rank-64
     // trailing updates save 17 %, the wider panel and triangular solves cost it again (profiles/r1_v4_kernels_full.md)
     const int need32 = lu_cl_smem_doubles(rl_cap, 32) * 8 + 64;
-    if (need32 <= max_smem &&
-        cudaFuncSetAttribute(k_lu_panel_cl<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, need32) == cudaSuccess) {
+    static SmemOptIn optin_lu;
+    if (need32 <= max_smem && optin_lu.ensure(k_lu_panel_cl<32>, need32) == cudaSuccess) {
       x->lu_cluster = true; x->lu_cluster_smem = need32; x->lu_nb = 32;
     }
     cudaGetLastError();
@@ -809,8 +778,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     int mode = 1;
     if (Lc.total > max_smem) { Lc = propose_cl_smem_layout(d.cap, d.delay, d.winmax, false); mode = 2; }
     if (Lc.total <= max_smem) {
-      cudaError_t ec = mode == 1 ? cudaFuncSetAttribute(k_propose_cl<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lc.total)
-                                 : cudaFuncSetAttribute(k_propose_cl<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, Lc.total);
+      static SmemOptIn optin_cl[2];
+      cudaError_t ec = mode == 1 ? optin_cl[1].ensure(k_propose_cl<true>, Lc.total) : optin_cl[0].ensure(k_propose_cl<false>, Lc.total);
       if (ec == cudaSuccess) { x->cluster_mode = mode; x->cluster_smem = Lc.total; }
       else cudaGetLastError();
     }
@@ -828,9 +797,6 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     }
   }
   x->small_tiles = d.max_k <= 512;   // (64x64 / 4-warp tiles on config 3, k = 245: measured, no gain)
-  // The persistent kernel (gemm_persist.cuh) hides the C0 latency of the flush but its main loop is slower
-  // than two independent 8-warp CTAs per SM (profiles/r1_gemm_variants.md); off until that is fixed.
-  x->persist = false && !x->small_tiles && 2 * d.B <= kPMaxProblems;
   *out = x;
   return CTAUX_OK;
 }
@@ -1059,13 +1025,8 @@ int ctaux_timing_get(ctaux_ctx* x, double* ms, int64_t* launches) {
 }
 
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
-                const double* B, int32_t ldb, double beta, double* C, int32_t ldc) {
-  return ctaux_dgemm_ex(stream, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, 0);
-}
-
-int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
-                   const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel) {
-  if (kernel < 0 || kernel > 8) return CTAUX_EINVAL;
+                const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel) {
+  if (kernel < 0 || kernel > 2) return CTAUX_EINVAL;
   if (M < 0 || N < 0 || K < 0 || !C || ldc < M) return CTAUX_EINVAL;
   if (K > 0 && (!A || !B || lda < M || ldb < K || (lda & 1) || (ldb & 1) || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)))
     return CTAUX_EINVAL;
@@ -1080,15 +1041,9 @@ int ctaux_dgemm_ex(void* stream, int32_t M, int32_t N, int32_t K, double alpha, 
   const int t64 = ((M + 63) / 64) * ((N + 63) / 64);
   cudaError_t e;
   switch (kernel) {
-    case 0: e = launch_gemm<GEMM_BIG>(fn, ((M + 127) / 128) * ((N + 63) / 64), 1, st); break;
-    case 1: e = launch_gemm<GEMM_SMALL>(fn, t64, 1, st); break;
-    case 2: e = launch_persist_cfg<0, 16, 4>(fn, 1, st); break;
-    case 3: e = launch_persist_cfg<1, 16, 4>(fn, 1, st); break;
-    case 4: e = launch_persist_cfg<0, 32, 3>(fn, 1, st); break;
-    case 5: e = launch_persist_cfg<1, 32, 3>(fn, 1, st); break;
-    case 6: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st); break;
-    case 7: e = launch_gemm<GEMM_Q5>(fn, t64, 1, st); break;
-    default: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st, 4 * sm_count()); break;  // 8: with L2 prefetch of C0
+    case 0: e = launch_gemm<GEMM_SMALL>(fn, t64, 1, st); break;
+    case 1: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st); break;
+    default: e = launch_gemm<GEMM_Q5>(fn, t64, 1, st); break;
   }
   CU_CHECK(e);
   return CTAUX_OK;

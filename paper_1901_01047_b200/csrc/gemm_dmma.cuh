@@ -256,7 +256,10 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB) gemm_grouped_kernel(DescFn
 // instead of the problem's own size, so every CTA can issue the loads of its compaction-map entries
 // (map of problem p at maps + (p >> 1) * map_stride, rows and columns alike) BEFORE the device-side descriptor
 // has arrived: the dependent chain  descriptor -> maps -> C0  loses one L2 round trip per CTA.
-// Tiles beyond the live size exit; the map array has at least tmax * BM entries.
+// Tiles beyond the live size exit.  The host's tile count comes from a hint of the live order that can be stale
+// (the order grows by up to `delay` per block step between two polls): when the problem has more tiles than
+// tmax x tmax, the CTAs of the launch stride over the uncovered ones afterwards, so a stale hint costs balance,
+// never correctness.  Speculative map reads are clamped to the walker's own map (map_stride entries).
 template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class DescFn>
 __global__ void __launch_bounds__(WM * WN * 32, MINB)
     gemm_flush_kernel(DescFn fn, const int* maps, int map_stride, int tmax) {
@@ -269,15 +272,29 @@ __global__ void __launch_bounds__(WM * WN * 32, MINB)
   const int* map = maps + (size_t)(blockIdx.y >> 1) * map_stride;
   int psrow[TM], pscol[TN * 2];
 #pragma unroll
-  for (int i = 0; i < TM; ++i) psrow[i] = __ldg(map + tile_m * BM + wm * (TM * 8) + i * 8 + g);
+  for (int i = 0; i < TM; ++i) psrow[i] = __ldg(map + min(tile_m * BM + wm * (TM * 8) + i * 8 + g, map_stride - 1));
 #pragma unroll
   for (int j = 0; j < TN; ++j)
 #pragma unroll
-    for (int h = 0; h < 2; ++h) pscol[j * 2 + h] = __ldg(map + tile_n * BN + wn * (TN * 8) + j * 8 + 2 * q + h);
+    for (int h = 0; h < 2; ++h)
+      pscol[j * 2 + h] = __ldg(map + min(tile_n * BN + wn * (TN * 8) + j * 8 + 2 * q + h, map_stride - 1));
   GemmDesc d;
   if (!fn(blockIdx.y, d)) return;
-  if (tile_m * BM >= d.M || tile_n * BN >= d.N) return;
-  gemm_tile<BM, BN, WM, WN, STAGES, true>(d, tile_m, tile_n, smem_gemm, psrow, pscol);
+  if (tile_m * BM < d.M && tile_n * BN < d.N)
+    gemm_tile<BM, BN, WM, WN, STAGES, true>(d, tile_m, tile_n, smem_gemm, psrow, pscol);
+  const int tm = (d.M + BM - 1) / BM, tn = (d.N + BN - 1) / BN;
+  if (tm <= tmax && tn <= tmax) return;
+  // uncovered tiles: rows of tiles at or beyond tmax (all columns), then columns at or beyond tmax of the covered rows
+  const int rows_x = tm > tmax ? tm - tmax : 0, cols_x = tn > tmax ? tn - tmax : 0;
+  const int tm_cov = tm < tmax ? tm : tmax;
+  const int extra = rows_x * tn + tm_cov * cols_x;
+  for (int e = blockIdx.x; e < extra; e += gridDim.x) {
+    int em, en;
+    if (e < rows_x * tn) { em = tmax + e % rows_x; en = e / rows_x; }
+    else { const int f = e - rows_x * tn; em = f % tm_cov; en = tmax + f / tm_cov; }
+    __syncthreads();   // the shared-memory ring of the previous tile is free
+    gemm_tile<BM, BN, WM, WN, STAGES>(d, em, en, smem_gemm);
+  }
 }
 
 }  // namespace ctaux

@@ -178,3 +178,86 @@ def parity_from_state(cfg, state, seeds, n_sweeps, mode, n_proposals=None, delay
             assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id, what
             worst = max([worst] + compare_N(W, w, o, what, tol=tol))
     return W, orcs, worst
+
+
+# ------------------------------------------------------------------ log replay by brute-force determinants
+def replay_windows(start_cfg, log, windows):
+    """Apply the accepted moves of `log` (entries numbered from the start configuration) to the start configuration and
+    return, for every proposal index inside one of the half-open `windows`, the configuration BEFORE that proposal:
+    list of (index, site list, tau list, spin list, version), version = number of accepted moves so far (two
+    proposals with the same version meet the same configuration)."""
+    site, tau, spin = list(start_cfg["site"]), list(start_cfg["tau"]), list(start_cfg["spin"])
+    want = sorted(i for lo, hi in windows for i in range(lo, hi))
+    out, version, wi = [], 0, 0
+    for i, e in enumerate(log):
+        if wi < len(want) and want[wi] == i:
+            out.append((i, list(site), list(tau), list(spin), version))
+            wi += 1
+        if wi >= len(want):
+            break
+        if e["accepted"]:
+            if e["type"] == 0:
+                site.append(int(e["arg"])); tau.append(float(e["tau"])); spin.append(int(e["spin"]))
+            elif e["type"] == 1:
+                j = int(e["arg"])
+                del site[j], tau[j], spin[j]
+            else:
+                spin[int(e["arg"])] = -spin[int(e["arg"])]
+            version += 1
+    return out
+
+
+def brute_force_verify(cfg, table, start_cfg, log, windows, rtol=1e-7, atol=1e-9, what=""):
+    """SURVEY 8d "log-replay verification" (built on P:201 Eq. (27)): every logged ratio R and every decision inside
+    the windows is re-derived from scratch -- the configuration before the proposal is rebuilt from the log, the
+    matrices A_sigma and A'_sigma are built by the oracle from the two vertex lists, their determinants are taken by
+    LAPACK (numpy slogdet), R = prefactor x prod_sigma det A'/det A, decision = (u < |R|).  Nothing of any fast-update
+    formula (Woodbury block on the device, rank-1 formulas of the oracle's T1 mode) enters.  Independent per proposal,
+    so it runs in parallel over the host cores; by induction a window whose ratios and decisions all check is a piece
+    of the brute-force chain.  Returns the largest |R_log - R_bf| / (rtol |R_bf| + atol)."""
+    snaps = replay_windows(start_cfg, log, windows)
+    K = cfg["K"]
+
+    def logdets(site, tau, spin):
+        if not site:
+            return [(0.0, 1.0), (0.0, 1.0)]
+        probe = OracleWalker.from_config(cfg, table, 0, T0)
+        probe.set_state(np.array(site, np.int32), np.array(tau), np.array(spin, np.int8))
+        out = []
+        for s in range(2):
+            sg, la = np.linalg.slogdet(probe.A(s))
+            out.append((la, sg))
+        return out
+
+    def one(snap):
+        i, site, tau, spin, version = snap
+        e = log[i]
+        k = len(site)
+        if e["type"] != 0 and k == 0:
+            return i, 0.0, None
+        d0 = logdets(site, tau, spin)
+        if e["type"] == 0:
+            s2, t2, p2 = site + [int(e["arg"])], tau + [float(e["tau"])], spin + [int(e["spin"])]
+            pref = K / (k + 1)
+        elif e["type"] == 1:
+            j = int(e["arg"])
+            s2, t2, p2 = site[:j] + site[j + 1:], tau[:j] + tau[j + 1:], spin[:j] + spin[j + 1:]
+            pref = k / K
+        else:
+            j = int(e["arg"])
+            s2, t2, p2 = site, tau, spin[:j] + [-spin[j]] + spin[j + 1:]
+            pref = 1.0
+        d1 = logdets(s2, t2, p2)
+        R = pref * d1[0][1] * d1[1][1] * d0[0][1] * d0[1][1] * math.exp(d1[0][0] + d1[1][0] - d0[0][0] - d0[1][0])
+        return i, R, None
+
+    with ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as ex:
+        res = list(ex.map(one, snaps))
+    worst = 0.0
+    for i, R, _ in res:
+        e = log[i]
+        err = abs(e["R"] - R) / (rtol * abs(R) + atol)
+        worst = max(worst, err)
+        assert err < 1.0, f"{what}: proposal {i}: logged R {e['R']!r} vs brute force {R!r} (x{err:.2e} of tolerance)"
+        assert int(e["accepted"]) == (1 if e["u"] < abs(R) else 0), f"{what}: proposal {i}: decision differs from brute force"
+    return worst

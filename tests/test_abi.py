@@ -13,10 +13,11 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "ctaux.h")
+TEST_HEADER = os.path.join(ROOT, "include", "ctaux_testing.h")
 
 
-def _declared():
-    src = open(HEADER).read()
+def _declared(header=HEADER):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(ctaux_[a-z_A-Z0-9]+)\s*\(", src)))
 
@@ -25,10 +26,14 @@ def test_library_exports_every_declared_symbol():
     from paper_1901_01047_b200 import binding
     L = binding.load_library()
     names = _declared()
-    assert len(names) >= 20
-    missing = [n for n in names if not hasattr(L, n)]
+    assert len(names) >= 19
+    helpers = _declared(TEST_HEADER)
+    missing = [n for n in names + helpers if not hasattr(L, n)]
     assert not missing, missing
     assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and include/ctaux.h disagree"
+    assert sorted(binding.TEST_EXPORTS) == helpers, "binding.TEST_EXPORTS and include/ctaux_testing.h disagree"
+    # every header under include/ is covered
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["ctaux.h", "ctaux_testing.h"]
 
 
 def test_ctypes_structs_match_the_header():

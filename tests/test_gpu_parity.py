@@ -36,7 +36,7 @@ def test_P12_device_philox_equals_oracle_philox():
         assert dev[i].tolist() == philox(ctr[i], key[i]).tolist()
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K,alpha,beta", [(1, 1, 1, -1.5, 0.5), (8, 8, 4, -1.5, 0.5), (130, 70, 33, -1.5, 0.5),
                                               (128, 128, 64, -1.0, 1.0), (257, 511, 100, -1.5, 0.5),
                                               (1000, 40, 1000, 1.0, 0.0), (64, 1000, 7, -1.0, 1.0),
@@ -44,9 +44,8 @@ def test_P12_device_philox_equals_oracle_philox():
                                               (64, 1834, 1834, 1.0, 0.0), (1898, 64, 1898, 1.0, 0.0),
                                               (700, 900, 129, 1.0, 1.0)])
 def test_dgemm_tiles_against_torch_fp64(M, N, K, alpha, beta, kernel):
-    """Every DMMA GEMM path (0/1: tile kernels of the small configs, 2/3: persistent kernel in both
-    tile orientations; several tiles, several K chunks, ragged tails, the in-place C0 - A*B form)
-    against torch's FP64 matmul."""
+    """Every DMMA GEMM tile configuration the walker launches (several tiles, several K chunks, ragged tails,
+    the in-place C0 - A*B form) against torch's FP64 matmul."""
     import torch
     pkg = _pkg()
     g = torch.Generator(device="cpu").manual_seed(M * 7 + N * 3 + K)
@@ -233,6 +232,20 @@ def test_config4_prefix_T1():
     """Config 4 (6x6, beta 20) from reset, k ~ 1100-1300: first 2 sweeps of 2 walkers against T1."""
     cfg = get_config(3)
     full_parity(cfg, 2, 2, T1, n_tol=N_TOL_THERMALISING)
+
+
+@pytest.mark.slow
+def test_config4_growth_from_empty_start_outruns_the_grid_hint():
+    """Large-k path (max_k > 512) from the EMPTY configuration without any rebuild: k grows from 0 to ~1000 in 18
+    sweeps, by up to ~60 per block step, i.e. several hundred between two polls of the host's live-order hint, so the
+    flush grid sized from that hint is too small again and again; the kernel strides over the tiles the grid does
+    not cover.  Any row or column of N left unwritten would derail the decisions within a few proposals."""
+    cfg = get_config(3)
+    W, orcs, worst = full_parity(cfg, 2, 18, T1, init_k=0, rebuild_every=0, check_N=False)
+    assert min(o.k for o in orcs) > 800
+    W.rebuild()
+    for w, o in enumerate(orcs):
+        compare_N(W, w, o, f"config 4 after growth + rebuild, walker {w}")
 
 
 @pytest.mark.slow

@@ -97,11 +97,13 @@ def _fock_ops(nsite):
     return ops
 
 
-def _fock_trace(Lx, Ly, beta, mu, sites, taus, avals):
-    """Tr[T_tau e^{-beta H0} prod_i e^{a_i n_{x_i}(tau_i)}] / Tr e^{-beta H0}: Eq. (27) literally."""
+def _fock_trace(Lx, Ly, beta, mu, sites, taus, avals, eps=None):
+    """Tr[T_tau e^{-beta H0} prod_i e^{a_i n_{x_i}(tau_i)}] / Tr e^{-beta H0}: Eq. (27) literally.
+    `eps`: dispersion on the cluster momenta (default: the isotropic one of Eq. (45))."""
     from ctaux_workloads import cluster_dispersion
     Nc = Lx * Ly
-    kx, ky, eps = cluster_dispersion(Lx, Ly)
+    kx, ky, eps0 = cluster_dispersion(Lx, Ly)
+    eps = eps0 if eps is None else eps
     h = np.zeros((Nc, Nc))
     for i in range(Nc):
         for j in range(Nc):
@@ -155,6 +157,57 @@ def test_P3_fock_space_trace_equals_det_A(mu, nv):
             la, sg = w.logdet(sidx)
             assert abs(got / want - 1) < 1e-11
             assert abs(sg * math.exp(la) / want - 1) < 1e-11
+
+
+@pytest.mark.parametrize("Lx,Ly,ty", [(3, 3, 1.0), (3, 2, 1.0), (2, 3, 1.0), (3, 3, 0.6)])
+@pytest.mark.parametrize("mu", [0.0, -0.3])
+def test_P3_fock_space_trace_on_3x3_and_3x2_clusters(Lx, Ly, ty, mu):
+    """Pins the displacement index d(i,j) = ((xi-xj) mod Lx) + Lx ((yi-yj) mod Ly) beyond the 2x2 cluster, where
+    (xi-xj) mod 2 cannot tell a wrap, a wrong row stride or an x<->y mix-up apart (Eq. (27) evaluated literally in
+    the 2^Nc-dimensional Fock space, Nc = 9 / 6, against det A of the oracle).  Lx != Ly catches a row stride of Ly
+    instead of Lx and swapped moduli; the 3x3 cluster with anisotropic hopping (t_y = 0.6 t_x, table built here from
+    the same closed form) catches an x<->y mix-up that the isotropic square cluster hides (g(dx,dy) = g(dy,dx)
+    there).  Every parameter set includes pairs whose raw displacement is negative in x, in y and in both (wraps)."""
+    from ctaux_workloads import cluster_dispersion
+    beta, U, K, M = 2.0, 4.0, 1.0, 256
+    Nc = Lx * Ly
+    kx, ky, _ = cluster_dispersion(Lx, Ly)
+    eps = -2.0 * (np.cos(kx) + ty * np.cos(ky))
+    if ty == 1.0:
+        T = g0_table(Lx, Ly, beta, mu, M)
+    else:   # closed form G0(r,tau) = -(1/Nc) sum_k cos(k.r) e^{-xi tau}/(1+e^{-beta xi}) with the anisotropic xi_k
+        tau = np.arange(M + 1) * (beta / M)
+        xi = eps - mu
+        wgt = np.exp(-xi[:, None] * tau[None, :]) / (1.0 + np.exp(-beta * xi[:, None]))
+        T = np.empty((Nc, M + 1))
+        for dy in range(Ly):
+            for dx in range(Lx):
+                T[dx + Lx * dy] = -(np.cos(kx * dx + ky * dy)[:, None] * wgt).sum(axis=0) / Nc
+        assert abs(T[1, 7] - T[Lx, 7]) > 1e-3          # g((1,0)) != g((0,1)): the table can tell x from y
+    rng = np.random.default_rng(1000 * Lx + 100 * Ly + int(10 * ty))
+    wraps = set()
+    for nv in (1, 2, 3, 4):
+        for trial in range(3):
+            sites = rng.integers(0, Nc, nv).astype(np.int32)
+            if nv == 2 and trial == 0:
+                sites = np.array([0, Nc - 1], np.int32)          # (0,0) and (Lx-1,Ly-1): wraps in x and y both ways
+            if nv == 3 and trial == 0:
+                sites = np.array([Lx - 1, Lx * (Ly - 1), 1], np.int32)   # x-only and y-only wraps, mixed (dx,dy)
+            taus = rng.choice(np.arange(1, M), nv, replace=False) * beta / M
+            spins = rng.choice([-1, 1], nv).astype(np.int8)
+            for i in sites:
+                for j in sites:
+                    wraps.add((int(i % Lx < j % Lx), int(i // Lx < j // Lx)))
+            w = OracleWalker(Lx, Ly, beta, U, K, T, 0)
+            w.set_state(sites, taus, spins)
+            gamma = math.log(w.exp_gamma)
+            for sidx, sigma in enumerate([+1, -1]):
+                a = [-gamma * sigma * int(s) for s in spins]
+                want = _fock_trace(Lx, Ly, beta, mu, sites, taus, a, eps=eps)
+                la, sg = w.logdet(sidx)
+                assert abs(sg * math.exp(la) / want - 1) < 1e-10, (Lx, Ly, ty, mu, nv, trial, sidx)
+                assert abs(np.linalg.det(w.A(sidx)) / want - 1) < 1e-10
+    assert wraps == {(0, 0), (0, 1), (1, 0), (1, 1)}
 
 
 # ----------------------------------------------------------------------------- P4: one vertex
@@ -528,3 +581,28 @@ def test_flips_keep_the_stationary_distribution():
     err = means.std(ddof=1) / math.sqrt(len(means))
     assert acc > 1000
     assert abs(means.mean() - want) < max(4 * err, 0.02), (means.mean(), err, want)
+
+
+# ----------------------------------------------------------------------------- T1 at the sizes it referees
+@pytest.mark.parametrize("name,seed,nprop", [("cfg4_6x6_b20", 0, 48), ("cfg5_6x6_b40", 1, 16)])
+def test_T1_equals_brute_force_at_full_size(name, seed, nprop):
+    """The rank-1 oracle (T1) referees the parity tests on configs 4-5 (k ~ 1700-3600, e^gamma = 4322 / 8642), far
+    from the k <= 65 where it is compared with T0 proposal by proposal.  Here: from the thermalised configuration of
+    tests/golden (written by the oracle), T1 runs `nprop` proposals; every logged ratio and decision is re-derived by
+    brute force -- A and A' built from the vertex lists, determinants by LAPACK (Eq. (27); SURVEY 8d log-replay
+    protocol) -- and T1's incrementally updated N is compared with the from-scratch inverse."""
+    from parity_helpers import brute_force_verify, load_thermalised
+    cfg = get_config(name)
+    T = table_for(cfg)
+    c0, next_id, p0 = load_thermalised(name, seed)
+    o = OracleWalker.from_config(cfg, T, 5, T1)
+    o.set_state(c0["site"], c0["tau"], c0["spin"], c0["id"], next_id, p0)
+    o.propose(nprop)
+    log = o.log()
+    assert log["accepted"].sum() >= nprop // 4 and set(np.unique(log["type"])) == {0, 1}
+    worst = brute_force_verify(cfg, T, c0, log, [(0, nprop)], rtol=1e-8, atol=1e-10, what=name)
+    assert worst < 1.0
+    for s in range(2):
+        Ninc, Ndir = o.N_incremental(s), o.N(s)
+        assert np.linalg.norm(Ninc - Ndir) / np.linalg.norm(Ndir) < 1e-10
+        assert np.linalg.norm(Ndir - np.linalg.inv(o.A(s))) / np.linalg.norm(Ndir) < 1e-10
