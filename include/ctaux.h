@@ -96,6 +96,16 @@ typedef struct ctaux_params {
                               (w6 * 3) >> 32 (0 insert, 1 remove, 2 flip), flip of the vertex at list position
                               (w1 * k) >> 32, R = prod_sigma det A'/det A.  0 (default): the two-move chain of
                               BASELINE.json.  This DOES change the chain (it is a different sampler).          */
+  double n_tol;            /* accuracy the library HOLDS for every N_sigma it hands out, as a relative Frobenius error against
+                              the exact inverse of A rebuilt from the configuration (BASELINE.json: 1e-10).  Fast updates of
+                              an inverse amplify the error N already carries, at a data-dependent rate, so a fixed cadence
+                              either wastes rebuilds or misses the bar: the library ESTIMATES the forward error of every
+                              N_sigma on the device (a 4-probe Hutchinson estimate of |(N A - 1) N|_F / |N|_F: two passes
+                              over N, A never stored) at the end of every ctaux_sweep call and every few block steps inside
+                              it, and runs the from-scratch rebuild (S1 + S5) of the context when the estimate exceeds
+                              n_tol / 3 at the end of a call (30 n_tol inside a call, where only the acceptance ratios depend
+                              on it).  0 = library default 1e-10; < 0 = monitor off (fixed cadence `rebuild_every` only).
+                              Chain-neutral like every rebuild.                                                            */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */
@@ -118,6 +128,8 @@ typedef struct ctaux_stats {
   double flops_usinv;      /* S4: 2*k'*r*r (U * S^-1), both spins                                     */
   int64_t guard_ends;      /* blocks ended early by the numerical guard (ctaux_params.guard_amp)      */
   int64_t acc_flip;        /* accepted auxiliary-spin flips since reset (flip_moves = 1)              */
+  int64_t monitor_rebuilds;/* rebuilds triggered by the error monitor (ctaux_params.n_tol), included in `rebuilds` */
+  double err_est;          /* last forward-error estimate of this walker's N (max over the two spins; 0 = none yet)  */
 } ctaux_stats;
 
 /* One entry of the decision log (48 bytes). */

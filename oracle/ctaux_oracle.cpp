@@ -597,6 +597,16 @@ void orc_get_A(void* h, int sidx, double* out) {
   w->build_A(sidx, w->L, A);
   std::copy(A.begin(), A.end(), out);
 }
+// A_sigma of a GIVEN vertex list (row-major k x k); the walker's own state is not touched.  Accessor for the
+// log-replay checks of the tests (determinants then taken by LAPACK): same build_A as everywhere else.
+void orc_build_A(void* h, int sidx, int k, const int32_t* site, const double* tau, const int8_t* spin, double* out) {
+  const Walker* w = (const Walker*)h;
+  std::vector<Vertex> V((size_t)k);
+  for (int i = 0; i < k; ++i) { V[i].id = (uint64_t)i; V[i].site = site[i]; V[i].tau = tau[i]; V[i].spin = spin[i]; }
+  std::vector<double> A;
+  w->build_A(sidx, V, A);
+  std::copy(A.begin(), A.end(), out);
+}
 // N_sigma = A_sigma^{-1} by DIRECT inversion (the definition), row-major. Returns 0 ok, -1 singular.
 int orc_get_N(void* h, int sidx, double* out) {
   Walker* w = (Walker*)h;

@@ -56,6 +56,7 @@ def lib():
             getattr(L, name).argtypes = [vp]
         L.orc_get_config.argtypes = [vp, vp, vp, vp, vp]
         L.orc_get_A.argtypes = [vp, i32, vp]
+        L.orc_build_A.argtypes = [vp, i32, i32, vp, vp, vp, vp]
         L.orc_get_N.argtypes = [vp, i32, vp]
         L.orc_get_N.restype = i32
         L.orc_get_N_incremental.argtypes = [vp, i32, vp]
@@ -160,6 +161,16 @@ class OracleWalker:
         k = self.k
         out = np.zeros((k, k), np.float64)
         lib().orc_get_A(self._h, sidx, out.ctypes.data)
+        return out
+
+    def A_of(self, sidx, site, tau, spin):
+        """A_sigma of a given vertex list (the walker's own configuration is not touched)."""
+        site = np.ascontiguousarray(site, dtype=np.int32)
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        spin = np.ascontiguousarray(spin, dtype=np.int8)
+        k = site.size
+        out = np.zeros((k, k), np.float64)
+        lib().orc_build_A(self._h, sidx, k, site.ctypes.data, tau.ctypes.data, spin.ctypes.data, out.ctypes.data)
         return out
 
     def N(self, sidx):

@@ -26,7 +26,8 @@ class _Params(C.Structure):
                 ("delay", C.c_int32), ("n_walkers", C.c_int32), ("init_k", C.c_int32),
                 ("max_k", C.c_int32), ("rebuild_every", C.c_int32), ("log_capacity", C.c_int32),
                 ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
-                ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32), ("flip_moves", C.c_int32)]
+                ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32), ("flip_moves", C.c_int32),
+                ("n_tol", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -36,7 +37,8 @@ class _Stats(C.Structure):
                 ("k", C.c_int32), ("sign", C.c_int32), ("flops_cand", C.c_double),
                 ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
                 ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double),
-                ("guard_ends", C.c_int64), ("acc_flip", C.c_int64)]
+                ("guard_ends", C.c_int64), ("acc_flip", C.c_int64), ("monitor_rebuilds", C.c_int64),
+                ("err_est", C.c_double)]
 
 
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
@@ -113,7 +115,7 @@ class Walkers:
 
     def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
                  rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None,
-                 guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0):
+                 guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0, n_tol=0.0):
         import torch
         if not torch.cuda.is_available():
             raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
@@ -134,6 +136,7 @@ class Walkers:
         p.fused_small = fused_small
         p.rebuild_mode = rebuild_mode
         p.flip_moves = flip_moves
+        p.n_tol = n_tol
         nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
         if nbytes == 0:
             raise CtauxError(-1, "ctaux_workspace_bytes", "invalid parameters")

@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 
+#include "error_monitor.cuh"
 #include "gemm_dmma.cuh"
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
@@ -250,6 +251,15 @@ struct ctaux_ctx {
   int cluster_smem;
   bool fused;         // small-k path: whole sweeps in k_walk_fused (walker_fused.cuh)
   int fused_smem, fcap;
+  // error monitor (ctaux_params.n_tol; error_monitor.cuh)
+  double n_tol;       // <= 0: off
+  double* mon;        // device [2B][3][kProbes][ld]
+  double* est_d;      // device [2B]
+  double* host_est;   // pinned [2B]
+  std::vector<double> last_est;   // per walker, max over spins
+  std::vector<int64_t> mon_rebuilds;
+  bool n_fresh;       // N comes straight from a rebuild: nothing to check
+  uint32_t probe_salt;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
   // timing
@@ -265,7 +275,7 @@ namespace {
 
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
-      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, total;
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -338,6 +348,8 @@ Layout make_layout(const DevCtx& d) {
   L.skbuf = take(d.max_k > 512 ? B * 2 * kMaxSplitK * d.skstride * 8 : 0);
   L.Tbuf = take(d.Tbuf ? B * 2 * (size_t)d.ld * d.ld * 8 : 0);   // d.Tbuf != null here only flags rebuild_mode 1
   L.resid = take(B * 2 * 8);
+  L.mon = take(B * 2 * 3 * kProbes * (size_t)d.ld * 8);
+  L.est = take(B * 2 * 8);
   L.total = o;
   return L;
 }
@@ -388,8 +400,48 @@ int grid_for(size_t work, int threads, int cap_blocks = 4096) {
   return (int)b;
 }
 
+void free_pinned(ctaux_ctx* x) {
+  if (x->host_flag) cudaFreeHost(x->host_flag);
+  if (x->host_est) cudaFreeHost(x->host_est);
+  x->host_flag = nullptr; x->host_est = nullptr;
+}
+
+// Error monitor: enqueue the forward-error estimate of every N (error_monitor.cuh) and its copy to pinned host memory.
+// The caller synchronises the stream before reading host_est.
+int enqueue_err_probe(ctaux_ctx* x) {
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  const int P = d.B * 2;
+  int kh = x->k_hint + 8 * d.delay;
+  if (kh > d.max_k) kh = d.max_k;
+  const int gx = kh / kMonWarps + 1 < 148 ? kh / kMonWarps + 1 : 148;   // the kernels stride over their columns
+  const uint32_t salt = ++x->probe_salt;
+  {
+    Scoped t(x, C_OTHER);
+    k_mon_vecmat<<<dim3(gx, P), kMonWarps * 32, 0, s>>>(d, x->mon, -1, 0, salt);
+    k_mon_resid<<<dim3(gx, P), kMonWarps * 32, 0, s>>>(d, x->mon, salt);
+    k_mon_vecmat<<<dim3(gx, P), kMonWarps * 32, 0, s>>>(d, x->mon, 1, 2, salt);
+    k_mon_final<<<P, 256, 0, s>>>(d, x->mon, x->est_d);
+    tick(x, C_OTHER); tick(x, C_OTHER); tick(x, C_OTHER); tick(x, C_OTHER);
+  }
+  CU_CHECK(cudaGetLastError());
+  CU_CHECK(cudaMemcpyAsync(x->host_est, x->est_d, sizeof(double) * P, cudaMemcpyDeviceToHost, s));
+  return CTAUX_OK;
+}
+// after a synchronise: record the estimates, return the largest
+double harvest_err_probe(ctaux_ctx* x) {
+  double worst = 0.0;
+  for (int w = 0; w < x->d.B; ++w) {
+    const double e = x->host_est[2 * w] > x->host_est[2 * w + 1] ? x->host_est[2 * w] : x->host_est[2 * w + 1];
+    x->last_est[w] = e;
+    worst = e > worst ? e : worst;
+  }
+  return worst;
+}
+
 // S5: from-scratch inverse of every walker's A (current configuration) into the current N buffer
 int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
+  x->n_fresh = true;
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
   // expansion orders are on the device: fetch the maximum (rebuilds are rare)
@@ -611,6 +663,7 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
       Scoped t(x, C_PROPOSE);
       k_walk_fused<<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
       tick(x, C_PROPOSE);
+      x->n_fresh = false;
     }
     CU_CHECK(cudaGetLastError());
     CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -639,11 +692,20 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
       int rc = enqueue_block_step(x);
       if (rc) return rc;
     }
+    x->n_fresh = false;
+    const bool probe = x->n_tol > 0.0;
+    if (probe) { int rc = enqueue_err_probe(x); if (rc) return rc; }
     CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(cudaStreamSynchronize(s));
     harvest_timing(x);
     if (x->host_flag[1] > 0) x->k_hint = x->host_flag[1];
     if (x->host_flag[0] <= 0) break;
+    // inside a call only the acceptance ratios depend on N: rebuild when the estimate passes 30 n_tol
+    if (probe && harvest_err_probe(x) > 30.0 * x->n_tol) {
+      int rc = do_rebuild(x, false, true);
+      if (rc) return rc;
+      for (int w = 0; w < d.B; ++w) x->mon_rebuilds[w] += 1;
+    }
   }
   // errors raised inside kernels
   std::vector<WalkerState> h(d.B);
@@ -705,6 +767,14 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   d.skbuf = (double*)(base + L.skbuf);
   d.Tbuf = prm->rebuild_mode == 1 ? (double*)(base + L.Tbuf) : nullptr;
   d.resid = (unsigned long long*)(base + L.resid);
+  x->mon = (double*)(base + L.mon);
+  x->est_d = (double*)(base + L.est);
+  x->n_tol = prm->n_tol == 0.0 ? 1e-10 : prm->n_tol;
+  x->host_est = nullptr;
+  x->last_est.assign(d.B, 0.0);
+  x->mon_rebuilds.assign(d.B, 0);
+  x->n_fresh = false;
+  x->probe_salt = 0;
   x->detsign = (int*)(base + L.detsign);
   x->seeds_d = (uint64_t*)(base + L.seeds);
   d.g00 = -prm->g0_table[0];
@@ -721,6 +791,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   cudaError_t e = cudaMemsetAsync(base, 0, L.total, x->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)d.table, prm->g0_table, (size_t)d.Nc * (d.M + 1) * 8, cudaMemcpyHostToDevice, x->stream);
   if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_flag, 2 * sizeof(int));
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_est, 2 * d.B * sizeof(double));
   if (e == cudaSuccess) e = cudaStreamSynchronize(x->stream);
   // proposal kernel shared memory: keep S^-1 of both spins in shared memory when it fits
   int dev = 0, max_smem = 0;
@@ -731,13 +802,13 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     x->sinv_smem = Ls.total <= max_smem;
     if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
     x->propose_smem = Ls.total;
-    if (Ls.total > max_smem) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_ECAPACITY; }
+    if (Ls.total > max_smem) { free_pinned(x); delete x; return CTAUX_ECAPACITY; }
     static SmemOptIn optin[2];   // the attribute is per function and device, shared by all contexts
     e = x->sinv_smem ? optin[1].ensure(k_propose<true>, Ls.total) : optin[0].ensure(k_propose<false>, Ls.total);
   }
   if (e != cudaSuccess) {
     g_last_cuda_error = std::string("ctaux_create: ") + cudaGetErrorString(e);
-    if (x->host_flag) cudaFreeHost(x->host_flag);
+    free_pinned(x);
     delete x;
     return CTAUX_ECUDA;
   }
@@ -747,11 +818,11 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     int fcap = d.max_k;
     while (fcap > 8 && fused_smem_layout(fcap).total > max_smem) fcap -= 4;
     const bool fits = fused_smem_layout(fcap).total <= max_smem && fcap <= 256 && 4 * fcap >= 3 * d.max_k;
-    if (prm->fused_small > 0 && !fits) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_ECAPACITY; }
+    if (prm->fused_small > 0 && !fits) { free_pinned(x); delete x; return CTAUX_ECAPACITY; }
     x->fused = prm->fused_small >= 0 && fits;
     // U = 0 (gamma = 0, E = 1): the delayed-block formulas divide by E - 1; only the fused path (which never does)
     // can run this degenerate case -- N stays 1, R_ins = K/(k+1), R_rem = k/K.  Refuse it loudly otherwise.
-    if (d.egp == 1.0 && !x->fused) { if (x->host_flag) cudaFreeHost(x->host_flag); delete x; return CTAUX_EINVAL; }
+    if (d.egp == 1.0 && !x->fused) { free_pinned(x); delete x; return CTAUX_EINVAL; }
     x->fcap = fcap;
     const int need = fused_smem_layout(fcap).total;
     x->fused_smem = need;
@@ -806,7 +877,7 @@ void ctaux_destroy(ctaux_ctx* x) {
   cudaStreamSynchronize(x->stream);
   for (cudaEvent_t e : x->ev_pool) cudaEventDestroy(e);
   if (x->hi) { cudaStreamSynchronize(x->hi); cudaStreamDestroy(x->hi); cudaEventDestroy(x->ev_fork); cudaEventDestroy(x->ev_join); }
-  if (x->host_flag) cudaFreeHost(x->host_flag);
+  free_pinned(x);
   delete x;
 }
 
@@ -885,6 +956,20 @@ int ctaux_sweep(ctaux_ctx* x, int32_t n_sweeps) {
     if (re > 0 && x->sweeps_since_rebuild >= re) {
       rc = do_rebuild(x, false, true);
       if (rc) { x->have_state = false; return rc; }
+      x->sweeps_since_rebuild = 0;
+    }
+  }
+  // what the caller reads after this call is held to n_tol: estimate the forward error of every N and rebuild the
+  // context when the estimate (safety factor 3 for the variance of the 4-probe estimator) says it is needed
+  if (x->n_tol > 0.0 && !x->n_fresh) {
+    int rc = enqueue_err_probe(x);
+    if (rc) { x->have_state = false; return rc; }
+    CU_CHECK(cudaStreamSynchronize(x->stream));
+    harvest_timing(x);
+    if (harvest_err_probe(x) > x->n_tol / 3.0) {
+      rc = do_rebuild(x, false, true);
+      if (rc) { x->have_state = false; return rc; }
+      for (int w = 0; w < x->d.B; ++w) x->mon_rebuilds[w] += 1;
       x->sweeps_since_rebuild = 0;
     }
   }
@@ -986,6 +1071,7 @@ int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   out->flops_cand = st.flops_cand; out->flops_flush = st.flops_flush; out->flops_rebuild = st.flops_rebuild;
   out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
   out->guard_ends = st.guard_ends; out->acc_flip = st.acc_flip;
+  out->monitor_rebuilds = x->mon_rebuilds[w]; out->err_est = x->last_est[w];
   return CTAUX_OK;
 }
 
