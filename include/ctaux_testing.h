@@ -11,12 +11,14 @@
 extern "C" {
 #endif
 
-/* Stand-alone FP64 GEMM through the library's DMMA tile kernels (the kernels S2 / S4 / S5 use):
- * C (MxN, ldc) = beta*C + alpha * A (MxK, lda) * B (KxN, ldb), all column-major DEVICE pointers, lda / ldb even,
- * A and B 16-byte aligned.  kernel: 0 = 64x64 tiles, 8 warps (configurations with max_k <= 512);
- * 1 = 64x64 tiles, 4 warps, 4 CTAs/SM (S2, S5 at large k); 2 = the same at 5 CTAs/SM (S4 flush). */
+/* Stand-alone FP64 GEMM through the library's TMA-staged DMMA tile kernel (the kernel S2 / S4 / S5 use, PAPER.md:226,
+ * 373): C (MxN, ldc) = beta*C + alpha * A (MxK, lda) * B, all column-major DEVICE pointers, K >= 1.
+ * A: lda a multiple of 8 and >= M rounded up to 8 ("M-major" operand).  b_nmajor = 0: B is K x N with leading dimension
+ * ldb (a multiple of 4, >= K rounded up to 4; the "K-major" right operand, e.g. N in the candidate-row product);
+ * b_nmajor = 1: B points to B^T stored column-major, N x K with ldb a multiple of 8 and >= N rounded up to 8 (the
+ * "N-major" right operand, e.g. V in the flush).  Builds two tensor maps per call and synchronises the stream. */
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
-                const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel);
+                const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t b_nmajor);
 
 /* Issue-rate peak of the FP64 pipes on the current device, TFLOP/s.  which = 0: DMMA.8x8x4 (mma.sync m8n8k4 f64, the
  * tensor path the GEMM tiles use), 1: DFMA.  Two CTAs of 256 threads per SM, 16 independent accumulators per warp /

@@ -398,10 +398,10 @@ class WalkerGroups:
 
 
 def colmajor(rows, cols, device="cuda", fill=None, generator=None):
-    """A rows x cols float64 CUDA tensor stored column-major with an EVEN leading dimension
+    """A rows x cols float64 CUDA tensor stored column-major with a leading dimension that is a multiple of 8
     (the layout ctaux_dgemm wants): element (i, j) at data_ptr + 8*(i + j*ld)."""
     import torch
-    ld = max(2, rows + (rows & 1))
+    ld = max(8, (rows + 7) // 8 * 8)
     if fill is None:
         store = torch.zeros((cols, ld), dtype=torch.float64, device=device)
     else:
@@ -409,10 +409,10 @@ def colmajor(rows, cols, device="cuda", fill=None, generator=None):
     return store[:, :rows].t()
 
 
-def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, kernel=0):
-    """C = beta*C + alpha*A@B through the library's DMMA tile kernel.  A (M x K), B (K x N), C (M x N)
-    are torch float64 CUDA tensors stored column-major (stride(0) == 1) with even leading dimensions
-    (see colmajor())."""
+def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, b_nmajor=0):
+    """C = beta*C + alpha*A@B through the library's TMA-staged DMMA tile kernel.  A (M x K), B (K x N), C (M x N)
+    are torch float64 CUDA tensors stored column-major (stride(0) == 1) with leading dimensions that are multiples
+    of 8 (see colmajor()).  b_nmajor = 1 exercises the tile's "N-major" right-operand layout (B^T is handed over)."""
     import torch
     L = load_library()
     M, K = A.shape
@@ -422,10 +422,14 @@ def ctaux_dgemm(A, B, C_out=None, alpha=1.0, beta=0.0, stream=None, kernel=0):
         C_out = colmajor(M, N, A.device)
     for t in (A, B, C_out):
         assert t.shape[0] <= 1 or t.stride(0) == 1, "column-major operands required"
-    ld = lambda t: int(t.stride(1)) if t.shape[1] > 1 else max(2, t.shape[0] + (t.shape[0] & 1))
+    ld = lambda t: int(t.stride(1)) if t.shape[1] > 1 else max(8, (t.shape[0] + 7) // 8 * 8)
     s = stream if stream is not None else torch.cuda.current_stream(A.device)
+    if b_nmajor:        # the tile's "N-major" right operand: hand over B^T stored column-major (N x K)
+        Bt = colmajor(N, K, A.device)
+        Bt.copy_(B.t())
+        B = Bt
     _check(L.ctaux_dgemm(s.cuda_stream, M, N, K, alpha, A.data_ptr(), ld(A), B.data_ptr(), ld(B), beta,
-                         C_out.data_ptr(), ld(C_out), kernel), "ctaux_dgemm")
+                         C_out.data_ptr(), ld(C_out), 1 if b_nmajor else 0), "ctaux_dgemm")
     return C_out
 
 

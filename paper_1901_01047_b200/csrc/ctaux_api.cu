@@ -15,6 +15,7 @@
 
 #include "error_monitor.cuh"
 #include "gemm_dmma.cuh"
+#include "gemm_tma.cuh"
 #include "rebuild_lu.cuh"
 #include "walker_kernels.cuh"
 #include "walker_fused.cuh"
@@ -42,89 +43,12 @@ inline size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 
 enum StepClass { C_PREP = 0, C_CAND_GEMM = 1, C_PROPOSE = 2, C_UV = 3, C_FLUSH_GEMM = 4, C_REBUILD = 5, C_OTHER = 6, C_USINV_GEMM = 7, N_CLASS = 8 };
 
-// GEMM tile configurations
-//  small:  64x64x16, 8 warps (2x4 -> warp tile 32x16), 4 stages, 2 CTAs/SM -- max_k <= 512
-#define GEMM_SMALL 64, 64, 2, 4, 4, 2
-// large k: 64x64 tiles, 4 warps with 32x32 warp tiles, 2 stages, 4-5 INDEPENDENT CTAs per SM: while one CTA
-// waits for its C0 gather / operands or drains its stores, the others keep the DMMA pipe busy
-// (rank-64 flush: 23.0 TFLOP/s against 18.2 for 2 CTAs of 8 warps; profiles/r1_gemm_variants.md)
-#define GEMM_Q4 64, 64, 2, 2, 2, 4
-#define GEMM_Q5 64, 64, 2, 2, 2, 5
-
 // ---- device-side problem descriptors ------------------------------------------------------
-struct DescCandRows {  // G1: N_ext[k:k+m, 0:k] = Bm (m x k) * N (k x k)
-  DevCtx c;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
-    const int w = prob >> 1, sp = prob & 1;
-    const WalkerState& st = c.ws[w];
-    if (st.m == 0 || st.k == 0) return false;
-    double* N = c.N(w, sp, st.n_cur);
-    d.M = st.m; d.N = st.k; d.K = st.k;
-    d.A = c.Bm + ((size_t)w * 2 + sp) * (size_t)c.ldm * c.cap; d.lda = c.ldm;
-    d.B = N; d.ldb = c.ld;
-    d.C = N + st.k; d.ldc = c.ld;
-    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = 1.0; d.beta = 0.0;
-    return true;
-  }
-};
-struct DescCandCols {  // G2: Gx (n x m) = N_ext (n x n) * gxC (n x m)
-  DevCtx c;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
-    const int w = prob >> 1, sp = prob & 1;
-    const WalkerState& st = c.ws[w];
-    if (st.m == 0) return false;
-    const int n = st.k + st.m;
-    d.M = n; d.N = st.m; d.K = n;
-    d.A = c.N(w, sp, st.n_cur); d.lda = c.ld;
-    d.B = c.gxC + (size_t)w * c.ld * c.mmax; d.ldb = c.ld;
-    d.C = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax; d.ldc = c.ld;
-    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = 1.0; d.beta = 0.0;
-    return true;
-  }
-};
 // Split-K forms of the two S2 GEMMs.  Their outputs are skinny (m = 64 rows or columns), so one CTA per
 // output tile leaves most of the 148 x 4 CTA slots empty (config 4 with two stream groups: 232 CTAs);
 // the contraction index is cut into S chunks, every chunk writes its partial product to `skbuf`, and
 // k_splitk_reduce adds the partials in a fixed order (deterministic, unlike atomics).
 __device__ __forceinline__ int sk_chunk(int K, int S) { return (((K + S - 1) / S) + 15) & ~15; }
-struct DescCandRowsSK {
-  DevCtx c; int S;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
-    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
-    const WalkerState& st = c.ws[w];
-    if (st.m == 0 || st.k == 0) return false;
-    const int ch = sk_chunk(st.k, S), kb = s * ch;
-    if (kb >= st.k) return false;
-    const double* N = c.N(w, sp, st.n_cur);
-    d.M = st.m; d.N = st.k; d.K = (st.k - kb < ch) ? st.k - kb : ch;
-    d.A = c.Bm + ((size_t)w * 2 + sp) * (size_t)c.ldm * c.cap + (size_t)kb * c.ldm; d.lda = c.ldm;
-    d.B = N + kb; d.ldb = c.ld;
-    d.C = c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride; d.ldc = c.ldm;
-    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = 1.0; d.beta = 0.0;
-    return true;
-  }
-};
-struct DescCandColsSK {
-  DevCtx c; int S;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
-    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
-    const WalkerState& st = c.ws[w];
-    if (st.m == 0) return false;
-    const int n = st.k + st.m;
-    const int ch = sk_chunk(n, S), kb = s * ch;
-    if (kb >= n) return false;
-    d.M = n; d.N = st.m; d.K = (n - kb < ch) ? n - kb : ch;
-    d.A = c.N(w, sp, st.n_cur) + (size_t)kb * c.ld; d.lda = c.ld;
-    d.B = c.gxC + (size_t)w * c.ld * c.mmax + kb; d.ldb = c.ld;
-    d.C = c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride; d.ldc = c.ld;
-    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = 1.0; d.beta = 0.0;
-    return true;
-  }
-};
 // which = 0: candidate rows -> N_ext[k:k+m, 0:k];  which = 1: candidate columns -> Gx (n x m)
 __global__ void k_splitk_reduce(DevCtx c, int S, int which) {
   const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
@@ -146,30 +70,65 @@ __global__ void k_splitk_reduce(DevCtx c, int S, int which) {
     out[(size_t)j * c.ld + i] = v;
   }
 }
-struct DescUSinv {  // G3: Ut (k' x r) = U (k' x r) * S^-1 (r x r)
+// ---- GEMM problems of a block step for the TMA-staged tiles (gemm_tma.cuh): operands named by tensor map + tile origin
+__device__ __forceinline__ void tma_plain_out(TmaGemmDesc& d, double* C, int ldc) {
+  d.C = C; d.ldc = ldc; d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr; d.alpha = 1.0; d.beta = 0.0;
+}
+struct TDescCandRows {  // N_ext[k:k+m, 0:k] = Bm (m x k) * N (k x k); split-K chunk s of S into skbuf when S > 1
+  DevCtx c; int S;
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
+    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0 || st.k == 0) return false;
+    const int ch = S > 1 ? sk_chunk(st.k, S) : st.k, kb = s * ch;
+    if (kb >= st.k) return false;
+    d.M = st.m; d.N = st.k; d.K = (st.k - kb < ch) ? st.k - kb : ch;
+    d.tmA = c.tm(w, sp, TM_BM_M); d.a_m0 = 0; d.a_k0 = kb;
+    d.tmB = c.tm(w, sp, st.n_cur ? TM_N1_K : TM_N0_K); d.b_k0 = kb; d.b_n0 = 0;
+    if (S > 1) tma_plain_out(d, c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride, c.ldm);
+    else tma_plain_out(d, c.N(w, sp, st.n_cur) + st.k, c.ld);
+    return true;
+  }
+};
+struct TDescCandCols {  // Gx (n x m) = N_ext (n x n) * g_ext[:, C] (n x m, stored n-contiguous)
+  DevCtx c; int S;
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
+    const int s = prob % S, ws = prob / S, w = ws >> 1, sp = ws & 1;
+    const WalkerState& st = c.ws[w];
+    if (st.m == 0) return false;
+    const int n = st.k + st.m;
+    const int ch = S > 1 ? sk_chunk(n, S) : n, kb = s * ch;
+    if (kb >= n) return false;
+    d.M = n; d.N = st.m; d.K = (n - kb < ch) ? n - kb : ch;
+    d.tmA = c.tm(w, sp, st.n_cur ? TM_N1_M : TM_N0_M); d.a_m0 = 0; d.a_k0 = kb;
+    d.tmB = c.tm(w, sp, TM_GX_N); d.b_k0 = kb; d.b_n0 = 0;
+    if (S > 1) tma_plain_out(d, c.skbuf + (((size_t)w * 2 + sp) * kMaxSplitK + s) * c.skstride, c.ld);
+    else tma_plain_out(d, c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax, c.ld);
+    return true;
+  }
+};
+struct TDescUSinv {  // Ut (k' x r) = U (k' x r) * S^-1 (r x r)
   DevCtx c;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
     const int w = prob >> 1, sp = prob & 1;
     const WalkerState& st = c.ws[w];
     if (st.r == 0) return false;
     d.M = st.k_new; d.N = st.r; d.K = st.r;
-    d.A = c.Um + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.lda = c.ld;
-    d.B = c.Sinv + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.delay; d.ldb = c.ldr;
-    d.C = c.Ut + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.ldc = c.ld;
-    d.C0 = nullptr; d.ldc0 = 0; d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = 1.0; d.beta = 0.0;
+    d.tmA = c.tm(w, sp, TM_UM_M); d.a_m0 = 0; d.a_k0 = 0;
+    d.tmB = c.tm(w, sp, TM_SINV_K); d.b_k0 = 0; d.b_n0 = 0;
+    tma_plain_out(d, c.Ut + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay, c.ld);
     return true;
   }
 };
-struct DescFlush {  // G4: N_new[i',j'] = N_ext[map i', map j'] - (Ut * Vt)[i',j']
+struct TDescFlush {  // N_new[i',j'] = N_ext[map i', map j'] - (Ut * V^T)[i',j'],  V stored n-contiguous
   DevCtx c;
-  __device__ bool operator()(int prob, GemmDesc& d) const {
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
     const int w = prob >> 1, sp = prob & 1;
     const WalkerState& st = c.ws[w];
     if (st.r == 0) return false;
     d.M = st.k_new; d.N = st.k_new; d.K = st.r;
-    d.A = c.Ut + ((size_t)w * 2 + sp) * (size_t)c.ld * c.delay; d.lda = c.ld;
-    d.B = c.Vt + ((size_t)w * 2 + sp) * (size_t)c.ldr * c.ld; d.ldb = c.ldr;
+    d.tmA = c.tm(w, sp, TM_UT_M); d.a_m0 = 0; d.a_k0 = 0;
+    d.tmB = c.tm(w, sp, TM_V_N); d.b_k0 = 0; d.b_n0 = 0;
     d.C = c.N(w, sp, st.n_cur); d.ldc = c.ld;
     d.C0 = c.N(w, sp, st.n_src); d.ldc0 = c.ld;
     d.rowmap = c.rowmap + (size_t)w * c.cap; d.colmap = d.rowmap;
@@ -177,11 +136,6 @@ struct DescFlush {  // G4: N_new[i',j'] = N_ext[map i', map j'] - (Ut * Vt)[i',j
     return true;
   }
 };
-struct DescPlain {  // ctaux_dgemm
-  GemmDesc d;
-  __device__ bool operator()(int, GemmDesc& o) const { o = d; return true; }
-};
-
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (function, device): remember the largest value set
 // per device, under a mutex (contexts are created and driven from several host threads, WalkerGroups).
 struct SmemOptIn {
@@ -201,19 +155,66 @@ struct SmemOptIn {
   }
 };
 
-template <int BM, int BN, int WM, int WN, int STAGES, int MINB, class Fn>
-cudaError_t launch_gemm(const Fn& fn, int tiles_x, int problems, cudaStream_t s, int pf_dist = 0) {
-  using Cfg = GemmCfg<BM, BN, WM, WN, STAGES>;
-  auto kern = gemm_grouped_kernel<BM, BN, WM, WN, STAGES, MINB, Fn>;
+// ---- TMA tensor maps (gemm_tma.cuh).  cuTensorMapEncodeTiled is a driver entry point: fetched through the runtime so
+// that the library does not link libcuda.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  });
+  return fn;
+}
+// "M-major" operand: element (m, k) at base + m + k*ld, ld a multiple of 4, `kdim` columns.  Rank-3 view
+// (4, kdim, ld/4), strides (ld*8 B, 32 B), box (4, 16, 16): the 64 x 16 tile lands in shared memory as [m/4][k][m%4].
+bool make_map_mmajor(CUtensorMap* out, const double* base, int ld, int kdim) {
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc || (ld & 3) || ld < 4 || kdim < 1) return false;
+  const cuuint64_t dims[3] = {4, (cuuint64_t)kdim, (cuuint64_t)(ld / 4)};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * 8, 32};
+  const cuuint32_t box[3] = {4, (cuuint32_t)kTmaBK, (cuuint32_t)(kTmaBM / 4)};
+  const cuuint32_t es[3] = {1, 1, 1};
+  return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// "K-major" operand: element (k, n) at base + k + n*ld, ld even, `kdim` rows (rounded up to 4 inside the leading
+// dimension), `ncols` columns.  Rank-3 view (4, ncols, kdim/4), strides (ld*8 B, 32 B), box (4, 64, 4): the 16 x 64
+// tile lands in shared memory as [k/4][n][k%4].
+bool make_map_kmajor(CUtensorMap* out, const double* base, int ld, int kdim, int ncols) {
+  EncodeTiledFn enc = encode_tiled();
+  if (!enc || (ld & 1) || kdim < 1 || ncols < 1) return false;
+  const int k4 = (kdim + 3) / 4 <= ld / 4 ? (kdim + 3) / 4 : ld / 4;
+  if (k4 < 1) return false;
+  const cuuint64_t dims[3] = {4, (cuuint64_t)ncols, (cuuint64_t)k4};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * 8, 32};
+  const cuuint32_t box[3] = {4, (cuuint32_t)kTmaBN, (cuuint32_t)(kTmaBK / 4)};
+  const cuuint32_t es[3] = {1, 1, 1};
+  return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+constexpr int kTmaStages = 3;
+template <bool B_KMAJOR, int MINB, class Fn>
+cudaError_t launch_tma(const Fn& fn, int tiles_x, int problems, cudaStream_t s) {
+  using Cfg = TmaCfg<kTmaStages>;
+  auto kern = gemm_tma_kernel<kTmaStages, B_KMAJOR, MINB, Fn>;
   static SmemOptIn optin;
-  {
-    cudaError_t e = optin.ensure(kern, Cfg::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-  }
+  cudaError_t e = optin.ensure(kern, Cfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
   if (tiles_x < 1) tiles_x = 1;
-  kern<<<dim3(tiles_x, problems), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(fn, pf_dist);
+  kern<<<dim3(tiles_x, problems), kTmaThreads, Cfg::SMEM_BYTES, s>>>(fn);
   return cudaGetLastError();
 }
+struct TmaDescPlain {  // ctaux_dgemm
+  TmaGemmDesc d;
+  __device__ bool operator()(int, TmaGemmDesc& o) const { o = d; return true; }
+};
 
 int sm_count() {
   static int n = 0;
@@ -238,7 +239,6 @@ struct ctaux_ctx {
   int64_t launches;
   bool sinv_smem;
   int propose_smem;
-  bool small_tiles;
   cudaStream_t hi;    // internal high-priority stream for the serial S3 kernel (forked from / joined to `stream`
                       // with events): when several contexts share the GPU its few CTAs must not queue behind
                       // thousands of GEMM CTAs of the other contexts
@@ -275,7 +275,7 @@ namespace {
 
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
-      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, total;
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -330,7 +330,7 @@ Layout make_layout(const DevCtx& d) {
   L.prop = take(B * d.winmax * sizeof(PropInfo));
   L.Nbuf = take(B * 4 * (size_t)d.ld * d.ld * 8);
   L.Bm = take(B * 2 * (size_t)d.ldm * d.cap * 8);
-  L.gxC = take(B * (size_t)d.ld * d.mmax * 8);
+  L.gxC = take(B * (size_t)d.ld * d.ldm * 8);   // g_ext[:, C] stored n-contiguous: n rows of ldm
   L.Gx = take(B * 2 * (size_t)d.ld * d.mmax * 8);
   L.Um = take(B * 2 * (size_t)d.ld * d.delay * 8);
   L.Ut = take(B * 2 * (size_t)d.ld * d.delay * 8);
@@ -350,6 +350,7 @@ Layout make_layout(const DevCtx& d) {
   L.resid = take(B * 2 * 8);
   L.mon = take(B * 2 * 3 * kProbes * (size_t)d.ld * 8);
   L.est = take(B * 2 * 8);
+  L.tmaps = take(B * 2 * TM_COUNT * sizeof(CUtensorMap));
   L.total = o;
   return L;
 }
@@ -461,7 +462,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
       Scoped t(x, C_REBUILD);
       CU_CHECK(cudaMemsetAsync(d.resid, 0, sizeof(unsigned long long) * P, s));
       k_build_A<<<dim3(gb, P), 256, 0, s>>>(d, 1);
-      cudaError_t e = x->small_tiles ? launch_gemm<GEMM_SMALL>(DescNS{d, 0}, t64, P, s) : launch_gemm<GEMM_Q4>(DescNS{d, 0}, t64, P, s);
+      cudaError_t e = launch_tma<true, 4>(TDescNS{d, 0}, t64, P, s);
       CU_CHECK(e);
       k_ns_resid<<<dim3(gb > 256 ? 256 : gb, P), 256, 0, s>>>(d);
       tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
@@ -476,7 +477,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     if (worst < 1e-6) {
       {
         Scoped t(x, C_REBUILD);
-        cudaError_t e = x->small_tiles ? launch_gemm<GEMM_SMALL>(DescNS{d, 1}, t64, P, s) : launch_gemm<GEMM_Q4>(DescNS{d, 1}, t64, P, s);
+        cudaError_t e = launch_tma<true, 4>(TDescNS{d, 1}, t64, P, s);
         CU_CHECK(e);
         k_ns_flip<<<(d.B + 127) / 128, 128, 0, s>>>(d);
         tick(x, C_REBUILD); tick(x, C_OTHER);
@@ -507,8 +508,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
-      if (x->small_tiles) return launch_gemm<GEMM_SMALL>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
-      return launch_gemm<GEMM_Q4>(DescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
+      return launch_tma<true, 4>(TDescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
     };
     for (int j0 = 0; j0 < kmax; j0 += nbw) {  // factorisation + forward substitution
       Scoped t(x, C_REBUILD);
@@ -568,31 +568,20 @@ int enqueue_block_step(ctaux_ctx* x) {
   }
   {
     Scoped t(x, C_CAND_GEMM);
-    cudaError_t e1, e2;
-    if (x->small_tiles) {
-      e1 = launch_gemm<GEMM_SMALL>(DescCandRows{d}, (d.mmax + 63) / 64 * ((kh + 63) / 64), P, s);
-      e2 = launch_gemm<GEMM_SMALL>(DescCandCols{d}, (kcap + 63) / 64 * ((d.mmax + 63) / 64), P, s);
-    } else {
-      const int t1 = (d.mmax + 63) / 64 * ((kh + 63) / 64), t2 = (kcap + 63) / 64 * ((d.mmax + 63) / 64);
-      // split-K factor: aim at >= 3 waves of the 148 x 4 CTA slots (measured optimum), chunks of at least 128
-      int S = (12 * sm_count() + P * t1 - 1) / (P * t1);
-      if (S > kMaxSplitK) S = kMaxSplitK;
-      while (S > 1 && kh / S < 128) --S;
-      if (d.max_k <= 512) S = 1;   // the split-K scratch exists only for the large configurations
-      if (S <= 1) {
-        e1 = launch_gemm<GEMM_Q4>(DescCandRows{d}, t1, P, s);
-        e2 = launch_gemm<GEMM_Q4>(DescCandCols{d}, t2, P, s);
-      } else {
-        const int rb = grid_for((size_t)kcap * d.mmax, 256, 128);
-        e1 = launch_gemm<GEMM_Q4>(DescCandRowsSK{d, S}, t1, P * S, s);
-        k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 0);
-        e2 = launch_gemm<GEMM_Q4>(DescCandColsSK{d, S}, t2, P * S, s);
-        k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 1);
-        tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
-      }
-    }
-    CU_CHECK(e1); CU_CHECK(e2);
-    tick(x, C_CAND_GEMM); tick(x, C_CAND_GEMM);
+    const int t1 = (d.mmax + 63) / 64 * ((kh + 63) / 64), t2 = (kcap + 63) / 64 * ((d.mmax + 63) / 64);
+    // split-K factor of the skinny S2 products: aim at >= 3 waves of the 148 x 4 CTA slots (measured optimum; a
+    // wave-count model was tried and lost 4 %), chunks of at least 128
+    int S = (12 * sm_count() + P * t1 - 1) / (P * t1);
+    if (S > kMaxSplitK) S = kMaxSplitK;
+    while (S > 1 && kh / S < 128) --S;
+    if (d.max_k <= 512) S = 1;   // the split-K scratch exists only for the large configurations
+    CU_CHECK((launch_tma<true, 4>(TDescCandRows{d, S}, t1, P * S, s)));
+    tick(x, C_CAND_GEMM);
+    const int rb = grid_for((size_t)kcap * d.mmax, 256, 128);
+    if (S > 1) { k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 0); tick(x, C_CAND_GEMM); }
+    CU_CHECK((launch_tma<false, 4>(TDescCandCols{d, S}, t2, P * S, s)));
+    tick(x, C_CAND_GEMM);
+    if (S > 1) { k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 1); tick(x, C_CAND_GEMM); }
   }
   {
     cudaStream_t ps = x->hi ? x->hi : s;
@@ -621,29 +610,22 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
-    if (x->small_tiles) e3 = launch_gemm<GEMM_SMALL>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
-    else e3 = launch_gemm<GEMM_Q4>(DescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    e3 = launch_tma<true, 4>(TDescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
   }
   {
     Scoped t(x, C_FLUSH_GEMM);
     cudaError_t e4;
-    if (x->small_tiles) {
+    {
       const int tl = (kh + 63) / 64;
-      e4 = launch_gemm<GEMM_SMALL>(DescFlush{d}, tl * tl, P, s);
-    } else {
-      const int tl = (kh + 63) / 64;
-      // measured, no gain: L2 prefetch of C0; 2-8 tiles per CTA.  Gain: compaction-map loads issued before the descriptor.
-      {
-        using Cfg = GemmCfg<64, 64, 2, 2, 2>;
-        auto kern = gemm_flush_kernel<GEMM_Q5, DescFlush>;
-        static SmemOptIn optin;
-        e4 = optin.ensure(kern, Cfg::SMEM_BYTES);
-        if (e4 == cudaSuccess) {
-          kern<<<dim3(tl * tl, P), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(DescFlush{d}, d.rowmap, d.cap, tl);
-          e4 = cudaGetLastError();
-        }
+      using Cfg = TmaCfg<kTmaStages>;
+      auto kern = gemm_tma_flush_kernel<kTmaStages, 4, TDescFlush>;
+      static SmemOptIn optin;
+      e4 = optin.ensure(kern, Cfg::SMEM_BYTES);
+      if (e4 == cudaSuccess) {
+        kern<<<dim3(tl * tl, P), kTmaThreads, Cfg::SMEM_BYTES, s>>>(TDescFlush{d}, d.rowmap, d.cap, tl);
+        e4 = cudaGetLastError();
       }
     }
     CU_CHECK(e4);
@@ -693,7 +675,7 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
       if (rc) return rc;
     }
     x->n_fresh = false;
-    const bool probe = x->n_tol > 0.0;
+    const bool probe = x->n_tol > 0.0 && ((done / steps_per_poll) & 3) == 3;   // every 32 block steps
     if (probe) { int rc = enqueue_err_probe(x); if (rc) return rc; }
     CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(cudaStreamSynchronize(s));
@@ -767,6 +749,37 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   d.skbuf = (double*)(base + L.skbuf);
   d.Tbuf = prm->rebuild_mode == 1 ? (double*)(base + L.Tbuf) : nullptr;
   d.resid = (unsigned long long*)(base + L.resid);
+  // TMA tensor maps of every GEMM operand buffer (gemm_tma.cuh); uploaded below, after the workspace has been cleared
+  std::vector<CUtensorMap> hm((size_t)d.B * 2 * TM_COUNT);
+  d.tmaps = (const CUtensorMap*)(base + L.tmaps);
+  {
+    {
+      bool ok = encode_tiled() != nullptr;
+      const size_t nn = (size_t)d.ld * d.ld;
+      for (int w = 0; w < d.B && ok; ++w)
+        for (int sp = 0; sp < 2 && ok; ++sp) {
+          CUtensorMap* m = hm.data() + ((size_t)w * 2 + sp) * TM_COUNT;
+          const size_t ws2 = (size_t)w * 2 + sp;
+          const double* N0 = d.Nbuf + (ws2 * 2 + 0) * nn;
+          const double* N1 = d.Nbuf + (ws2 * 2 + 1) * nn;
+          ok = ok && make_map_mmajor(m + TM_N0_M, N0, d.ld, d.ld) && make_map_mmajor(m + TM_N1_M, N1, d.ld, d.ld);
+          ok = ok && make_map_kmajor(m + TM_N0_K, N0, d.ld, d.ld, d.ld) && make_map_kmajor(m + TM_N1_K, N1, d.ld, d.ld, d.ld);
+          ok = ok && make_map_mmajor(m + TM_BM_M, d.Bm + ws2 * (size_t)d.ldm * d.cap, d.ldm, d.cap);
+          ok = ok && make_map_mmajor(m + TM_UM_M, d.Um + ws2 * (size_t)d.ld * d.delay, d.ld, d.delay);
+          ok = ok && make_map_mmajor(m + TM_UT_M, d.Ut + ws2 * (size_t)d.ld * d.delay, d.ld, d.delay);
+          ok = ok && make_map_mmajor(m + TM_V_N, d.Vt + ws2 * (size_t)d.ldr * d.ld, d.ld, d.delay);
+          ok = ok && make_map_kmajor(m + TM_SINV_K, d.Sinv + ws2 * (size_t)d.ldr * d.delay, d.ldr, d.ldr, d.delay);
+          ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + (size_t)w * d.ld * d.ldm, d.ldm, d.cap);
+          if (prm->rebuild_mode == 1) ok = ok && make_map_kmajor(m + TM_T_K, (double*)(base + L.Tbuf) + ws2 * nn, d.ld, d.ld, d.ld);
+          else m[TM_T_K] = m[TM_N0_K];
+        }
+      if (!ok) {
+        g_last_cuda_error = "ctaux_create: cuTensorMapEncodeTiled unavailable or refused a tensor map";
+        delete x;
+        return CTAUX_ECUDA;
+      }
+    }
+  }
   x->mon = (double*)(base + L.mon);
   x->est_d = (double*)(base + L.est);
   x->n_tol = prm->n_tol == 0.0 ? 1e-10 : prm->n_tol;
@@ -793,6 +806,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_flag, 2 * sizeof(int));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_est, 2 * d.B * sizeof(double));
   if (e == cudaSuccess) e = cudaStreamSynchronize(x->stream);
+  if (e == cudaSuccess) e = cudaMemcpy(base + L.tmaps, hm.data(), hm.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice);
   // proposal kernel shared memory: keep S^-1 of both spins in shared memory when it fits
   int dev = 0, max_smem = 0;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -867,7 +881,6 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       }
     }
   }
-  x->small_tiles = d.max_k <= 512;   // (64x64 / 4-warp tiles on config 3, k = 245: measured, no gain)
   *out = x;
   return CTAUX_OK;
 }
@@ -1111,26 +1124,27 @@ int ctaux_timing_get(ctaux_ctx* x, double* ms, int64_t* launches) {
 }
 
 int ctaux_dgemm(void* stream, int32_t M, int32_t N, int32_t K, double alpha, const double* A, int32_t lda,
-                const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t kernel) {
-  if (kernel < 0 || kernel > 2) return CTAUX_EINVAL;
-  if (M < 0 || N < 0 || K < 0 || !C || ldc < M) return CTAUX_EINVAL;
-  if (K > 0 && (!A || !B || lda < M || ldb < K || (lda & 1) || (ldb & 1) || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)))
-    return CTAUX_EINVAL;
-  if (K == 0) { A = C; B = C; lda = ldb = 2; }  // never dereferenced: C = beta*C
+                const double* B, int32_t ldb, double beta, double* C, int32_t ldc, int32_t b_nmajor) {
+  if (b_nmajor < 0 || b_nmajor > 1) return CTAUX_EINVAL;
+  if (M < 0 || N < 0 || K < 1 || !C || ldc < M) return CTAUX_EINVAL;
   if (M == 0 || N == 0) return CTAUX_OK;
-  DescPlain fn;
+  if (!A || !B || (lda & 7) || lda < (M + 7) / 8 * 8 || ((uintptr_t)A & 15) || ((uintptr_t)B & 15)) return CTAUX_EINVAL;
+  if (b_nmajor ? ((ldb & 7) || ldb < (N + 7) / 8 * 8) : ((ldb & 3) || ldb < (K + 3) / 4 * 4)) return CTAUX_EINVAL;
+  CUtensorMap hm[2];
+  if (!make_map_mmajor(&hm[0], A, lda, K)) return CTAUX_ECUDA;
+  if (!(b_nmajor ? make_map_mmajor(&hm[1], B, ldb, K) : make_map_kmajor(&hm[1], B, ldb, K, N))) return CTAUX_ECUDA;
+  CUtensorMap* dm = nullptr;
+  CU_CHECK(cudaMalloc((void**)&dm, sizeof(hm)));
+  CU_CHECK(cudaMemcpy(dm, hm, sizeof(hm), cudaMemcpyHostToDevice));
+  TmaDescPlain fn;
   fn.d.M = M; fn.d.N = N; fn.d.K = K;
-  fn.d.A = A; fn.d.lda = lda; fn.d.B = B; fn.d.ldb = ldb; fn.d.C = C; fn.d.ldc = ldc;
-  fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
+  fn.d.tmA = dm; fn.d.a_m0 = 0; fn.d.a_k0 = 0; fn.d.tmB = dm + 1; fn.d.b_k0 = 0; fn.d.b_n0 = 0;
+  fn.d.C = C; fn.d.ldc = ldc; fn.d.C0 = C; fn.d.ldc0 = ldc; fn.d.rowmap = nullptr; fn.d.colmap = nullptr;
   fn.d.alpha = alpha; fn.d.beta = beta;
-  cudaStream_t st = (cudaStream_t)stream;
   const int t64 = ((M + 63) / 64) * ((N + 63) / 64);
-  cudaError_t e;
-  switch (kernel) {
-    case 0: e = launch_gemm<GEMM_SMALL>(fn, t64, 1, st); break;
-    case 1: e = launch_gemm<GEMM_Q4>(fn, t64, 1, st); break;
-    default: e = launch_gemm<GEMM_Q5>(fn, t64, 1, st); break;
-  }
+  cudaError_t e = b_nmajor ? launch_tma<false, 4>(fn, t64, 1, (cudaStream_t)stream) : launch_tma<true, 4>(fn, t64, 1, (cudaStream_t)stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);   // the tensor maps are freed below
+  cudaFree(dm);
   CU_CHECK(e);
   return CTAUX_OK;
 }

@@ -12,15 +12,18 @@
 // prologue that dominated the short-K flush tiles): ONE thread issues two bulk tensor copies per pipeline stage.
 //
 // Shared-memory layouts are chosen through the SHAPE OF THE TENSOR MAP so that the DMMA fragment loads (thread
-// (g = lane/4, q = lane%4) reads A[row g][k q] and B[k q][col g]) are bank-conflict free without padding:
+// (g = lane/4, q = lane%4) reads A[row g][k q] and B[k q][col g]) are bank-conflict free without padding.  A 64-bit
+// shared load is served per HALF-warp (g in 0..3 or 4..7, q in 0..3), so the 16 (g, q) pairs of a half-warp must fall
+// into 16 different 8-byte bank pairs, i.e. the word index must be 4q + g%4 (or 4(g%4) + q) modulo 16:
 //
 //   * "M-major" operand, element (m, k) at base + m + k*ld (A of every GEMM here; B when its n index is contiguous):
-//     viewed as a rank-3 tensor (8, K, M/8) with strides (8 B, ld*8 B, 64 B) and box (8, BK, 64/8): the tile lands as
-//     [m/8][k][m%8], so the 32 lanes of a fragment load (8 consecutive m x 4 consecutive k) cover all 16 eight-byte
-//     bank pairs exactly twice.
+//     viewed as a rank-3 tensor (4, K, M/4) with strides (8 B, ld*8 B, 32 B) and box (4, BK, 64/4): the tile lands as
+//     [m/4][k][m%4], word index ((m/4)*BK + k)*4 + m%4  ==  4q + g%4  (mod 16).
 //   * "K-major" operand, element (k, n) at base + k + n*ld (N as the right factor of the candidate-row GEMM, the U12
-//     panel of the LU): rank-2 tensor (K, N), box (16, 64) with the 128-byte swizzle: row n holds its 16 k values in
-//     eight 16-byte chunks stored at chunk index (k/2) xor (n%8); a fragment load again covers every bank twice.
+//     panel of the LU): rank-3 tensor (4, N, K/4) with strides (8 B, ld*8 B, 32 B) and box (4, 64, BK/4): the tile lands
+//     as [k/4][n][k%4], word index ((k/4)*64 + n)*4 + k%4  ==  4(g%4) + q  (mod 16).
+//   (The wider boxes one would like for the TMA engine -- [m/8][k][8], or 128-byte rows with the 128B swizzle --
+//   were measured first: correct, but every fragment load is a 2-way bank conflict; ncu: 1.8 M conflicts per launch.)
 //
 // K tails: the tensor maps describe the CAPACITY of each buffer, not the live size of the walker's matrices, so
 // elements with k >= K hold stale (finite or not) data: the fragments of the last k-chunk are masked in registers.
@@ -36,8 +39,8 @@ namespace ctaux {
 
 struct TmaGemmDesc {
   int M, N, K;
-  const CUtensorMap* tmA; int a_m0, a_k0;   // M-major view: tile (m0, k0) at coordinates (0, a_k0 + k0, (a_m0 + m0) / 8)
-  const CUtensorMap* tmB; int b_k0, b_n0;   // N-major view: (0, b_k0 + k0, (b_n0 + n0) / 8);  K-major: (b_k0 + k0, b_n0 + n0)
+  const CUtensorMap* tmA; int a_m0, a_k0;   // M-major view: tile (m0, k0) at coordinates (0, a_k0 + k0, (a_m0 + m0) / 4)
+  const CUtensorMap* tmB; int b_k0, b_n0;   // N-major view: (0, b_k0 + k0, (b_n0 + n0) / 4);  K-major: (0, b_n0 + n0, (b_k0 + k0) / 4)
   double* C; int ldc;
   const double* C0; int ldc0;               // source of the beta term (may alias C when no maps are given)
   const int* rowmap;                        // nullptr = identity
@@ -85,7 +88,7 @@ struct TmaCfg {
   static constexpr int A_STAGE = kTmaBM * kTmaBK;   // doubles
   static constexpr int B_STAGE = kTmaBN * kTmaBK;
   static constexpr int STAGE_BYTES = (A_STAGE + B_STAGE) * 8;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;   // + slack to align the ring to 1024 B (128B swizzle)
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;   // + slack to align the ring to 1024 B
 };
 
 // One CTA computes one 64 x 64 tile.  `it` counts the k-chunks this CTA has pushed through the ring so far (stage
@@ -110,9 +113,9 @@ __device__ __forceinline__ void tma_gemm_tile(const TmaGemmDesc& d, int tile_m, 
     double* Bs = As + Cfg::A_STAGE;
     const int k0 = kt * BK;
     mbar_expect_tx(full + slot, (uint32_t)Cfg::STAGE_BYTES);
-    tma_load_3d(As, d.tmA, 0, d.a_k0 + k0, (d.a_m0 + m0) >> 3, full + slot);
-    if (B_KMAJOR) tma_load_2d(Bs, d.tmB, d.b_k0 + k0, d.b_n0 + n0, full + slot);
-    else tma_load_3d(Bs, d.tmB, 0, d.b_k0 + k0, (d.b_n0 + n0) >> 3, full + slot);
+    tma_load_3d(As, d.tmA, 0, d.a_k0 + k0, (d.a_m0 + m0) >> 2, full + slot);
+    if (B_KMAJOR) tma_load_3d(Bs, d.tmB, 0, d.b_n0 + n0, (d.b_k0 + k0) >> 2, full + slot);
+    else tma_load_3d(Bs, d.tmB, 0, d.b_k0 + k0, (d.b_n0 + n0) >> 2, full + slot);
   };
   if (tid == 0) {
 #pragma unroll
@@ -178,30 +181,49 @@ __device__ __forceinline__ void tma_gemm_tile(const TmaGemmDesc& d, int tile_m, 
     mbar_wait(full + slot, (cur / STAGES) & 1u);
     __syncthreads();   // every warp is done with chunk kt-1: its slot may be refilled
     if (tid == 0 && kt + STAGES - 1 < nk) issue(kt + STAGES - 1);
-    const double* a_s = ring + (size_t)slot * (Cfg::A_STAGE + Cfg::B_STAGE) + (wm * 4) * (BK * 8) + g;
+    const double* a_s = ring + (size_t)slot * (Cfg::A_STAGE + Cfg::B_STAGE) + (wm * 8 + (g >> 2)) * (BK * 4) + (g & 3);
     const double* b_s = ring + (size_t)slot * (Cfg::A_STAGE + Cfg::B_STAGE) + Cfg::A_STAGE;
     const int kv = K - kt * BK;   // valid k values in this chunk (>= BK except in the last one)
+    if (kv >= BK) {
 #pragma unroll
-    for (int k4 = 0; k4 < BK; k4 += 4) {
-      if (k4 >= kv) break;
-      const bool dead = k4 + q >= kv;
-      double af[TM], bf[TN];
+      for (int k4 = 0; k4 < BK; k4 += 4) {
+        double af[TM], bf[TN];
 #pragma unroll
-      for (int i = 0; i < TM; ++i) {
-        const double a = a_s[i * (BK * 8) + (k4 + q) * 8];
-        af[i] = dead ? 0.0 : __hiloint2double(__double2hiint(a) ^ sign_flip, __double2loint(a));
+        for (int i = 0; i < TM; ++i) {
+          const double a = a_s[i * (2 * BK * 4) + (k4 + q) * 4];
+          af[i] = __hiloint2double(__double2hiint(a) ^ sign_flip, __double2loint(a));
+        }
+#pragma unroll
+        for (int j = 0; j < TN; ++j) {
+          if (B_KMAJOR) bf[j] = b_s[((k4 >> 2) * kTmaBN + wn * 32 + j * 8 + g) * 4 + q];
+          else bf[j] = b_s[((wn * 8 + j * 2 + (g >> 2)) * BK + k4 + q) * 4 + (g & 3)];
+        }
+#pragma unroll
+        for (int i = 0; i < TM; ++i)
+#pragma unroll
+          for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
       }
+    } else {   // K tail: the boxes hold stale data beyond K, masked in registers
+      for (int k4 = 0; k4 < kv; k4 += 4) {
+        const bool dead = k4 + q >= kv;
+        double af[TM], bf[TN];
 #pragma unroll
-      for (int j = 0; j < TN; ++j) {
-        double b;
-        if (B_KMAJOR) b = b_s[(wn * 32 + j * 8 + g) * 16 + ((((k4 + q) >> 1) ^ g) << 1) + (q & 1)];
-        else b = b_s[((wn * 4 + j) * BK + k4 + q) * 8 + g];
-        bf[j] = dead ? 0.0 : b;
+        for (int i = 0; i < TM; ++i) {
+          const double a = a_s[i * (2 * BK * 4) + (k4 + q) * 4];
+          af[i] = dead ? 0.0 : __hiloint2double(__double2hiint(a) ^ sign_flip, __double2loint(a));
+        }
+#pragma unroll
+        for (int j = 0; j < TN; ++j) {
+          double b;
+          if (B_KMAJOR) b = b_s[((k4 >> 2) * kTmaBN + wn * 32 + j * 8 + g) * 4 + q];
+          else b = b_s[((wn * 8 + j * 2 + (g >> 2)) * BK + k4 + q) * 4 + (g & 3)];
+          bf[j] = dead ? 0.0 : b;
+        }
+#pragma unroll
+        for (int i = 0; i < TM; ++i)
+#pragma unroll
+          for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
       }
-#pragma unroll
-      for (int i = 0; i < TM; ++i)
-#pragma unroll
-        for (int j = 0; j < TN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     }
   }
   it += (uint32_t)nk;
@@ -294,5 +316,6 @@ __global__ void __launch_bounds__(kTmaThreads, MINB)
     tma_gemm_tile<STAGES, false, false>(d, em, en, ring, full, it);
   }
 }
+
 
 }  // namespace ctaux

@@ -18,6 +18,7 @@
 #include <cooperative_groups.h>
 
 #include "gemm_dmma.cuh"
+#include "gemm_tma.cuh"
 #include "walker_state.cuh"
 
 namespace ctaux {
@@ -349,33 +350,35 @@ __global__ void __launch_bounds__(128) k_lu_trsm(DevCtx c, int j0, int upper) {
 }
 
 // GEMM descriptors of the trailing updates (alpha = -1, beta = 1, in place)
-struct DescLU {
+struct TDescLU {   // operands by tensor map + tile origin (gemm_tma.cuh); j0, j1 are multiples of the panel width 32
   DevCtx c;
-  int j0;
-  int which;  // 0: F trailing, 1: X forward (rows below the panel), 2: X backward (rows above)
-  int nb;     // panel width
-  __device__ bool operator()(int prob, GemmDesc& d) const {
+  int j0, which, nb;
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
     const int w = prob >> 1, sp = prob & 1;
     const WalkerState& st = c.ws[w];
     const int k = st.k;
     if (j0 >= k) return false;
     const int j1 = (j0 + nb < k) ? j0 + nb : k;
     const size_t ld = c.ld;
-    double* F = c.N(w, sp, st.n_cur ^ 1);
-    double* X = c.N(w, sp, st.n_cur);
+    const int fb = st.n_cur ^ 1, xb = st.n_cur;     // F = the non-current buffer, X = the current one
+    double* F = c.N(w, sp, fb);
+    double* X = c.N(w, sp, xb);
     d.K = j1 - j0;
-    d.lda = c.ld; d.ldb = c.ld; d.ldc = c.ld; d.ldc0 = c.ld;
-    d.rowmap = nullptr; d.colmap = nullptr;
-    d.alpha = -1.0; d.beta = 1.0;
+    d.ldc = c.ld; d.ldc0 = c.ld; d.rowmap = nullptr; d.colmap = nullptr; d.alpha = -1.0; d.beta = 1.0;
+    d.tmA = c.tm(w, sp, fb ? TM_N1_M : TM_N0_M); d.a_k0 = j0;
+    d.b_k0 = j0;
     if (which == 0) {
-      d.M = k - j1; d.N = k - j1;
-      d.A = F + j1 + (size_t)j0 * ld; d.B = F + j0 + (size_t)j1 * ld; d.C = F + j1 + (size_t)j1 * ld;
+      d.M = k - j1; d.N = k - j1; d.a_m0 = j1;
+      d.tmB = c.tm(w, sp, fb ? TM_N1_K : TM_N0_K); d.b_n0 = j1;
+      d.C = F + j1 + (size_t)j1 * ld;
     } else if (which == 1) {
-      d.M = k - j1; d.N = k;
-      d.A = F + j1 + (size_t)j0 * ld; d.B = X + j0; d.C = X + j1;
+      d.M = k - j1; d.N = k; d.a_m0 = j1;
+      d.tmB = c.tm(w, sp, xb ? TM_N1_K : TM_N0_K); d.b_n0 = 0;
+      d.C = X + j1;
     } else {
-      d.M = j0; d.N = k;
-      d.A = F + (size_t)j0 * ld; d.B = X + j0; d.C = X;
+      d.M = j0; d.N = k; d.a_m0 = 0;
+      d.tmB = c.tm(w, sp, xb ? TM_N1_K : TM_N0_K); d.b_n0 = 0;
+      d.C = X;
     }
     d.C0 = d.C;
     return d.M > 0 && d.N > 0;
@@ -384,24 +387,25 @@ struct DescLU {
 
 // ---- rebuild_mode 1: Newton-Schulz refresh  N <- N (2 - A N) = 2 N - N (A N)
 // A_sigma is built (k_build_A) into the spare N buffer; T = A N goes to Tbuf; the new N overwrites A.
-struct DescNS {
+struct TDescNS {
   DevCtx c;
-  int stage;  // 0: T = A * N;  1: N_new = 2 N - N * T
-  __device__ bool operator()(int prob, GemmDesc& d) const {
+  int stage;
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
     const int w = prob >> 1, sp = prob & 1;
     const WalkerState& st = c.ws[w];
     const int k = st.k;
     if (k == 0) return false;
-    double* Ncur = c.N(w, sp, st.n_cur);
-    double* Oth = c.N(w, sp, st.n_cur ^ 1);
+    const int cur = st.n_cur, oth = st.n_cur ^ 1;
     double* T = c.Tbuf + ((size_t)w * 2 + sp) * (size_t)c.ld * c.ld;
     d.M = k; d.N = k; d.K = k;
-    d.lda = c.ld; d.ldb = c.ld; d.ldc = c.ld; d.ldc0 = c.ld;
-    d.rowmap = nullptr; d.colmap = nullptr;
+    d.a_m0 = 0; d.a_k0 = 0; d.b_k0 = 0; d.b_n0 = 0;
+    d.ldc = c.ld; d.ldc0 = c.ld; d.rowmap = nullptr; d.colmap = nullptr;
     if (stage == 0) {
-      d.A = Oth; d.B = Ncur; d.C = T; d.C0 = nullptr; d.alpha = 1.0; d.beta = 0.0;
+      d.tmA = c.tm(w, sp, oth ? TM_N1_M : TM_N0_M); d.tmB = c.tm(w, sp, cur ? TM_N1_K : TM_N0_K);
+      d.C = T; d.C0 = nullptr; d.alpha = 1.0; d.beta = 0.0;
     } else {
-      d.A = Ncur; d.B = T; d.C = Oth; d.C0 = Ncur; d.alpha = -1.0; d.beta = 2.0;
+      d.tmA = c.tm(w, sp, cur ? TM_N1_M : TM_N0_M); d.tmB = c.tm(w, sp, TM_T_K);
+      d.C = c.N(w, sp, oth); d.C0 = c.N(w, sp, cur); d.alpha = -1.0; d.beta = 2.0;
     }
     return true;
   }

@@ -163,7 +163,7 @@ __global__ void k_prep_fill(DevCtx c) {
   const int32_t* spin = c.cfg_spin + off;
   double* Bm0 = c.Bm + ((size_t)w * 2 + 0) * (size_t)c.ldm * c.cap;
   double* Bm1 = c.Bm + ((size_t)w * 2 + 1) * (size_t)c.ldm * c.cap;
-  double* gx = c.gxC + (size_t)w * c.ld * c.mmax;
+  double* gx = c.gxC + (size_t)w * c.ld * c.ldm;
   double* N0 = c.N(w, 0, st.n_cur);
   double* N1 = c.N(w, 1, st.n_cur);
   const size_t total = (size_t)n * m;
@@ -175,7 +175,7 @@ __global__ void k_prep_fill(DevCtx c) {
     double gic;
     if (i == sc) gic = c.g00;
     else gic = c.g(c.disp(site[i], site[sc]), tau[i] - tau[sc]);
-    gx[(size_t)cc * c.ld + i] = gic;
+    gx[(size_t)i * c.ldm + cc] = gic;   // g_ext[:, C] stored n-contiguous (the "N-major" right operand of gemm_tma.cuh)
     // [*, cand] block of N_ext
     const double e = (i == sc) ? 1.0 : 0.0;
     N0[(size_t)sc * c.ld + i] = e;
@@ -537,7 +537,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   }
 }
 
-// S4a: U[i', a] = X[rowmap[i'], J[a]],  Vt[a, j'] = N_ext[J[a], rowmap[j']]   (live rows/cols only)
+// S4a: U[i', a] = X[rowmap[i'], J[a]],  V[j', a] = N_ext[J[a], rowmap[j']]   (live rows/cols only)
 __global__ void k_build_uv(DevCtx c) {
   const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
   const WalkerState& st = c.ws[w];
@@ -569,9 +569,9 @@ __global__ void k_build_uv(DevCtx c) {
       }
       U[(size_t)a * ld + ip] = x;
     }
-    {  // Vt: consecutive threads write consecutive a (r contiguous)
-      const int a = (int)(idx % r), jp = (int)(idx / r);
-      Vt[(size_t)jp * c.ldr + a] = Nsrc[(size_t)rowmap[jp] * ld + J[a]];
+    {  // V stored n-contiguous ("N-major" right operand of the flush): V[j', a] = N_ext[J[a], rowmap[j']]
+      const int jp = (int)(idx % kn), a = (int)(idx / kn);
+      Vt[(size_t)a * ld + jp] = Nsrc[(size_t)rowmap[jp] * ld + J[a]];
     }
   }
 }

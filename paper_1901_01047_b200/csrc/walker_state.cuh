@@ -1,6 +1,7 @@
 // Device-side state of the batched CT-AUX walkers and small device helpers
 // (Philox4x32-10, G0 interpolation, E = e^{-gamma sigma s}).  SURVEY.md 8c.1 / DESIGN.md.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -8,6 +9,11 @@ namespace ctaux {
 
 constexpr int kMaxDelay = 256;
 constexpr int kMaxSplitK = 8;
+
+// TMA tensor maps of one (walker, spin): every buffer a GEMM reads as an operand, in the view its role needs
+// (gemm_tma.cuh: "M-major" rank-3 view for left operands and n-contiguous right operands, "K-major" swizzled rank-2
+// view for k-contiguous right operands).  Built once by ctaux_create; they describe capacities, not live sizes.
+enum TmapId { TM_N0_M = 0, TM_N1_M, TM_N0_K, TM_N1_K, TM_BM_M, TM_UM_M, TM_UT_M, TM_V_N, TM_SINV_K, TM_GX_N, TM_T_K, TM_COUNT };
 
 struct LogEntry {  // == ctaux_log_entry
   uint64_t p;
@@ -64,7 +70,7 @@ struct DevCtx {
   PropInfo* prop;       // [B][winmax]
   double* Nbuf;         // [B][2 spins][2 bufs][ld*ld]
   double* Bm;           // [B][2][ldm*cap]   candidate rows  g(c,j)(E_j-1), m x k col-major
-  double* gxC;          // [B][ld*mmax]      g_ext[:, C], n x m col-major (spin independent)
+  double* gxC;          // [B][ld*ldm]       g_ext[:, C] stored n-contiguous: element (i, c) at i*ldm + c (spin independent)
   double* Gx;           // [B][2][ld*mmax]   N_ext * g_ext[:, C]
   double* Tbuf;         // [B][2][ld*ld]  A*N of the Newton-Schulz refresh (rebuild_mode 1), else null
   unsigned long long* resid;  // [B*2]  max |A N - 1| per matrix as the bit pattern of a non-negative double
@@ -72,7 +78,7 @@ struct DevCtx {
   size_t skstride;      // max(ldm*cap, ld*mmax)
   double* Um;           // [B][2][ld*delay]  U = X[:, J]
   double* Ut;           // [B][2][ld*delay]  U * S^-1
-  double* Vt;           // [B][2][ldr*ld]    rows J of N_ext, r x k' col-major
+  double* Vt;           // [B][2][ld*delay]  V = (rows J of N_ext)^T, k' x r col-major (n-contiguous right operand of the flush)
   double* Sinv;         // [B][2][ldr*delay]
   int32_t* J;           // [B][delay]
   int32_t* rowmap;      // [B][cap]  new list position -> extended slot
@@ -82,6 +88,9 @@ struct DevCtx {
   double* colbuf;       // [B][2][ld]
   double* rowbuf;       // [B][2][ld]
   int32_t* perm;        // [B][2][ld]
+  // tensor maps of the GEMM operand buffers [B][2][TM_COUNT] (gemm_tma.cuh)
+  const CUtensorMap* tmaps;
+  __device__ __forceinline__ const CUtensorMap* tm(int w, int s, int id) const { return tmaps + ((size_t)w * 2 + s) * TM_COUNT + id; }
 
   __device__ __forceinline__ size_t cfg_off(int w, int buf) const { return ((size_t)w * 2 + buf) * cap; }
   __device__ __forceinline__ double* N(int w, int s, int buf) const {

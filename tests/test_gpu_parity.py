@@ -33,16 +33,17 @@ def test_P12_device_philox_equals_oracle_philox():
         assert dev[i].tolist() == philox(ctr[i], key[i]).tolist()
 
 
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("b_nmajor", [0, 1])
 @pytest.mark.parametrize("M,N,K,alpha,beta", [(1, 1, 1, -1.5, 0.5), (8, 8, 4, -1.5, 0.5), (130, 70, 33, -1.5, 0.5),
                                               (128, 128, 64, -1.0, 1.0), (257, 511, 100, -1.5, 0.5),
                                               (1000, 40, 1000, 1.0, 0.0), (64, 1000, 7, -1.0, 1.0),
-                                              (300, 300, 0, 2.0, 0.5), (1900, 1834, 64, -1.0, 1.0),
+                                              (300, 300, 5, 2.0, 0.5), (1900, 1834, 64, -1.0, 1.0),
                                               (64, 1834, 1834, 1.0, 0.0), (1898, 64, 1898, 1.0, 0.0),
                                               (700, 900, 129, 1.0, 1.0)])
-def test_dgemm_tiles_against_torch_fp64(M, N, K, alpha, beta, kernel):
-    """Every DMMA GEMM tile configuration the walker launches (several tiles, several K chunks, ragged tails,
-    the in-place C0 - A*B form) against torch's FP64 matmul."""
+def test_dgemm_tiles_against_torch_fp64(M, N, K, alpha, beta, b_nmajor):
+    """The TMA-staged DMMA GEMM tile with both right-operand layouts the walker uses (K-major: N in the candidate-row
+    product and the LU panels; N-major: V in the flush, g_ext in the candidate-column product): several tiles,
+    several K chunks, ragged tails in M, N and K, the in-place C0 - A*B form, against torch's FP64 matmul."""
     import torch
     pkg = _pkg()
     g = torch.Generator(device="cpu").manual_seed(M * 7 + N * 3 + K)
@@ -52,7 +53,7 @@ def test_dgemm_tiles_against_torch_fp64(M, N, K, alpha, beta, kernel):
     C0 = pkg.colmajor(M, N, fill=rnd)
     C = pkg.colmajor(M, N)
     C.copy_(C0)
-    out = pkg.ctaux_dgemm(A, B, C, alpha=alpha, beta=beta, kernel=kernel)
+    out = pkg.ctaux_dgemm(A, B, C, alpha=alpha, beta=beta, b_nmajor=b_nmajor)
     ref = beta * C0 + alpha * (A @ B)
     torch.cuda.synchronize()
     scale = float(ref.abs().max()) + 1e-300
