@@ -38,9 +38,10 @@ NOMINAL_FP64_TFLOPS = 40.0    # NVIDIA B200 datasheet, FP64 (vector = tensor) pe
 NOMINAL_BF16_TFLOPS = 2250.0
 FALLBACK_BF16_TFLOPS = 1590.0
 FALLBACK_HBM_GBS = 6650.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the flush kernel from the committed
-# `ncu --set full` capture of the same launch configuration (profiles/), bytes; None = not captured
-FLUSH_TRAFFIC_PER_WALKER = {"cfg4_6x6_b20": 97.4e6}   # profiles/r1_v3_flush_full.md (update): 779 MB / 8 walkers
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the flush kernel from the committed `ncu --set full`
+# capture of the SAME launch configuration, keyed (config, walkers per launch, delay): bytes per launch; absent = not
+# captured (the field is null then)
+FLUSH_TRAFFIC = {}
 
 
 def measured_peaks():
@@ -135,41 +136,84 @@ def dist_env():
 
 # --------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline and --impl reference): the oracle as it stands, never tuned.
-def oracle_sample(cfg, table, n_walkers, n_sweeps, mode_name="T1", first_seed=0):
-    """n_walkers chains (one per host thread), reset + n_sweeps sweeps each.  Returns
-    (accepted updates, proposals, seconds of the sweep loop, threads used)."""
-    from concurrent.futures import ThreadPoolExecutor
+ORACLE_WARMUP_SWEEPS = {"cfg1_2x2_b2": 200, "cfg2_2x2_b10": 60, "cfg3_4x4_b10": 40}
+
+
+def oracle_start_state(cfg, table):
+    """A THERMALISED start for the oracle sample, so that the CPU figure is taken at the same <k> and acceptance regime
+    as the GPU figure (T1 costs O(k^2) per proposal): the oracle-written configuration of tests/golden when there is one
+    (configs 3-5: minutes to hours of CPU to produce), else a warm-up run of the oracle itself (configs 1-2: seconds).
+    Returns (site, tau, spin, id, next_id, p, description)."""
+    import glob
     from oracle import ctaux_oracle as orc
-    mode = orc.T1 if mode_name == "T1" else orc.T0
-    walkers = []
-    for s in walker_seeds(n_walkers, first_seed):
-        w = orc.OracleWalker.from_config(cfg, table, int(s), mode)
-        w.reset(cfg["init_k"])
-        walkers.append(w)
-    threads = min(n_walkers, os.cpu_count() or 1)
-    t0 = time.perf_counter()
-    with ThreadPoolExecutor(max_workers=threads) as ex:
-        list(ex.map(lambda w: w.sweep(n_sweeps), walkers))
-    dt = time.perf_counter() - t0
-    acc = sum(w.acc_ins + w.acc_rem for w in walkers)
-    props = sum(w.p for w in walkers)
-    return acc, props, dt, threads
+    files = sorted(glob.glob(os.path.join(ROOT, "tests", "golden", f"thermalised_{cfg['name']}_seed*.txt")))
+    if files:
+        meta, rows = {}, []
+        with open(files[0]) as f:
+            for line in f:
+                if line.startswith("#"):
+                    _, key, val = line.split()
+                    meta[key] = val
+                elif line.strip():
+                    i, s, t, sp = line.split()
+                    rows.append((int(i), int(s), float.fromhex(t), int(sp)))
+        return ([r[1] for r in rows], [r[2] for r in rows], [r[3] for r in rows], [r[0] for r in rows], int(meta["next_id"]),
+                int(meta["p"]), f"oracle-thermalised start {os.path.basename(files[0])} ({meta['sweeps']} oracle sweeps, k = {len(rows)})")
+    ns = ORACLE_WARMUP_SWEEPS.get(cfg["name"], 20)
+    w = orc.OracleWalker.from_config(cfg, table, 12345, orc.T1)
+    w.reset(cfg["init_k"])
+    w.sweep(ns)
+    c = w.config()
+    return (c["site"], c["tau"], c["spin"], c["id"], w.next_id, w.p, f"start thermalised by {ns} oracle sweeps (untimed), k = {w.k}")
 
 
-# sweeps of the bounded oracle sample per config (about 10-30 s of CPU work on 8 cores)
-ORACLE_SAMPLE_SWEEPS = {"cfg1_2x2_b2": 4000, "cfg2_2x2_b10": 300, "cfg3_4x4_b10": 40, "cfg4_6x6_b20": 3,
-                        "cfg5_6x6_b40": 1}
+# proposals per chain in one bounded oracle sample (about 1-2 s of CPU per chain: T1 costs O(k^2) per proposal)
+ORACLE_SAMPLE_PROPOSALS = {"cfg1_2x2_b2": 400000, "cfg2_2x2_b10": 100000, "cfg3_4x4_b10": 10000, "cfg4_6x6_b20": 120,
+                           "cfg5_6x6_b40": 30}
+
+
+class OracleChains:
+    """One oracle chain (mode T1) per host thread, all from the common thermalised start, each with its own seed.  The
+    start-up (set_state and T1's first from-scratch inverse) is untimed; sample(n) advances every chain by n proposals
+    and returns (accepted updates, proposals, seconds)."""
+
+    def __init__(self, cfg, table, n_chains, first_seed=0):
+        from concurrent.futures import ThreadPoolExecutor
+        from oracle import ctaux_oracle as orc
+        self.start = oracle_start_state(cfg, table)
+        st = self.start
+        self.threads = min(n_chains, os.cpu_count() or 1)
+        self.ex = ThreadPoolExecutor(max_workers=self.threads)
+
+        def make(seed):
+            w = orc.OracleWalker.from_config(cfg, table, int(seed), orc.T1)
+            w.set_state(st[0], st[1], st[2], st[3], st[4], st[5])
+            w.propose(1)
+            return w
+
+        self.walkers = list(self.ex.map(make, walker_seeds(n_chains, first_seed)))
+
+    def sample(self, n):
+        a0 = sum(w.acc_ins + w.acc_rem for w in self.walkers)
+        p0 = sum(w.p for w in self.walkers)
+        t0 = time.perf_counter()
+        list(self.ex.map(lambda w: w.propose(n), self.walkers))
+        dt = time.perf_counter() - t0
+        return (sum(w.acc_ins + w.acc_rem for w in self.walkers) - a0, sum(w.p for w in self.walkers) - p0, dt)
+
+    def k_mean(self):
+        return float(np.mean([w.k for w in self.walkers]))
 
 
 def cpu_baseline(cfg, table):
     cores = os.cpu_count() or 1
-    nw = cores
-    ns = ORACLE_SAMPLE_SWEEPS.get(cfg["name"], 1)
-    acc, props, dt, threads = oracle_sample(cfg, table, nw, ns)
-    return {"value": acc / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "proposals_per_s": props / dt,
-            "sample": f"oracle T1 (rank-1 updates, from-scratch inverse every sweep), {nw} walkers x first {ns} "
-                      f"sweep(s) from reset (init_k={cfg['init_k']}), one thread per walker, {dt:.1f} s"}
+    ch = OracleChains(cfg, table, cores)
+    n = 8 * ORACLE_SAMPLE_PROPOSALS.get(cfg["name"], 100)
+    acc, props, dt = ch.sample(n)
+    return {"value": acc / dt, "unit": UNIT, "cores": ch.threads, "kind": "oracle",
+            "proposals_per_s": props / dt, "k_mean": ch.k_mean(),
+            "sample": f"oracle T1 (textbook rank-1 updates), {cores} chains (own seeds) x {n} proposals from the "
+                      f"{ch.start[6]}, one thread per chain, {dt:.1f} s; T1's once-per-sweep from-scratch inverse is not in the sample"}
 
 
 def run_reference(args):
@@ -179,24 +223,26 @@ def run_reference(args):
     cfg = get_config(args.config)
     table = table_for(cfg)
     cores = os.cpu_count() or 1
-    ns = max(1, ORACLE_SAMPLE_SWEEPS.get(cfg["name"], 1) // 4)
+    ch = OracleChains(cfg, table, cores)
+    n = ORACLE_SAMPLE_PROPOSALS.get(cfg["name"], 100)
     for _ in range(args.warmup):
-        oracle_sample(cfg, table, cores, 1 if cfg["name"] in ("cfg4_6x6_b20", "cfg5_6x6_b40") else ns)
+        ch.sample(max(1, n // 4))
     acc = props = 0
     dt = 0.0
-    threads = cores
     for step in range(args.steps):
-        a, p, t, threads = oracle_sample(cfg, table, cores, ns, first_seed=step * cores)
+        a, p, t = ch.sample(n)
         acc += a
         props += p
         dt += t
     value = acc / dt
-    sample = (f"each step = {cores} oracle T1 walkers x first {ns} sweep(s) from reset, one thread per walker "
-              f"(bounded sample of {cfg['name']}: {cfg['n_walkers']} walkers x {cfg['sweeps']} sweeps)")
+    threads = ch.threads
+    sample = (f"each step = {cores} oracle T1 chains (own seeds) x {n} proposals, continuing from the {ch.start[6]}, one thread "
+              f"per chain (bounded sample of {cfg['name']}: {cfg['n_walkers']} walkers x {cfg['sweeps']} sweeps; T1's "
+              f"once-per-sweep from-scratch inverse is not in the sample)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg["name"], "sample": sample},
+            "config": {"workload": cfg["name"], "sample": sample, "k_mean": ch.k_mean()},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "proposals_per_s": props / dt, "gpu_launches": 0}
@@ -308,8 +354,7 @@ def run_gpu(args):
         roofline = {"kernel": "gemm_flush_kernel<64,64,2,2,2,5,DescFlush> (S4 rank-r flush, DMMA m8n8k4; 64x64 tiles at 5 CTAs/SM "
                               "for k > 512, 8-warp 64x64 tiles below)", "bound": "tensor",
                     "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak if fp64_peak else None,
-                    "traffic": (FLUSH_TRAFFIC_PER_WALKER[cfg["name"]] * (B // G) if cfg["name"] in FLUSH_TRAFFIC_PER_WALKER and
-                                delay == cfg["delay"] else None),
+                    "traffic": FLUSH_TRAFFIC.get((cfg["name"], B // G, delay)),
                     "algorithmic_bytes": 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),   # read + write of N, both spins
                     "peak_source": "cuBLAS DGEMM 8192^3 measured live in this run (FP64 runs at max SM clock: no power cap)",
                     "peak_dmma_issue_rate": fp64_dmma,
@@ -339,7 +384,7 @@ def run_gpu(args):
                "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
                           "K": cfg["K"], "walkers_per_gpu": B, "stream_groups": G, "delay": delay, "sweeps_per_step": S,
                           "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh",
-                          "moves": "insert/remove/flip" if args.flips else "insert/remove", "l2": "inputs larger than L2" if B * 4 * (cfg["max_k"] ** 2) * 8 > 126e6 else
+                          "moves": "insert/remove/flip" if args.flips else "insert/remove", "l2": "inputs larger than L2" if B * 4 * (s1["k_mean"] ** 2) * 8 > 126e6 else
                           "working set fits L2 (latency-bound chain; no flush between steps)",
                           "parallelism": "replicas only"},
                "proposals_per_s": props_all / (ms_max * 1e-3), "k_mean": s1["k_mean"],
@@ -399,6 +444,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, replicas only)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":

@@ -179,7 +179,8 @@ int ctaux_get_config(ctaux_ctx* ctx, int32_t walker, int32_t* k, uint64_t* id, i
 int ctaux_get_N(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N, int32_t ld);
 
 /* Batched read-out (one synchronisation for the whole context).  k: HOST [n_walkers]; id / site / tau / spin:
- * HOST [n_walkers][max_k] (walker w at offset w*max_k, list order), any of them may be NULL. */
+ * HOST [n_walkers][max_k] (walker w at offset w*max_k, list order; entries at or beyond k[w] are unspecified), any of
+ * them may be NULL.  One gather kernel, one copy per field, one synchronisation. */
 int ctaux_get_config_all(ctaux_ctx* ctx, int32_t* k, uint64_t* id, int32_t* site, double* tau, int8_t* spin);
 
 /* Every N_sigma of the context into one HOST buffer: matrix (w, spin) is k_w x k_w, column-major with leading
@@ -190,6 +191,9 @@ int ctaux_get_N_all(ctaux_ctx* ctx, double* N);
 int ctaux_get_N_device(ctaux_ctx* ctx, int32_t walker, int32_t spin, double* N_dev, int32_t ld);
 
 int ctaux_get_stats(ctaux_ctx* ctx, int32_t walker, ctaux_stats* out);
+
+/* Counters of every walker with one synchronisation and one copy: out is a HOST array of n_walkers ctaux_stats. */
+int ctaux_get_stats_all(ctaux_ctx* ctx, ctaux_stats* out);
 
 /* Copy log entries [first, first+count) of one walker into a HOST array; entries are numbered from
  * the last reset and the log keeps the first log_capacity of them. Returns the number copied (>=0). */

@@ -43,7 +43,7 @@ class _Stats(C.Structure):
 
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
-           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats",
+           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
            "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
 TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
@@ -78,6 +78,7 @@ def load_library():
     L.ctaux_get_N_all.argtypes = [vp, vp]
     L.ctaux_get_N_device.argtypes = [vp, i32, i32, vp, i32]
     L.ctaux_get_stats.argtypes = [vp, i32, C.POINTER(_Stats)]
+    L.ctaux_get_stats_all.argtypes = [vp, vp]
     L.ctaux_get_log.restype = i64
     L.ctaux_get_log.argtypes = [vp, i32, vp, i64, i64]
     L.ctaux_launch_count.restype = i64
@@ -265,6 +266,12 @@ class Walkers:
         _check(self._L.ctaux_get_stats(self._h, w, C.byref(s)), "ctaux_get_stats")
         return {f: getattr(s, f) for f, _ in _Stats._fields_}
 
+    def get_stats_all(self):
+        arr = (_Stats * self.n_walkers)()
+        _check(self._L.ctaux_get_stats_all(self._h, C.addressof(arr)), "ctaux_get_stats_all")
+        names = [f for f, _ in _Stats._fields_]
+        return [{f: getattr(s, f) for f in names} for s in arr]
+
     def get_log(self, w, first=0, count=None):
         if count is None:
             count = self._params.log_capacity
@@ -364,8 +371,7 @@ class WalkerGroups:
         def one(W, g):
             lo = g * self.per
             cfgs[lo:lo + self.per] = W.get_config_all()
-            for i in range(self.per):
-                stats[lo + i] = W.get_stats(i)
+            stats[lo:lo + self.per] = W.get_stats_all()
             if with_N:
                 Ns[lo:lo + self.per] = W.get_N_all([len(c["site"]) for c in cfgs[lo:lo + self.per]])
 

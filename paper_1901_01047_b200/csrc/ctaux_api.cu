@@ -260,6 +260,8 @@ struct ctaux_ctx {
   std::vector<int64_t> mon_rebuilds;
   bool n_fresh;       // N comes straight from a rebuild: nothing to check
   uint32_t probe_salt;
+  PackedCfg pk;       // device staging of the packed configurations
+  uint64_t *pk_next, *pk_p;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
   // timing
@@ -275,7 +277,8 @@ namespace {
 
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
-      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps, total;
+      rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps,
+      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -351,6 +354,9 @@ Layout make_layout(const DevCtx& d) {
   L.mon = take(B * 2 * 3 * kProbes * (size_t)d.ld * 8);
   L.est = take(B * 2 * 8);
   L.tmaps = take(B * 2 * TM_COUNT * sizeof(CUtensorMap));
+  // packed staging of the configurations, [B][max_k] per field (ctaux_set_state / ctaux_get_config_all)
+  L.pk_k = take(B * 4); L.pk_id = take(B * (size_t)d.max_k * 8); L.pk_site = take(B * (size_t)d.max_k * 4);
+  L.pk_tau = take(B * (size_t)d.max_k * 8); L.pk_spin = take(B * (size_t)d.max_k); L.pk_next = take(B * 8); L.pk_p = take(B * 8);
   L.total = o;
   return L;
 }
@@ -780,6 +786,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       }
     }
   }
+  x->pk.k = (int32_t*)(base + L.pk_k); x->pk.id = (uint64_t*)(base + L.pk_id); x->pk.site = (int32_t*)(base + L.pk_site);
+  x->pk.tau = (double*)(base + L.pk_tau); x->pk.spin = (int8_t*)(base + L.pk_spin);
+  x->pk_next = (uint64_t*)(base + L.pk_next); x->pk_p = (uint64_t*)(base + L.pk_p);
   x->mon = (double*)(base + L.mon);
   x->est_d = (double*)(base + L.est);
   x->n_tol = prm->n_tol == 0.0 ? 1e-10 : prm->n_tol;
@@ -913,31 +922,25 @@ int ctaux_set_state(ctaux_ctx* x, const uint64_t* seeds, const int32_t* k, const
   if (!x || !seeds || !k || !id || !site || !tau || !spin || !next_id || !proposals) return CTAUX_EINVAL;
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
-  std::vector<int32_t> spin32((size_t)d.max_k);
+  int kmax = 0;
   for (int w = 0; w < d.B; ++w) {
     if (k[w] < 0 || k[w] > d.max_k) return CTAUX_EINVAL;
-    const size_t off = ((size_t)w * 2 + 0) * d.cap, src = (size_t)w * d.max_k;
-    for (int i = 0; i < k[w]; ++i) spin32[i] = spin[src + i];
-    CU_CHECK(cudaMemcpyAsync(d.cfg_site + off, site + src, 4 * (size_t)k[w], cudaMemcpyHostToDevice, s));
-    CU_CHECK(cudaMemcpyAsync(d.cfg_tau + off, tau + src, 8 * (size_t)k[w], cudaMemcpyHostToDevice, s));
-    CU_CHECK(cudaMemcpyAsync(d.cfg_id + off, id + src, 8 * (size_t)k[w], cudaMemcpyHostToDevice, s));
-    CU_CHECK(cudaMemcpyAsync(d.cfg_spin + off, spin32.data(), 4 * (size_t)k[w], cudaMemcpyHostToDevice, s));
-    CU_CHECK(cudaStreamSynchronize(s));
+    kmax = k[w] > kmax ? k[w] : kmax;
   }
-  // scalars: seeds | k | next_id | proposals staged through the (large enough) Um scratch
-  char* scratch = (char*)d.Um;
-  uint64_t* d_seeds = x->seeds_d;
-  int32_t* d_k = (int32_t*)scratch;
-  uint64_t* d_next = (uint64_t*)(scratch + align256(4 * (size_t)d.B));
-  uint64_t* d_p = (uint64_t*)(scratch + 2 * align256(8 * (size_t)d.B));
-  CU_CHECK(cudaMemcpyAsync(d_seeds, seeds, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
-  CU_CHECK(cudaMemcpyAsync(d_k, k, 4 * (size_t)d.B, cudaMemcpyHostToDevice, s));
-  CU_CHECK(cudaMemcpyAsync(d_next, next_id, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
-  CU_CHECK(cudaMemcpyAsync(d_p, proposals, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
-  k_set_state<<<(d.B + 127) / 128, 128, 0, s>>>(d, d_seeds, d_k, d_next, d_p);
-  tick(x, C_OTHER);
+  // one copy per field for the whole batch, then one scatter kernel (spins int8 -> int32 on the device)
+  const size_t nb = (size_t)d.B * d.max_k;
+  CU_CHECK(cudaMemcpyAsync(x->pk.k, k, 4 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk.id, id, 8 * nb, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk.site, site, 4 * nb, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk.tau, tau, 8 * nb, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk.spin, spin, nb, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->seeds_d, seeds, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk_next, next_id, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  CU_CHECK(cudaMemcpyAsync(x->pk_p, proposals, 8 * (size_t)d.B, cudaMemcpyHostToDevice, s));
+  k_scatter_state<<<dim3(grid_for((size_t)(kmax > 0 ? kmax : 1), 256, 16), d.B), 256, 0, s>>>(d, x->pk);
+  k_set_state<<<(d.B + 127) / 128, 128, 0, s>>>(d, x->seeds_d, x->pk.k, x->pk_next, x->pk_p);
+  tick(x, C_OTHER); tick(x, C_OTHER);
   CU_CHECK(cudaGetLastError());
-  CU_CHECK(cudaStreamSynchronize(s));
   x->sweeps_since_rebuild = 0;
   int rc = do_rebuild(x, true, false);
   x->have_state = (rc == CTAUX_OK);
@@ -1032,24 +1035,18 @@ int ctaux_get_N_device(ctaux_ctx* x, int32_t w, int32_t sp, double* N, int32_t l
 int ctaux_get_config_all(ctaux_ctx* x, int32_t* k, uint64_t* id, int32_t* site, double* tau, int8_t* spin) {
   if (!x || !k) return CTAUX_EINVAL;
   const DevCtx& d = x->d;
-  CU_CHECK(cudaStreamSynchronize(x->stream));
-  std::vector<WalkerState> h(d.B);
-  CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
-  std::vector<int32_t> tmp(spin ? d.max_k : 0);
-  for (int w = 0; w < d.B; ++w) {
-    const int kw = h[w].k;
-    k[w] = kw;
-    if (kw == 0) continue;
-    const size_t off = ((size_t)w * 2 + h[w].cfg_cur) * d.cap, dst = (size_t)w * d.max_k;
-    if (id) CU_CHECK(cudaMemcpyAsync(id + dst, d.cfg_id + off, 8 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
-    if (site) CU_CHECK(cudaMemcpyAsync(site + dst, d.cfg_site + off, 4 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
-    if (tau) CU_CHECK(cudaMemcpyAsync(tau + dst, d.cfg_tau + off, 8 * (size_t)kw, cudaMemcpyDeviceToHost, x->stream));
-    if (spin) {
-      CU_CHECK(cudaMemcpy(tmp.data(), d.cfg_spin + off, 4 * (size_t)kw, cudaMemcpyDeviceToHost));
-      for (int i = 0; i < kw; ++i) spin[dst + i] = (int8_t)tmp[i];
-    }
-  }
-  CU_CHECK(cudaStreamSynchronize(x->stream));
+  cudaStream_t s = x->stream;
+  // one gather kernel (spins int32 -> int8 on the device), then one copy per requested field and ONE synchronisation
+  k_gather_state<<<dim3(grid_for((size_t)d.max_k, 256, 16), d.B), 256, 0, s>>>(d, x->pk);
+  tick(x, C_OTHER);
+  CU_CHECK(cudaGetLastError());
+  const size_t nb = (size_t)d.B * d.max_k;
+  CU_CHECK(cudaMemcpyAsync(k, x->pk.k, 4 * (size_t)d.B, cudaMemcpyDeviceToHost, s));
+  if (id) CU_CHECK(cudaMemcpyAsync(id, x->pk.id, 8 * nb, cudaMemcpyDeviceToHost, s));
+  if (site) CU_CHECK(cudaMemcpyAsync(site, x->pk.site, 4 * nb, cudaMemcpyDeviceToHost, s));
+  if (tau) CU_CHECK(cudaMemcpyAsync(tau, x->pk.tau, 8 * nb, cudaMemcpyDeviceToHost, s));
+  if (spin) CU_CHECK(cudaMemcpyAsync(spin, x->pk.spin, nb, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(cudaStreamSynchronize(s));
   return CTAUX_OK;
 }
 
@@ -1072,11 +1069,7 @@ int ctaux_get_N_all(ctaux_ctx* x, double* N) {
   return CTAUX_OK;
 }
 
-int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
-  if (!x || w < 0 || w >= x->d.B || !out) return CTAUX_EINVAL;
-  CU_CHECK(cudaStreamSynchronize(x->stream));
-  WalkerState st;
-  CU_CHECK(cudaMemcpy(&st, x->d.ws + w, sizeof(st), cudaMemcpyDeviceToHost));
+static void fill_stats(const ctaux_ctx* x, int w, const WalkerState& st, ctaux_stats* out) {
   out->proposals = st.p; out->next_id = st.next_id;
   out->acc_ins = st.acc_ins; out->acc_rem = st.acc_rem; out->sweeps = st.sweeps;
   out->blocks = st.blocks; out->flushes = st.flushes; out->rebuilds = st.rebuilds; out->sum_rank = st.sum_rank;
@@ -1085,6 +1078,23 @@ int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
   out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
   out->guard_ends = st.guard_ends; out->acc_flip = st.acc_flip;
   out->monitor_rebuilds = x->mon_rebuilds[w]; out->err_est = x->last_est[w];
+}
+
+int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {
+  if (!x || w < 0 || w >= x->d.B || !out) return CTAUX_EINVAL;
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  WalkerState st;
+  CU_CHECK(cudaMemcpy(&st, x->d.ws + w, sizeof(st), cudaMemcpyDeviceToHost));
+  fill_stats(x, w, st, out);
+  return CTAUX_OK;
+}
+
+int ctaux_get_stats_all(ctaux_ctx* x, ctaux_stats* out) {
+  if (!x || !out) return CTAUX_EINVAL;
+  std::vector<WalkerState> h(x->d.B);
+  CU_CHECK(cudaMemcpyAsync(h.data(), x->d.ws, sizeof(WalkerState) * x->d.B, cudaMemcpyDeviceToHost, x->stream));
+  CU_CHECK(cudaStreamSynchronize(x->stream));
+  for (int w = 0; w < x->d.B; ++w) fill_stats(x, w, h[w], out + w);
   return CTAUX_OK;
 }
 

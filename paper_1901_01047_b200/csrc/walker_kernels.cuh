@@ -52,6 +52,37 @@ __global__ void k_set_state(DevCtx c, const uint64_t* seeds, const int32_t* k, c
   c.ws[w] = z;
 }
 
+// Batched hand-over of the configurations (ctaux_set_state / ctaux_get_config_all): the host moves ONE packed array
+// per field, [B][max_k] (walker w at offset w*max_k), and these kernels scatter it into / gather it from the per-walker
+// configuration buffers, converting the auxiliary spins between the int8 of the ABI and the int32 kept on the device.
+struct PackedCfg { int32_t* k; uint64_t* id; int32_t* site; double* tau; int8_t* spin; };
+
+__global__ void k_scatter_state(DevCtx c, PackedCfg pk) {   // -> configuration buffer 0 of every walker
+  const int w = blockIdx.y;
+  const int k = pk.k[w];
+  const size_t off = c.cfg_off(w, 0), src = (size_t)w * c.max_k;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < k; i += gridDim.x * blockDim.x) {
+    c.cfg_site[off + i] = pk.site[src + i];
+    c.cfg_tau[off + i] = pk.tau[src + i];
+    c.cfg_id[off + i] = pk.id[src + i];
+    c.cfg_spin[off + i] = (int32_t)pk.spin[src + i];
+  }
+}
+
+__global__ void k_gather_state(DevCtx c, PackedCfg pk) {    // current configuration buffer of every walker ->
+  const int w = blockIdx.y;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  const size_t off = c.cfg_off(w, st.cfg_cur), dst = (size_t)w * c.max_k;
+  if (blockIdx.x == 0 && threadIdx.x == 0) pk.k[w] = k;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < k; i += gridDim.x * blockDim.x) {
+    pk.site[dst + i] = c.cfg_site[off + i];
+    pk.tau[dst + i] = c.cfg_tau[off + i];
+    pk.id[dst + i] = c.cfg_id[off + i];
+    pk.spin[dst + i] = (int8_t)c.cfg_spin[off + i];
+  }
+}
+
 // S1: A_sigma[i][j] = delta_ij E_j - g_ij (E_j - 1) into the current N buffer (column-major).
 __global__ void k_build_A(DevCtx c, int into_other) {
   const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
