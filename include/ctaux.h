@@ -106,6 +106,12 @@ typedef struct ctaux_params {
                               n_tol / 3 at the end of a call (30 n_tol inside a call, where only the acceptance ratios depend
                               on it).  0 = library default 1e-10; < 0 = monitor off (fixed cadence `rebuild_every` only).
                               Chain-neutral like every rebuild.                                                            */
+  int32_t n_omega;         /* single-particle accumulator (S6): number N_w of positive
+                              fermionic Matsubara frequencies w_n = (2n+1) pi / beta, n = 0..N_w-1 (`sp-fermionic-frequencies`).
+                              0 = accumulator off (ctaux_accumulate returns CTAUX_ESTATE).                                  */
+  int32_t nfft_oversampling;/* m of Eq. (31): the tau grid has m * N_w points.  0 = library default 4; >= 2. */
+  int32_t nfft_window;     /* half-width w of the convolution kernel in grid cells (every sample touches 2w grid points,
+                              2w <= 32).  0 = library default 6 (aliasing error ~2e-5 with m = 4; m = 8, w = 10: < 1e-9).   */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */
@@ -198,6 +204,21 @@ int ctaux_get_stats_all(ctaux_ctx* ctx, ctaux_stats* out);
 /* Copy log entries [first, first+count) of one walker into a HOST array; entries are numbered from
  * the last reset and the log keeps the first log_capacity of them. Returns the number copied (>=0). */
 int64_t ctaux_get_log(ctaux_ctx* ctx, int32_t walker, ctaux_log_entry* out, int64_t first, int64_t count);
+
+/* S6 -- single-particle accumulation, needs n_omega > 0.
+ * ctaux_accumulate: for every walker and spin, M_sigma = (E - 1) N_sigma (factor on the row, so that
+ * G_c = G0 - G0 M G0) of the CURRENT configuration, times the walker's sign, is convolved with the NFFT kernel onto the
+ * context's tau grids (one per spin and displacement r_j - r_l; Eq. (30)-(31) PAPER.md:232-238) -- the delayed NFFT: no
+ * transform happens here.  Asynchronous on the context stream.  Call it between ctaux_sweep calls
+ * (`sweeps-per-measurement`).
+ * ctaux_get_M: the ONE transform at the end: out[spin][r][n] = (1/phi_n) sum_l grid[spin][r][l] e^{i w_n l beta/L}
+ * = sum over all accumulated configurations of sign * sum_{jl: r_j-r_l=r} M[j,l] e^{i w_n (tau_j - tau_l)}, as (re, im)
+ * pairs into the HOST array M [2][Nc][n_omega][2]; *sign_sum = sum of the signs, *n_meas = configurations accumulated
+ * (either may be NULL).  <M(r, iw_n)> = out / sign_sum; Eq. (28)-(29) then give G and Sigma.  Does not reset.
+ * ctaux_reset_accumulator: zero the grids and counters. */
+int ctaux_accumulate(ctaux_ctx* ctx);
+int ctaux_get_M(ctaux_ctx* ctx, double* M, double* sign_sum, int64_t* n_meas);
+int ctaux_reset_accumulator(ctaux_ctx* ctx);
 
 /* Kernel launches issued by this context since creation (bench.py's gpu_launches). */
 int64_t ctaux_launch_count(ctaux_ctx* ctx);

@@ -27,7 +27,7 @@ class _Params(C.Structure):
                 ("max_k", C.c_int32), ("rebuild_every", C.c_int32), ("log_capacity", C.c_int32),
                 ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32), ("flip_moves", C.c_int32),
-                ("n_tol", C.c_double)]
+                ("n_tol", C.c_double), ("n_omega", C.c_int32), ("nfft_oversampling", C.c_int32), ("nfft_window", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -44,7 +44,7 @@ class _Stats(C.Structure):
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
-           "ctaux_get_log", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
+           "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
 TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
 
@@ -81,6 +81,9 @@ def load_library():
     L.ctaux_get_stats_all.argtypes = [vp, vp]
     L.ctaux_get_log.restype = i64
     L.ctaux_get_log.argtypes = [vp, i32, vp, i64, i64]
+    L.ctaux_accumulate.argtypes = [vp]
+    L.ctaux_get_M.argtypes = [vp, vp, vp, vp]
+    L.ctaux_reset_accumulator.argtypes = [vp]
     L.ctaux_launch_count.restype = i64
     L.ctaux_launch_count.argtypes = [vp]
     L.ctaux_timing_enable.argtypes = [vp, i32]
@@ -116,7 +119,8 @@ class Walkers:
 
     def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
                  rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None,
-                 guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0, n_tol=0.0):
+                 guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0, n_tol=0.0, n_omega=0, nfft_oversampling=0,
+                 nfft_window=0):
         import torch
         if not torch.cuda.is_available():
             raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
@@ -138,6 +142,8 @@ class Walkers:
         p.rebuild_mode = rebuild_mode
         p.flip_moves = flip_moves
         p.n_tol = n_tol
+        p.n_omega, p.nfft_oversampling, p.nfft_window = n_omega, nfft_oversampling, nfft_window
+        self.n_omega, self.Nc = n_omega, Lx * Ly
         nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
         if nbytes == 0:
             raise CtauxError(-1, "ctaux_workspace_bytes", "invalid parameters")
@@ -265,6 +271,21 @@ class Walkers:
         s = _Stats()
         _check(self._L.ctaux_get_stats(self._h, w, C.byref(s)), "ctaux_get_stats")
         return {f: getattr(s, f) for f, _ in _Stats._fields_}
+
+    def accumulate(self):
+        """S6: add sign * M of every walker's current configuration to the tau-grid accumulators (delayed NFFT)."""
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_accumulate(self._h), "ctaux_accumulate")
+
+    def get_M(self):
+        """(M_sum complex [2][Nc][n_omega], sign_sum, n_meas): the one transform at the end of the run."""
+        out = np.zeros((2, self.Nc, self.n_omega, 2), np.float64)
+        ss, nm = C.c_double(0.0), C.c_int64(0)
+        _check(self._L.ctaux_get_M(self._h, out.ctypes.data, C.addressof(ss), C.addressof(nm)), "ctaux_get_M")
+        return out[..., 0] + 1j * out[..., 1], ss.value, nm.value
+
+    def reset_accumulator(self):
+        _check(self._L.ctaux_reset_accumulator(self._h), "ctaux_reset_accumulator")
 
     def get_stats_all(self):
         arr = (_Stats * self.n_walkers)()

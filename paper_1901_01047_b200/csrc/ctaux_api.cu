@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 
+#include "accumulator.cuh"
 #include "error_monitor.cuh"
 #include "gemm_dmma.cuh"
 #include "gemm_tma.cuh"
@@ -260,6 +261,8 @@ struct ctaux_ctx {
   std::vector<int64_t> mon_rebuilds;
   bool n_fresh;       // N comes straight from a rebuild: nothing to check
   uint32_t probe_salt;
+  AccCtx acc;         // S6 accumulator (accumulator.cuh); acc.n_omega == 0: off
+  int acc_smem;
   PackedCfg pk;       // device staging of the packed configurations
   uint64_t *pk_next, *pk_p;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
@@ -278,7 +281,7 @@ namespace {
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
       rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps,
-      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, total;
+      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -319,7 +322,16 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   return true;
 }
 
-Layout make_layout(const DevCtx& d) {
+struct AccSizes { int n_omega, m, w, L; };
+bool acc_sizes(const ctaux_params* p, AccSizes& a) {
+  a.n_omega = p->n_omega; a.m = p->nfft_oversampling ? p->nfft_oversampling : 4; a.w = p->nfft_window ? p->nfft_window : 6;
+  a.L = a.m * a.n_omega;
+  if (p->n_omega < 0 || p->nfft_oversampling < 0 || p->nfft_window < 0) return false;
+  if (p->n_omega == 0) return true;
+  return a.m >= 2 && a.w >= 1 && 2 * a.w <= 32 && a.L >= 4 * a.w && a.L <= 16384;
+}
+
+Layout make_layout(const DevCtx& d, const AccSizes& ac) {
   Layout L;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
@@ -357,6 +369,15 @@ Layout make_layout(const DevCtx& d) {
   // packed staging of the configurations, [B][max_k] per field (ctaux_set_state / ctaux_get_config_all)
   L.pk_k = take(B * 4); L.pk_id = take(B * (size_t)d.max_k * 8); L.pk_site = take(B * (size_t)d.max_k * 4);
   L.pk_tau = take(B * (size_t)d.max_k * 8); L.pk_spin = take(B * (size_t)d.max_k); L.pk_next = take(B * 8); L.pk_p = take(B * 8);
+  // S6 accumulator (n_omega > 0)
+  const size_t on = ac.n_omega > 0 ? 1 : 0;
+  L.acc_grid = take(on * 2 * d.Nc * (size_t)ac.L * 8);
+  L.acc_tab = take(on * 2 * ((size_t)ac.w * kAccTab + 1) * 8);
+  L.acc_phi = take(on * (size_t)ac.n_omega * 8);
+  L.acc_scal = take(on * 16);
+  L.acc_start = take(on * B * (size_t)(d.Nc + 1) * 4);
+  L.acc_list = take(on * B * (size_t)d.max_k * 4);
+  L.acc_out = take(on * 2 * d.Nc * (size_t)ac.n_omega * 16);
   L.total = o;
   return L;
 }
@@ -723,19 +744,21 @@ const char* ctaux_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 
 size_t ctaux_workspace_bytes(const ctaux_params* prm) {
   DevCtx d;
-  if (!derive_sizes(prm, d)) return 0;
-  return make_layout(d).total;
+  AccSizes ac;
+  if (!derive_sizes(prm, d) || !acc_sizes(prm, ac)) return 0;
+  return make_layout(d, ac).total;
 }
 
 int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   if (out) *out = nullptr;
   DevCtx d;
-  if (!out || !derive_sizes(prm, d) || !prm->g0_table || !prm->workspace) return CTAUX_EINVAL;
+  AccSizes ac;
+  if (!out || !derive_sizes(prm, d) || !acc_sizes(prm, ac) || !prm->g0_table || !prm->workspace) return CTAUX_EINVAL;
   if (((uintptr_t)prm->workspace & 255) != 0) return CTAUX_EINVAL;
   int ndev = 0;
   CU_CHECK(cudaGetDeviceCount(&ndev));
   if (ndev == 0) { g_last_cuda_error = "no CUDA device"; return CTAUX_ECUDA; }
-  const Layout L = make_layout(d);
+  const Layout L = make_layout(d, ac);
   if (prm->workspace_bytes < L.total) return CTAUX_ECAPACITY;
   ctaux_ctx* x = new ctaux_ctx();
   x->prm = *prm;
@@ -853,6 +876,53 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
       static SmemOptIn optin;
       if (optin.ensure(k_walk_fused, need) != cudaSuccess) x->fused = false;
     }
+  }
+  // S6 accumulator: window table and its Fourier coefficients (readings R4-R6 of DESIGN.md), shared-memory budget
+  memset(&x->acc, 0, sizeof(x->acc));
+  x->acc_smem = 0;
+  if (ac.n_omega > 0) {
+    AccCtx& a = x->acc;
+    a.n_omega = ac.n_omega; a.m = ac.m; a.w = ac.w; a.L = ac.L;
+    a.inv_delta = (double)ac.L / prm->beta;
+    a.grid = (double*)(base + L.acc_grid);
+    a.tab = (const double*)(base + L.acc_tab);
+    a.phi_hat = (const double*)(base + L.acc_phi);
+    a.sign_sum = (double*)(base + L.acc_scal);
+    a.n_meas = (long long*)(base + L.acc_scal + 8);
+    a.site_start = (int32_t*)(base + L.acc_start);
+    a.site_list = (int32_t*)(base + L.acc_list);
+    a.out = (double*)(base + L.acc_out);
+    const int nt = ac.w * kAccTab + 1;
+    const double sigma = 0.5 * ac.m, s2 = (2.0 * sigma / (2.0 * sigma - 1.0)) * ((double)ac.w / M_PI);
+    std::vector<double> tab(2 * (size_t)nt), phi(ac.n_omega);
+    for (int i = 0; i < nt; ++i) {
+      const double xx = (double)i / kAccTab, v = exp(-xx * xx / s2);
+      tab[i] = v;
+      tab[nt + i] = (-2.0 * xx / s2 * v) / kAccTab;      // derivative times the table step (cubic Hermite)
+    }
+    // phi_n = sum over the truncated window of phi(x Delta) cos(w_n x Delta) dx, trapezoid on a 64-fold refined grid
+    const int fine = 64;
+    const double delta = prm->beta / ac.L;
+    for (int n = 0; n < ac.n_omega; ++n) {
+      const double wn = (2 * n + 1) * M_PI / prm->beta;
+      double acc = 0.0;
+      for (int i = -ac.w * fine; i <= ac.w * fine; ++i) {
+        const double xx = (double)i / fine;
+        const double wgt = (i == -ac.w * fine || i == ac.w * fine) ? 0.5 : 1.0;
+        acc += wgt * exp(-xx * xx / s2) * cos(wn * xx * delta);
+      }
+      phi[n] = acc / fine;
+    }
+    cudaError_t ea = cudaMemcpy((void*)a.tab, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice);
+    if (ea == cudaSuccess) ea = cudaMemcpy((void*)a.phi_hat, phi.data(), phi.size() * 8, cudaMemcpyHostToDevice);
+    const int tab_bytes = 2 * nt * 8;
+    int copies = (max_smem - tab_bytes - 1024) / (8 * ac.L);
+    if (copies > kAccThreads / 32) copies = kAccThreads / 32;
+    if (ea != cudaSuccess || copies < 1) { free_pinned(x); delete x; return ea != cudaSuccess ? CTAUX_ECUDA : CTAUX_ECAPACITY; }
+    a.copies = copies;
+    x->acc_smem = copies * 8 * ac.L + tab_bytes;
+    static SmemOptIn optin_acc;
+    if (optin_acc.ensure(k_accumulate, x->acc_smem) != cudaSuccess) { free_pinned(x); delete x; return CTAUX_ECUDA; }
   }
   x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
   if (d.max_k > 512) {
@@ -1112,6 +1182,45 @@ int64_t ctaux_get_log(ctaux_ctx* x, int32_t w, ctaux_log_entry* out, int64_t fir
                  cudaMemcpyDeviceToHost) != cudaSuccess)
     return CTAUX_ECUDA;
   return count;
+}
+
+int ctaux_accumulate(ctaux_ctx* x) {
+  if (!x) return CTAUX_EINVAL;
+  if (!x->have_state || x->acc.n_omega == 0) return CTAUX_ESTATE;
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  Scoped t(x, C_OTHER);
+  k_acc_bucket<<<d.B, 256, (d.Nc + 1) * sizeof(int), s>>>(d, x->acc);
+  k_accumulate<<<dim3(d.Nc, 2 * d.B), kAccThreads, x->acc_smem, s>>>(d, x->acc);
+  k_acc_sign<<<1, 1, 0, s>>>(d, x->acc);
+  tick(x, C_OTHER); tick(x, C_OTHER); tick(x, C_OTHER);
+  CU_CHECK(cudaGetLastError());
+  return CTAUX_OK;
+}
+
+int ctaux_get_M(ctaux_ctx* x, double* M, double* sign_sum, int64_t* n_meas) {
+  if (!x || !M) return CTAUX_EINVAL;
+  if (x->acc.n_omega == 0) return CTAUX_ESTATE;
+  const DevCtx& d = x->d;
+  cudaStream_t s = x->stream;
+  k_acc_finalize<<<dim3(d.Nc, 2), 128, 0, s>>>(d, x->acc);
+  tick(x, C_OTHER);
+  CU_CHECK(cudaGetLastError());
+  double scal[2];
+  CU_CHECK(cudaMemcpyAsync(M, x->acc.out, (size_t)2 * d.Nc * x->acc.n_omega * 16, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(cudaMemcpyAsync(scal, x->acc.sign_sum, 16, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(cudaStreamSynchronize(s));
+  if (sign_sum) *sign_sum = scal[0];
+  if (n_meas) { long long nm; memcpy(&nm, &scal[1], 8); *n_meas = (int64_t)nm; }
+  return CTAUX_OK;
+}
+
+int ctaux_reset_accumulator(ctaux_ctx* x) {
+  if (!x) return CTAUX_EINVAL;
+  if (x->acc.n_omega == 0) return CTAUX_ESTATE;
+  CU_CHECK(cudaMemsetAsync(x->acc.grid, 0, (size_t)2 * x->d.Nc * x->acc.L * 8, x->stream));
+  CU_CHECK(cudaMemsetAsync(x->acc.sign_sum, 0, 16, x->stream));
+  return CTAUX_OK;
 }
 
 int64_t ctaux_launch_count(ctaux_ctx* x) { return x ? x->launches : 0; }
