@@ -220,6 +220,22 @@ int ctaux_accumulate(ctaux_ctx* ctx);
 int ctaux_get_M(ctaux_ctx* ctx, double* M, double* sign_sum, int64_t* n_meas);
 int ctaux_reset_accumulator(ctaux_ctx* ctx);
 
+/* Bare cluster propagator of the DCA: the table ctaux_create consumes, computed on the device from the
+ * cluster self-energy instead of the isolated-cluster closed form.
+ *   Gbar(K, iw_n) = patch average of [i w_n - eps_k + mu - Sigma_c(K, iw_n)]^-1   (Eq. (6)-(8) PAPER.md:85-93; standard
+ *                   square patches of the periodic Lx x Ly cluster, n_quad x n_quad midpoint rule; n_quad = 1 = the
+ *                   isolated cluster; eps_k = -2t (cos kx + cos ky), Eq. (45))
+ *   G0c(K, iw_n)  = [Gbar^-1 + Sigma_c]^-1                                        (cluster exclusion, Eq. (9))
+ *   table[d][m]   = G0c(r_d, m beta / n_tau), m = 0..n_tau (0+ and beta- at the ends), STANDARD sign, row d = dx + Lx dy:
+ *                   (1/Nc) sum_K e^{iK.r}, Matsubara sum over +-n from the n_omega positive frequencies with the
+ *                   three-moment tail summed analytically (truncation error O(n_omega^-3)).
+ * sigma_c: HOST [Nc][n_omega][2] (re, im; K = 2 pi (nx/Lx, ny/Ly) at index nx + Lx ny; must obey Sigma_c(-K) = Sigma_c(K)),
+ * or NULL for Sigma_c = 0.  table: HOST [Nc][n_tau + 1].  workspace: DEVICE scratch of ctaux_g0_workspace_bytes().
+ * Synchronises the stream. */
+size_t ctaux_g0_workspace_bytes(int32_t Lx, int32_t Ly, int32_t n_omega, int32_t n_tau);
+int ctaux_g0_table(void* stream, int32_t Lx, int32_t Ly, double t, double mu, double beta, int32_t n_omega, int32_t n_quad,
+                   const double* sigma_c, int32_t n_tau, double* table, void* workspace, size_t workspace_bytes);
+
 /* Kernel launches issued by this context since creation (bench.py's gpu_launches). */
 int64_t ctaux_launch_count(ctaux_ctx* ctx);
 

@@ -44,7 +44,7 @@ class _Stats(C.Structure):
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
-           "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
+           "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_g0_workspace_bytes", "ctaux_g0_table", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
 TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
 
@@ -84,6 +84,9 @@ def load_library():
     L.ctaux_accumulate.argtypes = [vp]
     L.ctaux_get_M.argtypes = [vp, vp, vp, vp]
     L.ctaux_reset_accumulator.argtypes = [vp]
+    L.ctaux_g0_workspace_bytes.restype = C.c_size_t
+    L.ctaux_g0_workspace_bytes.argtypes = [i32, i32, i32, i32]
+    L.ctaux_g0_table.argtypes = [vp, i32, i32, C.c_double, C.c_double, C.c_double, i32, i32, vp, i32, vp, vp, C.c_size_t]
     L.ctaux_launch_count.restype = i64
     L.ctaux_launch_count.argtypes = [vp]
     L.ctaux_timing_enable.argtypes = [vp, i32]
@@ -422,6 +425,31 @@ class WalkerGroups:
     def close(self):
         for W in self.groups:
             W.close()
+
+
+def g0_table_from_sigma(Lx, Ly, t, mu, beta, n_omega, n_quad, n_tau, sigma_c=None, device="cuda:0"):
+    """The DCA bare cluster propagator G0c(r, tau) as the [Nc][n_tau + 1] table ctaux_create consumes (ctaux_g0_table:
+    coarse graining, cluster exclusion and the Fourier transforms run on the device).  sigma_c: complex [Nc][n_omega] or None."""
+    import torch
+    if not torch.cuda.is_available():
+        raise CtauxError(-3, "ctaux_g0_table", "no CUDA device: this package has no CPU fallback")
+    L = load_library()
+    nbytes = L.ctaux_g0_workspace_bytes(Lx, Ly, n_omega, n_tau)
+    if nbytes == 0:
+        raise CtauxError(-1, "ctaux_g0_workspace_bytes", "invalid parameters")
+    dev = torch.device(device)
+    sig_ptr = None
+    if sigma_c is not None:
+        sc = np.asarray(sigma_c, dtype=np.complex128)
+        assert sc.shape == (Lx * Ly, n_omega)
+        sig = np.ascontiguousarray(np.stack([sc.real, sc.imag], axis=-1))
+        sig_ptr = sig.ctypes.data
+    table = np.zeros((Lx * Ly, n_tau + 1), np.float64)
+    with torch.cuda.device(dev):
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+        _check(L.ctaux_g0_table(torch.cuda.current_stream(dev).cuda_stream, Lx, Ly, t, mu, beta, n_omega, n_quad, sig_ptr,
+                                n_tau, table.ctypes.data, ws.data_ptr(), nbytes), "ctaux_g0_table")
+    return table
 
 
 def colmajor(rows, cols, device="cuda", fill=None, generator=None):

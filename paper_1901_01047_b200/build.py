@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libctaux_b200.so")
 SOURCES = ["ctaux_api.cu"]
-HEADERS = ["gemm_dmma.cuh", "gemm_tma.cuh", "walker_state.cuh", "error_monitor.cuh", "accumulator.cuh", "walker_kernels.cuh", "walker_fused.cuh", "walker_propose_cl.cuh", "rebuild_lu.cuh", os.path.join("..", "..", "include", "ctaux.h"),
+HEADERS = ["gemm_dmma.cuh", "gemm_tma.cuh", "walker_state.cuh", "error_monitor.cuh", "accumulator.cuh", "dca_g0.cuh", "walker_kernels.cuh", "walker_fused.cuh", "walker_propose_cl.cuh", "rebuild_lu.cuh", os.path.join("..", "..", "include", "ctaux.h"),
            os.path.join("..", "..", "include", "ctaux_testing.h")]
 
 

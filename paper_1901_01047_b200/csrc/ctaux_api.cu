@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "accumulator.cuh"
+#include "dca_g0.cuh"
 #include "error_monitor.cuh"
 #include "gemm_dmma.cuh"
 #include "gemm_tma.cuh"
@@ -1220,6 +1221,59 @@ int ctaux_reset_accumulator(ctaux_ctx* x) {
   if (x->acc.n_omega == 0) return CTAUX_ESTATE;
   CU_CHECK(cudaMemsetAsync(x->acc.grid, 0, (size_t)2 * x->d.Nc * x->acc.L * 8, x->stream));
   CU_CHECK(cudaMemsetAsync(x->acc.sign_sum, 0, 16, x->stream));
+  return CTAUX_OK;
+}
+
+// device scratch of ctaux_g0_table: sigma | remK | mom | remR | momR | table ; off[6] = total
+static bool g0_layout(int Lx, int Ly, int n_omega, int n_tau, size_t off[7]) {
+  if (Lx < 1 || Ly < 1 || n_omega < 1 || n_tau < 1 || (long long)Lx * Ly > 4096) return false;
+  const size_t Nc = (size_t)Lx * Ly;
+  size_t o = 0;
+  auto take = [&](size_t b) { size_t r = o; o = align256(o + b); return r; };
+  off[0] = take(Nc * n_omega * 16);
+  off[1] = take(Nc * n_omega * 16);
+  off[2] = take(Nc * 16);
+  off[3] = take(Nc * n_omega * 16);
+  off[4] = take(Nc * 16);
+  off[5] = take(Nc * ((size_t)n_tau + 1) * 8);
+  off[6] = o;
+  return true;
+}
+
+size_t ctaux_g0_workspace_bytes(int32_t Lx, int32_t Ly, int32_t n_omega, int32_t n_tau) {
+  size_t off[7];
+  if (!g0_layout(Lx, Ly, n_omega, n_tau, off)) return 0;
+  return off[6];
+}
+
+int ctaux_g0_table(void* stream, int32_t Lx, int32_t Ly, double t, double mu, double beta, int32_t n_omega, int32_t n_quad,
+                   const double* sigma_c, int32_t n_tau, double* table, void* workspace, size_t workspace_bytes) {
+  size_t off[7];
+  if (!table || !workspace || !(beta > 0) || n_quad < 1 || n_quad > 64 || !g0_layout(Lx, Ly, n_omega, n_tau, off)) return CTAUX_EINVAL;
+  if (workspace_bytes < ctaux_g0_workspace_bytes(Lx, Ly, n_omega, n_tau)) return CTAUX_ECAPACITY;
+  if (((uintptr_t)workspace & 255) != 0) return CTAUX_EINVAL;
+  int ndev = 0;
+  CU_CHECK(cudaGetDeviceCount(&ndev));
+  if (ndev == 0) { g_last_cuda_error = "no CUDA device"; return CTAUX_ECUDA; }
+  cudaStream_t s = (cudaStream_t)stream;
+  char* base = (char*)workspace;
+  G0Ctx c;
+  c.Lx = Lx; c.Ly = Ly; c.Nc = Lx * Ly; c.n_omega = n_omega; c.n_quad = n_quad; c.n_tau = n_tau;
+  c.t = t; c.mu = mu; c.beta = beta;
+  c.sigma = nullptr;
+  if (sigma_c) {
+    CU_CHECK(cudaMemcpyAsync(base + off[0], sigma_c, (size_t)c.Nc * n_omega * 16, cudaMemcpyHostToDevice, s));
+    c.sigma = (const double*)(base + off[0]);
+  }
+  c.remK = (double*)(base + off[1]); c.mom = (double*)(base + off[2]); c.remR = (double*)(base + off[3]);
+  c.momR = (double*)(base + off[4]); c.table = (double*)(base + off[5]);
+  k_g0_coarse<<<c.Nc, 256, (size_t)n_quad * n_quad * 8, s>>>(c);
+  k_g0_to_r<<<c.Nc, 256, 0, s>>>(c);
+  const long long warps = (long long)c.Nc * (n_tau + 1);
+  k_g0_to_tau<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, s>>>(c);
+  CU_CHECK(cudaGetLastError());
+  CU_CHECK(cudaMemcpyAsync(table, c.table, (size_t)c.Nc * (n_tau + 1) * 8, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(cudaStreamSynchronize(s));
   return CTAUX_OK;
 }
 
