@@ -262,6 +262,8 @@ struct ctaux_ctx {
   std::vector<int64_t> mon_rebuilds;
   bool n_fresh;       // N comes straight from a rebuild: nothing to check
   uint32_t probe_salt;
+  double *lu_inv, *lu_tmp;   // S5 scratch (rebuild_lu.cuh)
+  int32_t* lu_pos;
   AccCtx acc;         // S6 accumulator (accumulator.cuh); acc.n_omega == 0: off
   int acc_smem;
   PackedCfg pk;       // device staging of the packed configurations
@@ -282,7 +284,7 @@ namespace {
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
       rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps,
-      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, total;
+      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, lu_inv, lu_tmp, lu_pos, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -379,6 +381,10 @@ Layout make_layout(const DevCtx& d, const AccSizes& ac) {
   L.acc_start = take(on * B * (size_t)(d.Nc + 1) * 4);
   L.acc_list = take(on * B * (size_t)d.max_k * 4);
   L.acc_out = take(on * 2 * d.Nc * (size_t)ac.n_omega * 16);
+  // S5 two-level LU: explicit inverse of the 128 x 128 diagonal block, row scratch, row permutation
+  L.lu_inv = take(B * 2 * (size_t)kLuOuter * kLuOuter * 8);
+  L.lu_tmp = take(B * 2 * (size_t)kLuOuter * d.ld * 8);
+  L.lu_pos = take(B * 2 * (size_t)d.ld * 4);
   L.total = o;
   return L;
 }
@@ -532,40 +538,63 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
       tick(x, C_REBUILD); tick(x, C_REBUILD);
     }
     const int cb = grid_for((size_t)2 * kmax, 128, 64);
-    const int nbw = x->lu_nb;
-    auto trailing = [&](int j0, int which, int Mmax, int Nmax) -> cudaError_t {
+    int* dsg = set_sign ? x->detsign : nullptr;
+    const int tri_smem = kLuOuter * (kLuOuter + 1) * 8;
+    static SmemOptIn optin_tri;
+    CU_CHECK(optin_tri.ensure(k_lu_tri_inv, tri_smem));
+    auto gemm2 = [&](int J0, int j0, int wa, int wb, int Mmax, int Nmax) -> cudaError_t {
       if (Mmax <= 0 || Nmax <= 0) return cudaSuccess;
       tick(x, C_REBUILD);
-      return launch_tma<true, 4>(TDescLU{d, j0, which, nbw}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), P, s);
+      return launch_tma<true, 4>(TDescLU2{d, J0, j0, wa, wb, x->lu_tmp}, ((Mmax + 63) / 64) * ((Nmax + 63) / 64), wb >= 0 ? 2 * P : P, s);
     };
-    for (int j0 = 0; j0 < kmax; j0 += nbw) {  // factorisation + forward substitution
+    // forward: two-level right-looking LU of F with partial pivoting, X' = L^-1 in position space (rebuild_lu.cuh)
+    for (int J0 = 0; J0 < kmax; J0 += kLuOuter) {
       Scoped t(x, C_REBUILD);
-      const int j1 = j0 + nbw < kmax ? j0 + nbw : kmax;
-      int* dsg = set_sign ? x->detsign : nullptr;
-      if (x->lu_cluster) {
-        const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
-        if (nbw == 64) k_lu_panel_cl<64><<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, dsg, rl_cap);
-        else k_lu_panel_cl<32><<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, dsg, rl_cap);
-      } else {
-        k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, dsg);
+      const int J1 = J0 + kLuOuter < kmax ? J0 + kLuOuter : kmax;
+      for (int j0 = J0; j0 < J1; j0 += kLuNb) {
+        const int j1 = j0 + kLuNb < kmax ? j0 + kLuNb : kmax;
+        if (x->lu_cluster) {
+          const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
+          k_lu_panel_cl<32><<<P * kLuCl, kLuClThreads, x->lu_cluster_smem, s>>>(d, j0, dsg, rl_cap);
+        } else {
+          k_lu_panel<<<P, pthreads, 0, s>>>(d, j0, dsg);
+        }
+        tick(x, C_REBUILD);
+        if (J1 - J0 > j1 - j0) {     // the other columns of the outer block
+          k_lu_swap_range<<<dim3(1, P), 128, 0, s>>>(d, j0, j1, J0, j0, j1, J1, 0);
+          tick(x, C_REBUILD);
+        }
+        if (j1 < J1) {
+          k_lu_trsm_range<<<dim3(1, P), 128, 0, s>>>(d, j0, j1, J1);
+          tick(x, C_REBUILD);
+          CU_CHECK(gemm2(J0, j0, 0, -1, kmax - j1, J1 - j1));
+        }
       }
-      if (nbw == 64) {
-        k_lu_swap<64><<<dim3(cb, P), 128, 0, s>>>(d, j0);
-        k_lu_trsm<64><<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
-      } else {
-        k_lu_swap<32><<<dim3(cb, P), 128, 0, s>>>(d, j0);
-        k_lu_trsm<32><<<dim3(cb, P), 128, 0, s>>>(d, j0, 0);
-      }
-      tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
-      CU_CHECK(trailing(j0, 0, kmax - j1, kmax - j1));
-      CU_CHECK(trailing(j0, 1, kmax - j1, kmax));
-    }
-    for (int j0 = (kmax - 1) / nbw * nbw; j0 >= 0; j0 -= nbw) {  // backward substitution
-      Scoped t(x, C_REBUILD);
-      if (nbw == 64) k_lu_trsm<64><<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
-      else k_lu_trsm<32><<<dim3(cb, P), 128, 0, s>>>(d, j0, 1);
+      // the block's interchanges on the columns right of it and on X' left of it
+      k_lu_swap_range<<<dim3(cb, P), 128, 0, s>>>(d, J0, J1, J1, kmax, 0, 0, J0);
+      k_lu_tri_inv<<<P, 512, tri_smem, s>>>(d, x->lu_inv, J0, 0);
+      tick(x, C_REBUILD); tick(x, C_REBUILD);
+      CU_CHECK(gemm2(J0, 0, 1, 2, kLuOuter, kmax));                      // tmp = L11^-1 [F12 | X'(rows of the block)]
+      k_lu_copyback<<<dim3(grid_for((size_t)kLuOuter * kmax, 256, 256), P), 256, 0, s>>>(d, x->lu_tmp, x->lu_inv, J0, 0);
       tick(x, C_REBUILD);
-      CU_CHECK(trailing(j0, 2, j0, kmax));
+      CU_CHECK(gemm2(J0, 0, 3, 4, kmax - J1, kmax));                      // rank-128 trailing updates of F and X'
+    }
+    // backward: N' = U^-1 X', outer blocks from the last to the first
+    for (int J0 = (kmax - 1) / kLuOuter * kLuOuter; J0 >= 0; J0 -= kLuOuter) {
+      Scoped t(x, C_REBUILD);
+      k_lu_tri_inv<<<P, 512, tri_smem, s>>>(d, x->lu_inv, J0, 1);
+      tick(x, C_REBUILD);
+      CU_CHECK(gemm2(J0, 0, 5, -1, kLuOuter, kmax));
+      k_lu_copyback<<<dim3(grid_for((size_t)kLuOuter * kmax, 256, 256), P), 256, 0, s>>>(d, x->lu_tmp, x->lu_inv, J0, 1);
+      tick(x, C_REBUILD);
+      CU_CHECK(gemm2(J0, 0, 6, -1, J0, kmax));
+    }
+    {   // N = N' P: column scatter into the buffer that held the factors; the buffers swap roles
+      Scoped t(x, C_REBUILD);
+      k_lu_perm<<<(P + 63) / 64, 64, 0, s>>>(d, x->lu_pos);
+      k_lu_scatter_cols<<<dim3(grid_for((size_t)kmax * kmax, 256, 1024), P), 256, 0, s>>>(d, x->lu_pos);
+      k_lu_flip<<<(d.B + 127) / 128, 128, 0, s>>>(d);
+      tick(x, C_REBUILD); tick(x, C_REBUILD); tick(x, C_REBUILD);
     }
   }
   if (set_sign) { k_set_sign_from_det<<<(d.B + 127) / 128, 128, 0, s>>>(d, x->detsign); tick(x, C_OTHER); }
@@ -800,6 +829,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
           ok = ok && make_map_mmajor(m + TM_V_N, d.Vt + ws2 * (size_t)d.ldr * d.ld, d.ld, d.delay);
           ok = ok && make_map_kmajor(m + TM_SINV_K, d.Sinv + ws2 * (size_t)d.ldr * d.delay, d.ldr, d.ldr, d.delay);
           ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + (size_t)w * d.ld * d.ldm, d.ldm, d.cap);
+          ok = ok && make_map_mmajor(m + TM_LINV_M, (double*)(base + L.lu_inv) + ws2 * (size_t)kLuOuter * kLuOuter, kLuOuter, kLuOuter);
           if (prm->rebuild_mode == 1) ok = ok && make_map_kmajor(m + TM_T_K, (double*)(base + L.Tbuf) + ws2 * nn, d.ld, d.ld, d.ld);
           else m[TM_T_K] = m[TM_N0_K];
         }
@@ -813,6 +843,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   x->pk.k = (int32_t*)(base + L.pk_k); x->pk.id = (uint64_t*)(base + L.pk_id); x->pk.site = (int32_t*)(base + L.pk_site);
   x->pk.tau = (double*)(base + L.pk_tau); x->pk.spin = (int8_t*)(base + L.pk_spin);
   x->pk_next = (uint64_t*)(base + L.pk_next); x->pk_p = (uint64_t*)(base + L.pk_p);
+  x->lu_inv = (double*)(base + L.lu_inv); x->lu_tmp = (double*)(base + L.lu_tmp); x->lu_pos = (int32_t*)(base + L.lu_pos);
   x->mon = (double*)(base + L.mon);
   x->est_d = (double*)(base + L.est);
   x->n_tol = prm->n_tol == 0.0 ? 1e-10 : prm->n_tol;

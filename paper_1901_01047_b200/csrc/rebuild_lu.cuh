@@ -439,3 +439,264 @@ __global__ void k_ns_flip(DevCtx c) {
 }
 
 }  // namespace ctaux
+
+namespace ctaux {
+
+// ===================================================================================================================
+// Two-level blocking of the rebuild (round 2).  The one-level right-looking LU above updates the whole trailing matrix
+// with rank kLuNb = 32 after every panel: arithmetic intensity 4 flop/B, the HBM side of the FP64 ridge (5.4), and the
+// forward substitution ran over the structural zeros of the identity.  Now:
+//   * panels of 32 columns are factorised as before (partial pivoting over the full height), but their rank-32 updates
+//     touch only the columns of the current OUTER block of kLuOuter = 128 columns;
+//   * once per outer block: the block's 128 interchanges are applied to the rest, the 128 x 128 unit-lower block L11 is
+//     inverted explicitly (|L_ij| <= 1 under partial pivoting), U12 = L11^-1 F12 and the trailing update
+//     F22 -= L21 U12 run as rank-128 GEMMs on the TMA tiles (intensity 16 flop/B);
+//   * X' = L^-1 is built IN POSITION SPACE instead of X = L^-1 P: it starts as the identity, receives only the
+//     interchanges of rows that are not yet pivots (columns left of the block), and stays lower triangular, so the
+//     forward GEMMs cover columns [0, J1) only -- k^3/3 instead of k^3 flops;
+//   * backward: per outer block U11^-1 (explicit 128 x 128 inverse) and a rank-128 update of the rows above;
+//   * N = N' P: one column scatter at the end (into the buffer that held F) and the buffers swap roles.
+// Flops: 2/3 + 1/3 + 1 = 2 k^3, the algorithmic count.
+constexpr int kLuOuter = 128;
+
+// interchanges of the pivots [p0, min(p1, k)) applied, in order, to the F columns [fa, fb) U [fc, fd) and the X columns
+// [0, xc); one thread per column
+__global__ void __launch_bounds__(128) k_lu_swap_range(DevCtx c, int p0, int p1, int fa, int fb, int fc, int fd, int xc) {
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (p0 >= k) return;
+  if (p1 > k) p1 = k;
+  if (fb > k) fb = k;
+  if (fd > k) fd = k;
+  if (xc > k) xc = k;
+  const int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  double* X = c.N(w, sp, st.n_cur);
+  __shared__ int s_piv[kLuOuter];
+  const int np = p1 - p0;
+  if (threadIdx.x < np) s_piv[threadIdx.x] = ipiv[p0 + threadIdx.x];
+  __syncthreads();
+  const int n1 = fb > fa ? fb - fa : 0, n2 = fd > fc ? fd - fc : 0, n3 = xc > 0 ? xc : 0;
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n1 + n2 + n3; t += gridDim.x * blockDim.x) {
+    double* col = t < n1 ? F + (size_t)(fa + t) * c.ld : (t < n1 + n2 ? F + (size_t)(fc + t - n1) * c.ld : X + (size_t)(t - n1 - n2) * c.ld);
+    for (int q = 0; q < np; ++q) {
+      const int p = s_piv[q];
+      if (p != p0 + q) {
+        const double a = col[p0 + q], b = col[p];
+        col[p0 + q] = b;
+        col[p] = a;
+      }
+    }
+  }
+}
+
+// rows j0..j1 of the F columns [c0, min(c1, k))  <-  L11^-1 (unit lower, the 32-wide diagonal block at j0)
+__global__ void __launch_bounds__(128) k_lu_trsm_range(DevCtx c, int j0, int c0, int c1) {
+  constexpr int NB = kLuNb;
+  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (j0 >= k) return;
+  const int j1 = (j0 + NB < k) ? j0 + NB : k;
+  if (c1 > k) c1 = k;
+  const int nb = j1 - j0, ld = c.ld;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  __shared__ double T[NB][NB + 1];
+  for (int idx = threadIdx.x; idx < nb * nb; idx += blockDim.x) {
+    const int i = idx % nb, j = idx / nb;
+    T[i][j] = F[(size_t)(j0 + j) * ld + j0 + i];
+  }
+  __syncthreads();
+  for (int t = c0 + blockIdx.x * blockDim.x + threadIdx.x; t < c1; t += gridDim.x * blockDim.x) {
+    double* col = F + (size_t)t * ld + j0;
+    double x[NB];
+#pragma unroll
+    for (int i = 0; i < NB; ++i) x[i] = (i < nb) ? col[i] : 0.0;
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+      if (i < nb) {
+        double s = x[i];
+#pragma unroll
+        for (int l = 0; l < NB; ++l)
+          if (l < i) s -= T[i][l] * x[l];
+        x[i] = s;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+      if (i < nb) col[i] = x[i];
+  }
+}
+
+// explicit inverse of the diagonal block of F at J0 (size nbk = min(128, k - J0)) into Linv [128 x 128], column-major,
+// leading dimension 128:  upper == 0: unit-lower L11;  upper == 1: upper-triangular U11 (with its diagonal).
+// Four lanes share a column of the inverse; the triangle sits in shared memory.
+__global__ void __launch_bounds__(512) k_lu_tri_inv(DevCtx c, double* linv_all, int J0, int upper) {
+  extern __shared__ double s_T[];   // [128][129]
+  const int prob = blockIdx.x, w = prob >> 1, sp = prob & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (J0 >= k) return;
+  const int nbk = (k - J0 < kLuOuter) ? k - J0 : kLuOuter;
+  const double* F = c.N(w, sp, st.n_cur ^ 1);
+  double* out = linv_all + (size_t)prob * kLuOuter * kLuOuter;
+  for (int idx = threadIdx.x; idx < kLuOuter * kLuOuter; idx += blockDim.x) {
+    const int i = idx % kLuOuter, j = idx / kLuOuter;
+    s_T[i * (kLuOuter + 1) + j] = (i < nbk && j < nbk) ? F[(size_t)(J0 + j) * c.ld + J0 + i] : 0.0;
+    out[idx] = 0.0;
+  }
+  __syncthreads();
+  const int col = threadIdx.x >> 2, q = threadIdx.x & 3;
+  const unsigned qmask = 0xFu << (threadIdx.x & 28);
+  double* x = out + (size_t)col * kLuOuter;      // column `col` of the inverse, owned by this quad
+  if (col < nbk) {
+    if (!upper) {
+      if (q == 0) x[col] = 1.0;
+      __syncwarp(qmask);
+      for (int i = col + 1; i < nbk; ++i) {
+        double s = 0.0;
+        for (int l = col + q; l < i; l += 4) s += s_T[i * (kLuOuter + 1) + l] * x[l];
+        s += __shfl_xor_sync(qmask, s, 1);
+        s += __shfl_xor_sync(qmask, s, 2);
+        if (q == 0) x[i] = -s;
+        __syncwarp(qmask);
+      }
+    } else {
+      if (q == 0) x[col] = 1.0 / s_T[col * (kLuOuter + 1) + col];
+      __syncwarp(qmask);
+      for (int i = col - 1; i >= 0; --i) {
+        double s = 0.0;
+        for (int l = i + 1 + q; l <= col; l += 4) s += s_T[i * (kLuOuter + 1) + l] * x[l];
+        s += __shfl_xor_sync(qmask, s, 1);
+        s += __shfl_xor_sync(qmask, s, 2);
+        if (q == 0) x[i] = -s / s_T[i * (kLuOuter + 1) + i];
+        __syncwarp(qmask);
+      }
+    }
+  }
+}
+
+// rows J0..J1 back from the scratch `tmp` [128][ld] (row i, column cidx at tmp[i + cidx*128]):
+//   mode 0 (forward):  F[J0:J1, J1:k) = tmp,  X[J0:J1, 0:J0) = tmp,  X[J0:J1, J0:J1) = Linv
+//   mode 1 (backward): X[J0:J1, 0:k) = tmp
+__global__ void k_lu_copyback(DevCtx c, const double* tmp_all, const double* linv_all, int J0, int mode) {
+  const int prob = blockIdx.y, w = prob >> 1, sp = prob & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  if (J0 >= k) return;
+  const int nbk = (k - J0 < kLuOuter) ? k - J0 : kLuOuter, J1 = J0 + nbk;
+  double* F = c.N(w, sp, st.n_cur ^ 1);
+  double* X = c.N(w, sp, st.n_cur);
+  const double* tmp = tmp_all + (size_t)prob * kLuOuter * c.ld;
+  const double* linv = linv_all + (size_t)prob * kLuOuter * kLuOuter;
+  const size_t total = (size_t)nbk * k;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % nbk), cidx = (int)(idx / nbk);
+    if (mode == 1) X[(size_t)cidx * c.ld + J0 + i] = tmp[(size_t)cidx * kLuOuter + i];
+    else if (cidx >= J1) F[(size_t)cidx * c.ld + J0 + i] = tmp[(size_t)cidx * kLuOuter + i];
+    else if (cidx < J0) X[(size_t)cidx * c.ld + J0 + i] = tmp[(size_t)cidx * kLuOuter + i];
+    else X[(size_t)cidx * c.ld + J0 + i] = linv[(size_t)(cidx - J0) * kLuOuter + i];
+  }
+}
+
+// row permutation of P A = L U as an index array: pos[i] = original row that sits in position i
+__global__ void k_lu_perm(DevCtx c, int32_t* pos_all) {
+  const int prob = blockIdx.x * blockDim.x + threadIdx.x;
+  if (prob >= 2 * c.B) return;
+  const int w = prob >> 1, sp = prob & 1;
+  const int k = c.ws[w].k;
+  const int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
+  int32_t* pos = pos_all + (size_t)prob * c.ld;
+  for (int i = 0; i < k; ++i) pos[i] = i;
+  for (int j = 0; j < k; ++j) {
+    const int p = ipiv[j];
+    if (p != j) { const int a = pos[j]; pos[j] = pos[p]; pos[p] = a; }
+  }
+}
+// N = N' P:  N[:, pos[i]] = N'[:, i], written into the buffer that held the LU factors
+__global__ void k_lu_scatter_cols(DevCtx c, const int32_t* pos_all) {
+  const int prob = blockIdx.y, w = prob >> 1, sp = prob & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  const double* X = c.N(w, sp, st.n_cur);
+  double* O = c.N(w, sp, st.n_cur ^ 1);
+  const int32_t* pos = pos_all + (size_t)prob * c.ld;
+  const size_t total = (size_t)k * k;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx % k), j = (int)(idx / k);
+    O[(size_t)pos[j] * c.ld + i] = X[(size_t)j * c.ld + i];
+  }
+}
+__global__ void k_lu_flip(DevCtx c) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= c.B) return;
+  WalkerState& st = c.ws[w];
+  if (st.k > 0) st.n_cur ^= 1;
+  st.n_src = st.n_cur;
+}
+
+// GEMM problems of the two-level LU (alpha = -1, beta = 1 in place, or alpha = 1, beta = 0 into the row scratch).
+//   0: F[j1:, j1:J1) -= F[j1:, j0:j1) F[j0:j1, j1:J1)                (inner, rank <= 32, inside the outer block)
+//   1: tmp[:, J1:k)   = Linv F[J0:J1, J1:k)         2: tmp[:, 0:J0) = Linv X[J0:J1, 0:J0)
+//   3: F[J1:, J1:)   -= F[J1:, J0:J1) F[J0:J1, J1:)  4: X[J1:, 0:J1) -= F[J1:, J0:J1) X[J0:J1, 0:J1)
+//   5: tmp[:, 0:k)    = Uinv X[J0:J1, 0:k)           6: X[0:J0, 0:k) -= F[0:J0, J0:J1) X[J0:J1, 0:k)
+// A launch covers `which_a` for problems [0, 2B) and `which_b` (if >= 0) for problems [2B, 4B).
+struct TDescLU2 {
+  DevCtx c;
+  int J0, j0, which_a, which_b;
+  double* tmp_all;
+  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
+    const int P = 2 * c.B;
+    const int which = prob < P ? which_a : which_b;
+    if (prob >= P) prob -= P;
+    if (which < 0) return false;
+    const int w = prob >> 1, sp = prob & 1;
+    const WalkerState& st = c.ws[w];
+    const int k = st.k;
+    if (J0 >= k) return false;
+    const int J1 = (J0 + kLuOuter < k) ? J0 + kLuOuter : k;
+    const size_t ld = c.ld;
+    const int fb = st.n_cur ^ 1, xb = st.n_cur;
+    double* F = c.N(w, sp, fb);
+    double* X = c.N(w, sp, xb);
+    double* tmp = tmp_all + (size_t)prob * kLuOuter * c.ld;
+    const CUtensorMap *FM = c.tm(w, sp, fb ? TM_N1_M : TM_N0_M), *FK = c.tm(w, sp, fb ? TM_N1_K : TM_N0_K);
+    const CUtensorMap* XK = c.tm(w, sp, xb ? TM_N1_K : TM_N0_K);
+    d.rowmap = nullptr; d.colmap = nullptr;
+    d.alpha = -1.0; d.beta = 1.0; d.ldc = c.ld; d.ldc0 = c.ld;
+    if (which == 0) {
+      if (j0 >= k) return false;
+      const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
+      d.M = k - j1; d.N = J1 - j1; d.K = j1 - j0;
+      d.tmA = FM; d.a_m0 = j1; d.a_k0 = j0; d.tmB = FK; d.b_k0 = j0; d.b_n0 = j1;
+      d.C = F + j1 + (size_t)j1 * ld;
+    } else if (which == 1 || which == 2 || which == 5) {
+      d.M = J1 - J0; d.K = J1 - J0;
+      d.tmA = c.tm(w, sp, TM_LINV_M); d.a_m0 = 0; d.a_k0 = 0;
+      d.b_k0 = J0;
+      if (which == 1) { d.N = k - J1; d.tmB = FK; d.b_n0 = J1; d.C = tmp + (size_t)J1 * kLuOuter; }
+      else if (which == 2) { d.N = J0; d.tmB = XK; d.b_n0 = 0; d.C = tmp; }
+      else { d.N = k; d.tmB = XK; d.b_n0 = 0; d.C = tmp; }
+      d.alpha = 1.0; d.beta = 0.0; d.ldc = kLuOuter; d.ldc0 = 0;
+      d.C0 = nullptr;
+      return d.M > 0 && d.N > 0;
+    } else if (which == 3) {
+      d.M = k - J1; d.N = k - J1; d.K = J1 - J0;
+      d.tmA = FM; d.a_m0 = J1; d.a_k0 = J0; d.tmB = FK; d.b_k0 = J0; d.b_n0 = J1;
+      d.C = F + J1 + (size_t)J1 * ld;
+    } else if (which == 4) {
+      d.M = k - J1; d.N = J1; d.K = J1 - J0;
+      d.tmA = FM; d.a_m0 = J1; d.a_k0 = J0; d.tmB = XK; d.b_k0 = J0; d.b_n0 = 0;
+      d.C = X + J1;
+    } else {
+      d.M = J0; d.N = k; d.K = J1 - J0;
+      d.tmA = FM; d.a_m0 = 0; d.a_k0 = J0; d.tmB = XK; d.b_k0 = J0; d.b_n0 = 0;
+      d.C = X;
+    }
+    d.C0 = d.C;
+    return d.M > 0 && d.N > 0;
+  }
+};
+
+}  // namespace ctaux

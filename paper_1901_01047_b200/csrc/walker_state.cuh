@@ -13,7 +13,7 @@ constexpr int kMaxSplitK = 8;
 // TMA tensor maps of one (walker, spin): every buffer a GEMM reads as an operand, in the view its role needs
 // (gemm_tma.cuh: "M-major" rank-3 view for left operands and n-contiguous right operands, "K-major" swizzled rank-2
 // view for k-contiguous right operands).  Built once by ctaux_create; they describe capacities, not live sizes.
-enum TmapId { TM_N0_M = 0, TM_N1_M, TM_N0_K, TM_N1_K, TM_BM_M, TM_UM_M, TM_UT_M, TM_V_N, TM_SINV_K, TM_GX_N, TM_T_K, TM_COUNT };
+enum TmapId { TM_N0_M = 0, TM_N1_M, TM_N0_K, TM_N1_K, TM_BM_M, TM_UM_M, TM_UT_M, TM_V_N, TM_SINV_K, TM_GX_N, TM_T_K, TM_LINV_M, TM_COUNT };
 
 struct LogEntry {  // == ctaux_log_entry
   uint64_t p;
