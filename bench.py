@@ -339,6 +339,18 @@ def run_gpu(args):
     tim = W.timing_get()
     W.timing_enable(False)
     dk = diff(s2, s1)
+    # the S5 rebuild is latency-bound (pivot search per column), and inside a step all stream groups rebuild AT THE
+    # SAME TIME: timed here that way (one ctaux_rebuild per group, concurrently), besides the one-group-at-a-time figure
+    torch.cuda.synchronize()
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    r0.record(stream)
+    W.rebuild()
+    torch.cuda.synchronize()
+    r1.record(stream)
+    torch.cuda.synchronize()
+    rebuild_concurrent_ms = r0.elapsed_time(r1)
+    s3 = total_stats(W, B)
+    rebuild_concurrent_flops = s3["flops_rebuild"] - s2["flops_rebuild"]
 
     # max over ranks of the device time; sum over ranks of the work
     ms_max, (acc_all, props_all) = aggregate(ms_total, [acc, d["proposals"]], device=dev)
@@ -372,7 +384,10 @@ def run_gpu(args):
                         "note": "dependent-latency bound chain (one CTA per walker): no roofline applies; see DESIGN.md section 9"}
         steps_ms = {k: v["ms"] for k, v in tim.items()}
         other = {"cand_gemm_tflops": dk["flops_cand"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0,
-                 "rebuild_tflops": dk["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0}
+                 "rebuild_tflops": dk["flops_rebuild"] / (tim["rebuild"]["ms"] * 1e-3) / 1e12 if tim["rebuild"]["ms"] > 0 else 0.0,
+                 "rebuild_all_groups_concurrent_ms": rebuild_concurrent_ms,
+                 "rebuild_all_groups_concurrent_tflops": rebuild_concurrent_flops / (rebuild_concurrent_ms * 1e-3) / 1e12
+                 if rebuild_concurrent_ms > 0 else 0.0}
         cand_tf = other["cand_gemm_tflops"]
         roofline_s2 = {"kernel": "gemm_grouped_kernel<DescCandRows/Cols[SK]> (S2 candidate products, the largest share of a "
                                  "large-k step; ncu: DMMA pipe 81 % busy, profiles/r1_v4_kernels_full.md)",

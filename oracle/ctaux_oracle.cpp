@@ -37,6 +37,12 @@
 //   NEXT-1 (off by default, orc_set_flips): auxiliary-spin flip as a third move, type = (w6*3)>>32, vertex at list
 //       position (w1*k)>>32, R = prod_sigma det A'/det A.  Pinned by the Fock-space trace ratio, T1 == T0, and the
 //       atomic-limit <k> with flips on; the word -> move mapping is a convention (parity unpinned).
+//   NEXT-4 (off by default, orc_set_pairs): general density-density interaction between OPPOSITE spins, Eq. (19)-(21)
+//       H_int = sum_p U_p [n_{a_p up} n_{b_p dn} - (n_{a_p up} + n_{b_p dn})/2] over N_corr pairs
+//       p = (a_p, b_p, U_p) (on-site U: a = b; V between neighbours / layers / orbitals: a != b).  A
+//       vertex is (p, tau, s); Eq. (24)-(25): cosh(gamma_p) = 1 + U_p beta N_corr / (2K); the up matrix sees site a_p,
+//       the down matrix site b_p; both N_sigma stay k x k.  Vertex.site then holds the PAIR index.
+//       Interactions between EQUAL spins (V', two rows of one N_sigma per vertex) are not covered.
 // Pins (tests/test_oracle_*.py): closed-form table values, Fock-space trace = det A,
 // one-vertex closed form, U->0 Poisson law, atomic-limit <k>, reversibility,
 // permutation / spin symmetry, Philox against cuRAND's host generator, T1 == T0.
@@ -181,6 +187,11 @@ struct Walker {
   double beta, U, K;
   std::vector<double> table;  // [Nc][M+1], standard sign
   double egp, egm;            // e^{+gamma}, e^{-gamma}
+  // NEXT-4: interacting pairs (empty = the on-site Hubbard model: pair p = site p, N_corr = Nc, one gamma)
+  std::vector<int> pair_a, pair_b;
+  std::vector<double> pair_egp;
+  int n_corr() const { return pair_a.empty() ? Nc : (int)pair_a.size(); }
+  int site_of(int sidx, int p) const { return pair_a.empty() ? p : (sidx == 0 ? pair_a[p] : pair_b[p]); }
   double tau_scale;           // M / beta
   // chain
   uint32_t key[2];
@@ -212,9 +223,10 @@ struct Walker {
     egm = 1.0 / egp;
   }
   // E(sigma, s) = exp(-gamma sigma s): sigma = +1 (up, index 0) / -1 (down, index 1)
-  double E(int sidx, int s) const {
+  double E(int sidx, int s, int p = 0) const {
     const int sigma = (sidx == 0) ? +1 : -1;
-    return (sigma * s > 0) ? egm : egp;
+    const double eg = pair_a.empty() ? egp : pair_egp[p];
+    return (sigma * s > 0) ? 1.0 / eg : eg;
   }
   // displacement index d(i,j) = ((xi-xj) mod Lx) + Lx ((yi-yj) mod Ly)
   int disp(int i, int j) const {
@@ -235,9 +247,9 @@ struct Walker {
     const double* T = &table[(size_t)d * (M + 1)];
     return -sg * (T[m] + f * (T[m + 1] - T[m]));
   }
-  double g_vv(const Vertex& a, const Vertex& b, bool same) const {
+  double g_vv(int sidx, const Vertex& a, const Vertex& b, bool same) const {
     if (same) return -table[0];  // g(0, 0+)
-    return g(disp(a.site, b.site), a.tau - b.tau);
+    return g(disp(site_of(sidx, a.site), site_of(sidx, b.site)), a.tau - b.tau);
   }
   // A_sigma[i][j] = delta_ij E_j - g_ij (E_j - 1)
   void build_A(int sidx, const std::vector<Vertex>& V, std::vector<double>& A) const {
@@ -245,8 +257,8 @@ struct Walker {
     A.assign((size_t)n * n, 0.0);
     for (int i = 0; i < n; ++i)
       for (int j = 0; j < n; ++j) {
-        const double Ej = E(sidx, V[j].spin);
-        const double gij = g_vv(V[i], V[j], i == j);
+        const double Ej = E(sidx, V[j].spin, V[j].site);
+        const double gij = g_vv(sidx, V[i], V[j], i == j);
         A[(size_t)i * n + j] = (i == j ? Ej : 0.0) - gij * (Ej - 1.0);
       }
   }
@@ -277,7 +289,7 @@ struct Walker {
     Vertex v;
     v.id = 0;
     v.spin = ((w[0] >> 1) & 1u) ? -1 : +1;
-    v.site = (int32_t)(((uint64_t)w[1] * (uint64_t)Nc) >> 32);
+    v.site = (int32_t)(((uint64_t)w[1] * (uint64_t)n_corr()) >> 32);   // site of the on-site model, pair index in general
     v.tau = beta * unif53(w[2], w[3]);
     if (v.tau >= beta) v.tau = std::nextafter(beta, 0.0);
     return v;
@@ -325,11 +337,11 @@ struct Walker {
     const int k = (int)L.size();
     double r = 1.0;
     for (int s = 0; s < 2; ++s) {
-      const double Ev = E(s, v.spin);
+      const double Ev = E(s, v.spin, v.site);
       std::vector<double> q(k), pr(k);
       for (int i = 0; i < k; ++i) {
-        q[i] = -g_vv(L[i], v, false) * (Ev - 1.0);
-        pr[i] = -g_vv(v, L[i], false) * (E(s, L[i].spin) - 1.0);
+        q[i] = -g_vv(s, L[i], v, false) * (Ev - 1.0);
+        pr[i] = -g_vv(s, v, L[i], false) * (E(s, L[i].spin, L[i].site) - 1.0);
       }
       const double d = Ev - (-table[0]) * (Ev - 1.0);
       W.Nq[s].assign(k, 0.0);
@@ -383,7 +395,7 @@ struct Walker {
   double ratio_flip_T1(int j, double r[2]) const {
     const int k = (int)L.size();
     for (int s = 0; s < 2; ++s) {
-      const double Eo = E(s, L[j].spin), En = E(s, -L[j].spin);
+      const double Eo = E(s, L[j].spin, L[j].site), En = E(s, -L[j].spin, L[j].site);
       r[s] = 1.0 + (En - Eo) * (1.0 - N[s][(size_t)j * k + j]) / (Eo - 1.0);
     }
     return r[0] * r[1];
@@ -391,7 +403,7 @@ struct Walker {
   void apply_flip_T1(int j, const double r[2]) {
     const int k = (int)L.size();
     for (int s = 0; s < 2; ++s) {
-      const double Eo = E(s, L[j].spin), En = E(s, -L[j].spin);
+      const double Eo = E(s, L[j].spin, L[j].site), En = E(s, -L[j].spin, L[j].site);
       const double f = (En - Eo) / r[s] / (Eo - 1.0);
       std::vector<double>& Nm = N[s];
       std::vector<double> x(k), row(k);
@@ -550,6 +562,20 @@ void* orc_create(int Lx, int Ly, double beta, double U, double K, int M, const d
 }
 void orc_destroy(void* h) { delete (Walker*)h; }
 void orc_reset(void* h, int init_k) { ((Walker*)h)->reset(init_k); }
+// NEXT-4: interacting pairs (a_p up, b_p down, U_p).  gamma_p from Eq. (25) with N_corr = n_pairs.  n_pairs = 0 restores
+// the on-site model.  Call before reset / set_state.
+void orc_set_pairs(void* h, int n_pairs, const int32_t* a, const int32_t* b, const double* U) {
+  Walker* w = (Walker*)h;
+  w->pair_a.assign(a, a + n_pairs);
+  w->pair_b.assign(b, b + n_pairs);
+  w->pair_egp.resize(n_pairs);
+  for (int p = 0; p < n_pairs; ++p) {
+    const double c = 1.0 + U[p] * w->beta * (double)n_pairs / (2.0 * w->K);
+    w->pair_egp[p] = c + std::sqrt(c * c - 1.0);
+  }
+  w->det_valid = false; w->N_valid = false;
+}
+double orc_pair_exp_gamma(void* h, int p) { return ((Walker*)h)->pair_egp[p]; }
 void orc_set_flips(void* h, int on) { ((Walker*)h)->flips = on ? 1 : 0; }
 int64_t orc_acc_flip(void* h) { return ((Walker*)h)->acc_flip; }
 void orc_set_mode(void* h, int mode) { Walker* w = (Walker*)h; w->mode = mode; w->N_valid = false; w->det_valid = false; }

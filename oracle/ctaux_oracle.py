@@ -44,6 +44,9 @@ def lib():
         L.orc_reset.argtypes = [vp, i32]
         L.orc_set_mode.argtypes = [vp, i32]
         L.orc_set_flips.argtypes = [vp, i32]
+        L.orc_set_pairs.argtypes = [vp, i32, vp, vp, vp]
+        L.orc_pair_exp_gamma.argtypes = [vp, i32]
+        L.orc_pair_exp_gamma.restype = f64
         L.orc_acc_flip.restype = i64
         L.orc_acc_flip.argtypes = [vp]
         L.orc_set_state.argtypes = [vp, i32, vp, vp, vp, vp, u64, u64]
@@ -117,6 +120,18 @@ class OracleWalker:
     def set_flips(self, on=True):
         """Enable the auxiliary-spin flip as a third move.  Default: off."""
         lib().orc_set_flips(self._h, 1 if on else 0)
+
+    def set_pairs(self, a, b, U):
+        """NEXT-4: general opposite-spin density-density interaction, pairs p = (a_p up, b_p down, U_p); the `site` of a
+        vertex (configurations, logs) is then the pair index.  Call before reset / set_state."""
+        a = np.ascontiguousarray(a, dtype=np.int32)
+        b = np.ascontiguousarray(b, dtype=np.int32)
+        U = np.ascontiguousarray(U, dtype=np.float64)
+        assert a.size == b.size == U.size
+        lib().orc_set_pairs(self._h, a.size, a.ctypes.data, b.ctypes.data, U.ctypes.data)
+
+    def pair_exp_gamma(self, p):
+        return lib().orc_pair_exp_gamma(self._h, int(p))
 
     acc_flip = property(lambda s: lib().orc_acc_flip(s._h))
 

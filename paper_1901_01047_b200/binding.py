@@ -363,6 +363,9 @@ class WalkerGroups:
     def sweep(self, n_sweeps):
         self._each(lambda W, g: W.sweep(n_sweeps))
 
+    def rebuild(self):
+        self._each(lambda W, g: W.rebuild())
+
     def _loc(self, w):
         return self.groups[w // self.per], w % self.per
 

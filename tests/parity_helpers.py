@@ -22,6 +22,7 @@ EXACT_FIELDS = ("p", "type", "arg", "tau", "spin", "accepted", "u")
 R_RTOL = 1e-6
 R_ATOL = 1e-8
 N_FROB_TOL = 1e-10     # BASELINE.json north_star: relative Frobenius error of N
+WORST_R = {"frac": 0.0}   # largest R error seen in this session, in units of the tolerance (printed by conftest.py)
 
 
 def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None, flips=0):
@@ -52,6 +53,9 @@ def compare_logs(dev_log, orc_log, what="", r_rtol=None, r_atol=None):
             raise AssertionError(f"{what}: field {f} first differs at entry {i}: dev={dev_log[i]} orc={orc_log[i]} "
                                  f"(oracle margin at that proposal {margin:.3e})")
     both = np.abs(orc_log["R"]) > 0
+    if len(dev_log):
+        frac = np.abs(dev_log["R"] - orc_log["R"]) / (r_rtol * np.abs(orc_log["R"]) + r_atol)
+        WORST_R["frac"] = max(WORST_R["frac"], float(frac.max()))
     err = np.abs(dev_log["R"] - orc_log["R"]) - (r_rtol * np.abs(orc_log["R"]) + r_atol)
     assert err.size == 0 or err.max() < 0, f"{what}: R error beyond tolerance by {err.max():.3e} at entry {err.argmax()}"
     assert np.all(dev_log["R"][~both] == 0.0)
