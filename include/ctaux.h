@@ -106,6 +106,19 @@ typedef struct ctaux_params {
                               n_tol / 3 at the end of a call (30 n_tol inside a call, where only the acceptance ratios depend
                               on it).  0 = library default 1e-10; < 0 = monitor off (fixed cadence `rebuild_every` only).
                               Chain-neutral like every rebuild.                                                            */
+  int32_t n_pairs;         /* general density-density interaction between OPPOSITE spins (Eq. (19)-(21)
+                              PAPER.md:174-182, model parameters U, V of PAPER.md:743-778):
+                                H_int = sum_p U_p [ n_{a_p up} n_{b_p down} - (n_{a_p up} + n_{b_p down}) / 2 ]
+                              over N_corr = n_pairs pairs p = (pair_a[p], pair_b[p], pair_U[p]): on-site repulsion a = b,
+                              inter-site / inter-layer / inter-orbital V between opposite spins a != b.  A vertex is then
+                              (p, tau, s): the `site` of configurations and logs is the PAIR index; cosh(gamma_p) =
+                              1 + U_p beta N_corr / (2K) (Eq. (25)); N_up is built on the sites a_p, N_down on the sites
+                              b_p, both stay k x k.  0 = the on-site Hubbard model (pair p = site p,
+                              N_corr = Nc, coupling `U`).  Interactions between EQUAL spins (V': two rows of one N_sigma per
+                              vertex) are not supported.                                                                    */
+  const int32_t* pair_a;   /* HOST [n_pairs] site of the up electron of pair p (ignored when n_pairs = 0)                    */
+  const int32_t* pair_b;   /* HOST [n_pairs] site of the down electron                                                       */
+  const double* pair_U;    /* HOST [n_pairs] coupling U_p > 0                                                                */
   int32_t n_omega;         /* single-particle accumulator (S6): number N_w of positive
                               fermionic Matsubara frequencies w_n = (2n+1) pi / beta, n = 0..N_w-1 (`sp-fermionic-frequencies`).
                               0 = accumulator off (ctaux_accumulate returns CTAUX_ESTATE).                                  */

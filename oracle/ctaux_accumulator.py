@@ -144,9 +144,10 @@ class DelayedNFFT:
         ph[-1] *= 0.5
         return (ph[:, None] * np.cos(wn[None, :] * (x * self.delta)[:, None])).sum(axis=0) / fine
 
-    def accumulate(self, site, tau, M_up, M_dn, sign=1):
+    def accumulate(self, site, tau, M_up, M_dn, sign=1, site_dn=None):
         """Spread sign * M[j,l] at time tau_j - tau_l (folded antiperiodically, R4) and displacement r_j - r_l onto
-        the 2w nearest grid points, for both spins."""
+        the 2w nearest grid points, for both spins.  site_dn: the sites the DOWN matrix is built on when they differ from
+        those of the up matrix (general interactions, NEXT-4: vertex p = (a_p up, b_p down))."""
         site = np.asarray(site)
         tau = np.asarray(tau, dtype=np.float64)
         self.sign_sum += sign
@@ -154,13 +155,15 @@ class DelayedNFFT:
         k = site.size
         if k == 0:
             return
-        d = displacement(self.Lx, self.Ly, site, site).reshape(-1)
+        d_up = displacement(self.Lx, self.Ly, site, site).reshape(-1)
+        d_dn = d_up if site_dn is None else displacement(self.Lx, self.Ly, np.asarray(site_dn), np.asarray(site_dn)).reshape(-1)
         t = (tau[:, None] - tau[None, :]).reshape(-1)
         sg = np.where(t < 0.0, -1.0, 1.0)
         t = np.where(t < 0.0, t + self.beta, t)
         x = t / self.delta
         l0 = np.floor(x).astype(np.int64)
         for sidx, M in enumerate((M_up, M_dn)):
+            d = d_up if sidx == 0 else d_dn
             val = sign * sg * np.asarray(M).reshape(-1)
             for o in range(-self.w + 1, self.w + 1):          # grid points l0 - w + 1 ... l0 + w
                 l = l0 + o

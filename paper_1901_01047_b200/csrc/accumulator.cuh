@@ -35,34 +35,34 @@ struct AccCtx {
   const double* phi_hat;       // [n_omega]
   double* sign_sum;            // [1]
   long long* n_meas;           // [1]
-  int32_t* site_start;         // [B][Nc + 1]
-  int32_t* site_list;          // [B][max_k]
+  int32_t* site_start;         // [B][2][Nc + 1]   buckets per spin sector (the two sectors may see different sites)
+  int32_t* site_list;          // [B][2][max_k]
   double* out;                 // [2][Nc][n_omega][2]  finalised coefficients (re, im)
 };
 
-// bucket the vertices of every walker by site (counting sort; list order inside a bucket)
+// bucket the vertices of every (walker, spin sector) by the site that sector sees (counting sort; list order inside a bucket)
 __global__ void __launch_bounds__(256) k_acc_bucket(DevCtx c, AccCtx a) {
   extern __shared__ int s_cnt[];   // [Nc + 1]
-  const int w = blockIdx.x;
+  const int w = blockIdx.x >> 1, sp = blockIdx.x & 1;
   const WalkerState& st = c.ws[w];
   const int k = st.k;
-  const int32_t* site = c.cfg_site + c.cfg_off(w, st.cfg_cur);
+  const int32_t* pair = c.cfg_site + c.cfg_off(w, st.cfg_cur);
   for (int i = threadIdx.x; i <= c.Nc; i += blockDim.x) s_cnt[i] = 0;
   __syncthreads();
-  for (int i = threadIdx.x; i < k; i += blockDim.x) atomicAdd(&s_cnt[site[i] + 1], 1);
+  for (int i = threadIdx.x; i < k; i += blockDim.x) atomicAdd(&s_cnt[c.site(sp, pair[i]) + 1], 1);
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int i = 0; i < c.Nc; ++i) s_cnt[i + 1] += s_cnt[i];
   }
   __syncthreads();
-  int32_t* start = a.site_start + (size_t)w * (c.Nc + 1);
+  int32_t* start = a.site_start + (size_t)blockIdx.x * (c.Nc + 1);
   for (int i = threadIdx.x; i <= c.Nc; i += blockDim.x) start[i] = s_cnt[i];
   // stable fill: one thread per site walks the list (k is a few thousand at most, Nc threads in parallel)
-  int32_t* list = a.site_list + (size_t)w * c.max_k;
+  int32_t* list = a.site_list + (size_t)blockIdx.x * c.max_k;
   for (int sidx = threadIdx.x; sidx < c.Nc; sidx += blockDim.x) {
     int pos = s_cnt[sidx];
     for (int i = 0; i < k; ++i)
-      if (site[i] == sidx) list[pos++] = i;
+      if (c.site(sp, pair[i]) == sidx) list[pos++] = i;
   }
 }
 
@@ -101,8 +101,9 @@ __global__ void __launch_bounds__(kAccThreads) k_accumulate(DevCtx c, AccCtx a) 
   const double* tau = c.cfg_tau + off;
   const int32_t* spin = c.cfg_spin + off;
   const double* N = c.N(wk, sp, st.n_cur);
-  const int32_t* start = a.site_start + (size_t)wk * (c.Nc + 1);
-  const int32_t* list = a.site_list + (size_t)wk * c.max_k;
+  const int32_t* pair = c.cfg_site + off;
+  const int32_t* start = a.site_start + (size_t)prob * (c.Nc + 1);
+  const int32_t* list = a.site_list + (size_t)prob * c.max_k;
   const double sgn_w = (double)st.sign;
   const int rx = r % c.Lx, ry = r / c.Lx;
   if (warp < a.copies) {
@@ -126,7 +127,7 @@ __global__ void __launch_bounds__(kAccThreads) k_accumulate(DevCtx c, AccCtx a) 
           if (t < 0.0) { sg = -sg; t += c.beta; }
           x = t * a.inv_delta;
           l0 = (int)floor(x);
-          val = sg * (c.E(sp, spin[j]) - 1.0) * N[(size_t)l * c.ld + j];
+          val = sg * (c.E(sp, spin[j], pair[j]) - 1.0) * N[(size_t)l * c.ld + j];
         }
         const int cnt = npair - base < 32 ? npair - base : 32;
         // ... and the warp spreads them one at a time, one lane per touched grid point

@@ -284,7 +284,7 @@ namespace {
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
       rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps,
-      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, lu_inv, lu_tmp, lu_pos, total;
+      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, lu_inv, lu_tmp, lu_pos, pair_site, pair_E, pair_iem1, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -316,10 +316,14 @@ bool derive_sizes(const ctaux_params* p, DevCtx& d) {
   d.Tbuf = p->rebuild_mode == 1 ? reinterpret_cast<double*>(1) : nullptr;   // flag for make_layout; set for real in create
   d.log_capacity = p->log_capacity;
   d.beta = p->beta; d.K = p->K; d.tau_scale = (double)p->n_tau / p->beta;
-  // Eq. (25): cosh(gamma) = 1 + U beta Ncorr / (2K)
-  const double ch = 1.0 + p->U * p->beta * (double)d.Nc / (2.0 * p->K);
-  d.egp = ch + sqrt(ch * ch - 1.0);
-  d.egm = 1.0 / d.egp;
+  // interacting pairs: N_corr = n_pairs, or the Nc on-site pairs of the single-band Hubbard model
+  if (p->n_pairs < 0 || p->n_pairs > 65535) return false;
+  if (p->n_pairs > 0) {
+    if (!p->pair_a || !p->pair_b || !p->pair_U) return false;
+    for (int q = 0; q < p->n_pairs; ++q)
+      if (p->pair_a[q] < 0 || p->pair_a[q] >= d.Nc || p->pair_b[q] < 0 || p->pair_b[q] >= d.Nc || !(p->pair_U[q] >= 0.0)) return false;
+  }
+  d.n_pairs = p->n_pairs > 0 ? p->n_pairs : d.Nc;
   const double ga = p->guard_amp;
   d.guard_amp = (ga == 0.0) ? 1e2 : ((ga < 0.0 || !(ga < 1e300)) ? 1e308 : ga);
   return true;
@@ -348,7 +352,7 @@ Layout make_layout(const DevCtx& d, const AccSizes& ac) {
   L.prop = take(B * d.winmax * sizeof(PropInfo));
   L.Nbuf = take(B * 4 * (size_t)d.ld * d.ld * 8);
   L.Bm = take(B * 2 * (size_t)d.ldm * d.cap * 8);
-  L.gxC = take(B * (size_t)d.ld * d.ldm * 8);   // g_ext[:, C] stored n-contiguous: n rows of ldm
+  L.gxC = take(B * 2 * (size_t)d.ld * d.ldm * 8);   // g_ext[:, C] stored n-contiguous: n rows of ldm
   L.Gx = take(B * 2 * (size_t)d.ld * d.mmax * 8);
   L.Um = take(B * 2 * (size_t)d.ld * d.delay * 8);
   L.Ut = take(B * 2 * (size_t)d.ld * d.delay * 8);
@@ -378,13 +382,16 @@ Layout make_layout(const DevCtx& d, const AccSizes& ac) {
   L.acc_tab = take(on * 2 * ((size_t)ac.w * kAccTab + 1) * 8);
   L.acc_phi = take(on * (size_t)ac.n_omega * 8);
   L.acc_scal = take(on * 16);
-  L.acc_start = take(on * B * (size_t)(d.Nc + 1) * 4);
-  L.acc_list = take(on * B * (size_t)d.max_k * 4);
+  L.acc_start = take(on * B * 2 * (size_t)(d.Nc + 1) * 4);
+  L.acc_list = take(on * B * 2 * (size_t)d.max_k * 4);
   L.acc_out = take(on * 2 * d.Nc * (size_t)ac.n_omega * 16);
   // S5 two-level LU: explicit inverse of the 128 x 128 diagonal block, row scratch, row permutation
   L.lu_inv = take(B * 2 * (size_t)kLuOuter * kLuOuter * 8);
   L.lu_tmp = take(B * 2 * (size_t)kLuOuter * d.ld * 8);
   L.lu_pos = take(B * 2 * (size_t)d.ld * 4);
+  L.pair_site = take(2 * (size_t)d.n_pairs * 4);
+  L.pair_E = take(2 * (size_t)d.n_pairs * 8);
+  L.pair_iem1 = take(2 * (size_t)d.n_pairs * 8);
   L.total = o;
   return L;
 }
@@ -732,7 +739,8 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
       if (rc) return rc;
     }
     x->n_fresh = false;
-    const bool probe = x->n_tol > 0.0 && ((done / steps_per_poll) & 3) == 3;   // every 32 block steps
+    // every 32 block steps at large k (two passes over N per check), every 8 where the matrices are small
+    const bool probe = x->n_tol > 0.0 && (d.max_k <= 512 || ((done / steps_per_poll) & 3) == 3);
     if (probe) { int rc = enqueue_err_probe(x); if (rc) return rc; }
     CU_CHECK(cudaMemcpyAsync(x->host_flag, d.n_active, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(cudaStreamSynchronize(s));
@@ -828,7 +836,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
           ok = ok && make_map_mmajor(m + TM_UT_M, d.Ut + ws2 * (size_t)d.ld * d.delay, d.ld, d.delay);
           ok = ok && make_map_mmajor(m + TM_V_N, d.Vt + ws2 * (size_t)d.ldr * d.ld, d.ld, d.delay);
           ok = ok && make_map_kmajor(m + TM_SINV_K, d.Sinv + ws2 * (size_t)d.ldr * d.delay, d.ldr, d.ldr, d.delay);
-          ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + (size_t)w * d.ld * d.ldm, d.ldm, d.cap);
+          ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + ws2 * (size_t)d.ld * d.ldm, d.ldm, d.cap);
           ok = ok && make_map_mmajor(m + TM_LINV_M, (double*)(base + L.lu_inv) + ws2 * (size_t)kLuOuter * kLuOuter, kLuOuter, kLuOuter);
           if (prm->rebuild_mode == 1) ok = ok && make_map_kmajor(m + TM_T_K, (double*)(base + L.Tbuf) + ws2 * nn, d.ld, d.ld, d.ld);
           else m[TM_T_K] = m[TM_N0_K];
@@ -855,6 +863,23 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   x->detsign = (int*)(base + L.detsign);
   x->seeds_d = (uint64_t*)(base + L.seeds);
   d.g00 = -prm->g0_table[0];
+  // pair tables: sites per spin sector, E = e^{-+gamma_p} and 1/(E - 1); Eq. (25) PAPER.md:194 with N_corr = n_pairs
+  std::vector<int32_t> h_psite(2 * (size_t)d.n_pairs);
+  std::vector<double> h_pE(2 * (size_t)d.n_pairs), h_piem(2 * (size_t)d.n_pairs);
+  bool any_free = false;   // a pair with U_p = 0 (gamma = 0, E = 1): only the fused path (which never divides by E - 1) runs it
+  for (int q = 0; q < d.n_pairs; ++q) {
+    const double Uq = prm->n_pairs > 0 ? prm->pair_U[q] : prm->U;
+    const double ch = 1.0 + Uq * prm->beta * (double)d.n_pairs / (2.0 * prm->K);
+    const double egp = ch + sqrt(ch * ch - 1.0), egm = 1.0 / egp;
+    h_psite[q] = prm->n_pairs > 0 ? prm->pair_a[q] : q;
+    h_psite[d.n_pairs + q] = prm->n_pairs > 0 ? prm->pair_b[q] : q;
+    h_pE[q] = egm; h_pE[d.n_pairs + q] = egp;
+    h_piem[q] = 1.0 / (egm - 1.0); h_piem[d.n_pairs + q] = 1.0 / (egp - 1.0);
+    any_free = any_free || egp == 1.0;
+  }
+  d.pair_site = (const int32_t*)(base + L.pair_site);
+  d.pair_E = (const double*)(base + L.pair_E);
+  d.pair_iem1 = (const double*)(base + L.pair_iem1);
   x->d = d;
   x->have_state = false;
   x->k_hint = d.max_k;
@@ -871,6 +896,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   if (e == cudaSuccess) e = cudaMallocHost((void**)&x->host_est, 2 * d.B * sizeof(double));
   if (e == cudaSuccess) e = cudaStreamSynchronize(x->stream);
   if (e == cudaSuccess) e = cudaMemcpy(base + L.tmaps, hm.data(), hm.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(base + L.pair_site, h_psite.data(), h_psite.size() * 4, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(base + L.pair_E, h_pE.data(), h_pE.size() * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(base + L.pair_iem1, h_piem.data(), h_piem.size() * 8, cudaMemcpyHostToDevice);
   // proposal kernel shared memory: keep S^-1 of both spins in shared memory when it fits
   int dev = 0, max_smem = 0;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -900,7 +928,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     x->fused = prm->fused_small >= 0 && fits;
     // U = 0 (gamma = 0, E = 1): the delayed-block formulas divide by E - 1; only the fused path (which never does)
     // can run this degenerate case -- N stays 1, R_ins = K/(k+1), R_rem = k/K.  Refuse it loudly otherwise.
-    if (d.egp == 1.0 && !x->fused) { free_pinned(x); delete x; return CTAUX_EINVAL; }
+    if (any_free && !x->fused) { free_pinned(x); delete x; return CTAUX_EINVAL; }
     x->fcap = fcap;
     const int need = fused_smem_layout(fcap).total;
     x->fused_smem = need;
@@ -1222,7 +1250,7 @@ int ctaux_accumulate(ctaux_ctx* x) {
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
   Scoped t(x, C_OTHER);
-  k_acc_bucket<<<d.B, 256, (d.Nc + 1) * sizeof(int), s>>>(d, x->acc);
+  k_acc_bucket<<<2 * d.B, 256, (d.Nc + 1) * sizeof(int), s>>>(d, x->acc);
   k_accumulate<<<dim3(d.Nc, 2 * d.B), kAccThreads, x->acc_smem, s>>>(d, x->acc);
   k_acc_sign<<<1, 1, 0, s>>>(d, x->acc);
   tick(x, C_OTHER); tick(x, C_OTHER); tick(x, C_OTHER);

@@ -72,14 +72,14 @@ __global__ void __launch_bounds__(kMonWarps * 32) k_mon_resid(DevCtx c, double* 
   const int32_t* site = c.cfg_site + off;
   const double* tau = c.cfg_tau + off;
   for (int l = blockIdx.x * kMonWarps + warp; l < k; l += gridDim.x * kMonWarps) {
-    const double El = c.E(sp, c.cfg_spin[off + l]);
-    const int sl = site[l];
+    const double El = c.E(sp, c.cfg_spin[off + l], site[l]);
+    const int sl = c.site(sp, site[l]);
     const double tl = tau[l];
     double acc[kProbes];
 #pragma unroll
     for (int p = 0; p < kProbes; ++p) acc[p] = 0.0;
     for (int j = lane; j < k; j += 32) {
-      const double a = (j == l) ? (El - c.g00 * (El - 1.0)) : -c.g(c.disp(site[j], sl), tau[j] - tl) * (El - 1.0);
+      const double a = (j == l) ? (El - c.g00 * (El - 1.0)) : -c.g(c.disp(c.site(sp, site[j]), sl), tau[j] - tl) * (El - 1.0);
 #pragma unroll
       for (int p = 0; p < kProbes; ++p) acc[p] += y[(size_t)p * c.ld + j] * a;
     }

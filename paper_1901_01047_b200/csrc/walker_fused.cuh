@@ -99,7 +99,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
   int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, log_count = st.log_count;
   double min_margin = st.min_margin, sum_k = 0.0;
   int sweeps_done = 0;
-  const double em1p = c.egm - 1.0, em1m = c.egp - 1.0;   // E - 1 for sigma*s = +1 / -1
+  // site_s[] holds the PAIR index of every slot (= the site in the on-site model); E and the site a spin sector sees
+  // come from the pair tables of DevCtx
   __syncthreads();
 
   for (int sw = 0; sw < n_sweeps && !status; ++sw) {
@@ -118,18 +119,20 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
       if (type == 0) {
         // ---------------------------------------------------------------- insertion
         vs = ((wa[0] >> 1) & 1u) ? -1 : +1;
-        const int vsite = (int)(((uint64_t)wa[1] * (uint64_t)c.Nc) >> 32);
+        const int vsite = (int)(((uint64_t)wa[1] * (uint64_t)c.n_pairs) >> 32);   // pair index of the proposed vertex
         vtau = c.beta * unif53(wa[2], wa[3]);
         if (vtau >= c.beta) vtau = nextafter(c.beta, 0.0);
         arg = vsite;
-        const double Ev1 = ((sp == 0) == (vs > 0)) ? em1p : em1m;          // E_v - 1
+        const double Ev1 = c.E(sp, vs, vsite) - 1.0;          // E_v - 1
+        const int vs_site = c.site(sp, vsite);                // the site this spin sector sees
         for (int a = lt; a < hi; a += kFusedGroup) {
           double qa = 0.0, pa = 0.0;
           const int sa = spin_s[a];
           if (sa != 0) {
-            const double Ea1 = ((sp == 0) == (sa > 0)) ? em1p : em1m;
-            qa = -c.g(c.disp(site_s[a], vsite), tau_s[a] - vtau) * Ev1;
-            pa = -c.g(c.disp(vsite, site_s[a]), vtau - tau_s[a]) * Ea1;
+            const double Ea1 = c.E(sp, sa, site_s[a]) - 1.0;
+            const int a_site = c.site(sp, site_s[a]);
+            qa = -c.g(c.disp(a_site, vs_site), tau_s[a] - vtau) * Ev1;
+            pa = -c.g(c.disp(vs_site, a_site), vtau - tau_s[a]) * Ea1;
           }
           qv[a] = qa; pv[a] = pa;
         }
@@ -182,7 +185,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
         if ((tid & 31) == 0) red[sp * 4 + (lt >> 5)] = part;
         __syncthreads();
-        const double e0 = vs > 0 ? em1p : em1m, e1 = vs > 0 ? em1m : em1p;   // E_v - 1 for spin up / down
+        const double e0 = c.E(0, vs, vsite) - 1.0, e1 = c.E(1, vs, vsite) - 1.0;   // E_v - 1 for spin up / down
         const double d0 = (e0 + 1.0) - c.g00 * e0;
         const double d1 = (e1 + 1.0) - c.g00 * e1;
         const double stil0 = d0 - ((red[0] + red[1]) + (red[2] + red[3]));
@@ -235,8 +238,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         arg = j;
         slot = live[j];
         const int so = spin_s[slot];
-        const double eo0 = so > 0 ? em1p : em1m, en0 = so > 0 ? em1m : em1p;   // spin up: E(s) - 1, E(-s) - 1
-        const double eo1 = so > 0 ? em1m : em1p, en1 = so > 0 ? em1p : em1m;   // spin down
+        const int pr = site_s[slot];
+        const double eo0 = c.E(0, so, pr) - 1.0, en0 = c.E(0, -so, pr) - 1.0;   // spin up: E(s) - 1, E(-s) - 1
+        const double eo1 = c.E(1, so, pr) - 1.0, en1 = c.E(1, -so, pr) - 1.0;   // spin down
         const double n0 = Nup[slot + slot * lds], n1 = Ndn[slot + slot * lds];
         const double r0 = 1.0 + (en0 - eo0) * (1.0 - n0) / eo0;
         const double r1 = 1.0 + (en1 - eo1) * (1.0 - n1) / eo1;

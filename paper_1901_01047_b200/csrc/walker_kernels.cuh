@@ -21,7 +21,7 @@ __global__ void k_init_config(DevCtx c, const uint64_t* seeds, int init_k) {
     double tau = c.beta * unif53(r[2], r[3]);
     if (tau >= c.beta) tau = nextafter(c.beta, 0.0);
     c.cfg_spin[off + i] = ((r[0] >> 1) & 1u) ? -1 : +1;
-    c.cfg_site[off + i] = (int32_t)(((uint64_t)r[1] * (uint64_t)c.Nc) >> 32);
+    c.cfg_site[off + i] = (int32_t)(((uint64_t)r[1] * (uint64_t)c.n_pairs) >> 32);   // pair index (= site in the on-site model)
     c.cfg_tau[off + i] = tau;
     c.cfg_id[off + i] = (uint64_t)i;
   }
@@ -94,10 +94,10 @@ __global__ void k_build_A(DevCtx c, int into_other) {
   for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
        idx += (size_t)gridDim.x * blockDim.x) {
     const int i = (int)(idx % k), j = (int)(idx / k);
-    const double Ej = c.E(sp, c.cfg_spin[off + j]);
+    const double Ej = c.E(sp, c.cfg_spin[off + j], c.cfg_site[off + j]);
     double v;
     if (i == j) v = Ej - c.g00 * (Ej - 1.0);
-    else v = -c.g(c.disp(c.cfg_site[off + i], c.cfg_site[off + j]), c.cfg_tau[off + i] - c.cfg_tau[off + j]) * (Ej - 1.0);
+    else v = -c.g(c.pdisp(sp, c.cfg_site[off + i], c.cfg_site[off + j]), c.cfg_tau[off + i] - c.cfg_tau[off + j]) * (Ej - 1.0);
     A[(size_t)j * c.ld + i] = v;
   }
 }
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(1024) k_prep_window(DevCtx c) {
       double tau = c.beta * unif53(wa[2], wa[3]);
       if (tau >= c.beta) tau = nextafter(c.beta, 0.0);
       c.cfg_spin[off] = ((wa[0] >> 1) & 1u) ? -1 : +1;
-      c.cfg_site[off] = (int32_t)(((uint64_t)wa[1] * (uint64_t)c.Nc) >> 32);
+      c.cfg_site[off] = (int32_t)(((uint64_t)wa[1] * (uint64_t)c.n_pairs) >> 32);
       c.cfg_tau[off] = tau;
       c.cfg_id[off] = ~0ull;
     }
@@ -194,7 +194,8 @@ __global__ void k_prep_fill(DevCtx c) {
   const int32_t* spin = c.cfg_spin + off;
   double* Bm0 = c.Bm + ((size_t)w * 2 + 0) * (size_t)c.ldm * c.cap;
   double* Bm1 = c.Bm + ((size_t)w * 2 + 1) * (size_t)c.ldm * c.cap;
-  double* gx = c.gxC + (size_t)w * c.ld * c.ldm;
+  double* gx0 = c.gxC + ((size_t)w * 2 + 0) * c.ld * c.ldm;
+  double* gx1 = c.gxC + ((size_t)w * 2 + 1) * c.ld * c.ldm;
   double* N0 = c.N(w, 0, st.n_cur);
   double* N1 = c.N(w, 1, st.n_cur);
   const size_t total = (size_t)n * m;
@@ -202,20 +203,28 @@ __global__ void k_prep_fill(DevCtx c) {
        idx += (size_t)gridDim.x * blockDim.x) {
     const int i = (int)(idx % n), cc = (int)(idx / n);
     const int sc = k + cc;
-    // column: g(i, c)
-    double gic;
-    if (i == sc) gic = c.g00;
-    else gic = c.g(c.disp(site[i], site[sc]), tau[i] - tau[sc]);
-    gx[(size_t)i * c.ldm + cc] = gic;   // g_ext[:, C] stored n-contiguous (the "N-major" right operand of gemm_tma.cuh)
+    const int pi = site[i], pc = site[sc];                    // pair indices; the two spin sectors may see different sites
+    const int i0 = c.site(0, pi), i1 = c.site(1, pi), c0 = c.site(0, pc), c1 = c.site(1, pc);
+    const bool same = (i0 == i1) && (c0 == c1);                // on-site pairs: one interpolation serves both spins
+    // column: g(i, c), stored n-contiguous (the "N-major" right operand of gemm_tma.cuh)
+    double gic0, gic1;
+    if (i == sc) { gic0 = c.g00; gic1 = c.g00; }
+    else {
+      gic0 = c.g(c.disp(i0, c0), tau[i] - tau[sc]);
+      gic1 = same ? gic0 : c.g(c.disp(i1, c1), tau[i] - tau[sc]);
+    }
+    gx0[(size_t)i * c.ldm + cc] = gic0;
+    gx1[(size_t)i * c.ldm + cc] = gic1;
     // [*, cand] block of N_ext
     const double e = (i == sc) ? 1.0 : 0.0;
     N0[(size_t)sc * c.ld + i] = e;
     N1[(size_t)sc * c.ld + i] = e;
     // row: g(c, j)(E_j - 1), only against the live vertices j < k
     if (i < k) {
-      const double gci = c.g(c.disp(site[sc], site[i]), tau[sc] - tau[i]);
-      Bm0[(size_t)i * c.ldm + cc] = gci * (c.E(0, spin[i]) - 1.0);
-      Bm1[(size_t)i * c.ldm + cc] = gci * (c.E(1, spin[i]) - 1.0);
+      const double gci0 = c.g(c.disp(c0, i0), tau[sc] - tau[i]);
+      const double gci1 = same ? gci0 : c.g(c.disp(c1, i1), tau[sc] - tau[i]);
+      Bm0[(size_t)i * c.ldm + cc] = gci0 * (c.E(0, spin[i], pi) - 1.0);
+      Bm1[(size_t)i * c.ldm + cc] = gci1 * (c.E(1, spin[i], pi) - 1.0);
     }
   }
 }
@@ -232,7 +241,7 @@ constexpr int kGroup = kPropThreads / 2;  // threads per spin
 
 struct ProposeSmem {
   // byte offsets into dynamic shared memory
-  int sinv, scol, srow, tv, tpv, red, snn, live0, live1, spin, J, jpos, prop, flip, total;
+  int sinv, scol, srow, tv, tpv, jiem, red, snn, live0, live1, spin, J, jpos, prop, flip, total;
 };
 
 __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
@@ -244,6 +253,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.srow = o; o += 2 * delay * 8;
   L.tv = o; o += 2 * delay * 8;
   L.tpv = o; o += 2 * delay * 8;
+  L.jiem = o; o += 2 * delay * 8;
   L.red = o; o += 2 * 2 * 8 * 8;
   L.snn = o; o += 4 * 8;
   L.prop = o; o += winmax * 16;
@@ -274,6 +284,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   double* srow = reinterpret_cast<double*>(smraw + L.srow) + sp * c.delay;
   double* tv = reinterpret_cast<double*>(smraw + L.tv) + sp * c.delay;
   double* tpv = reinterpret_cast<double*>(smraw + L.tpv) + sp * c.delay;
+  double* jiem = reinterpret_cast<double*>(smraw + L.jiem) + sp * c.delay;   // 1/(E0 - 1) of the buffered block-start vertices
   double* red = reinterpret_cast<double*>(smraw + L.red);   // [2][8] dot products, [2][8] sums of magnitudes
   double* snn2 = reinterpret_cast<double*>(smraw + L.snn);  // [2 parities][2 spins]
   PropInfo* prop = reinterpret_cast<PropInfo*>(smraw + L.prop);
@@ -290,7 +301,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   const double* Ncur = c.N(w, sp, st.n_cur);
   const double* Gx = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
   const int ld = c.ld;
-  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
+  const int32_t* pair_g = c.cfg_site + off_old;   // pair index of every extended slot
 
   for (int i = tid; i < n; i += kPropThreads) spin_s[i] = (signed char)c.cfg_spin[off_old + i];
   for (int i = tid; i < k0; i += kPropThreads) { live[i] = i; flipped[i] = 0; }
@@ -298,12 +309,10 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   for (int i = tid; i <= c.winmax; i += kPropThreads) jpos[i] = -1;
   __syncthreads();
 
-  auto X = [&](int i, int j) -> double {
+  // X[i, j] with the factor 1/(E0_j - 1) of a block-start column j handed in by the caller
+  auto X = [&](int i, int j, double iem_j) -> double {
     const double dlt = (i == j) ? 1.0 : 0.0;
-    if (j < k0) {
-      const bool em = ((sp == 0) == (spin_s[j] > 0));
-      return (dlt - Ncur[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
-    }
+    if (j < k0) return (dlt - Ncur[(size_t)j * ld + i]) * iem_j;
     return dlt - Gx[(size_t)(j - k0) * ld + i];
   };
 
@@ -341,7 +350,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
-    double R = 0.0, stil_own = 1.0, amp = 1.0;
+    double R = 0.0, stil_own = 1.0, amp = 1.0, iem_own = 0.0;
     // removal of a vertex inserted earlier in this block: the two changes of that slot cancel, so
     // the buffered insertion is taken OUT of the block (exact treatment of a twice-touched spin,
     // PAPER.md:228): ratio = (S^-1)_aa / dE_a, then S^-1 is downdated.
@@ -351,30 +360,34 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       apos = jpos[slot - k0];
       const int s = spin_s[slot];
       const double sa0 = Sbase[apos + (size_t)apos * lds], sa1 = Sbase[sstride + apos + (size_t)apos * lds];
-      R = pref * ((sa0 / (c.E(0, s) - 1.0)) * (sa1 / (c.E(1, s) - 1.0)));
+      const int pr = pair_g[slot];
+      R = pref * ((sa0 / (c.E(0, s, pr) - 1.0)) * (sa1 / (c.E(1, s, pr) - 1.0)));
       accept = pi.u < fabs(R);
       stil_own = sp == 0 ? sa0 : sa1;
     } else if (slot >= 0) {
       const int s = spin_s[slot];
-      const double E0 = c.E(0, s), E1 = c.E(1, s);
+      const int pr = pair_g[slot];
+      const double E0 = c.E(0, s, pr), E1 = c.E(1, s, pr);
       // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s) - E0));
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s) - E1));
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s, pr) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s, pr) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
+      const double iem_slot = c.iem1(sp, s, pr);     // 1/(E0 - 1) of this slot's column (used when slot < k0)
+      iem_own = iem_slot;
       // thread roles inside a spin group of 128: half 0 builds s_col and t = S^-1 s_col (and the dot
       // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass
       const int half = lt >> 6, la = lt & 63;
       for (int a = la; a < r; a += 64) {
         const int ja = Js[a];
-        if (half == 0) scol[a] = X(ja, slot);
-        else srow[a] = X(slot, ja);
+        if (half == 0) scol[a] = X(ja, slot, iem_slot);
+        else srow[a] = X(slot, ja, jiem[a]);
       }
       double* snn = snn2 + (i & 1) * 2;   // double buffered: read after the second barrier of this proposal
       if (lt == 0) {
         // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
         // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
-        if (slot < k0 && type == 1) snn[sp] = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
-        else snn[sp] = 1.0 / dE_own + X(slot, slot);
+        if (slot < k0 && type == 1) snn[sp] = -Ncur[(size_t)slot * ld + slot] * iem_slot;
+        else snn[sp] = 1.0 / dE_own + X(slot, slot, iem_slot);
       }
       __syncthreads();
       double part = 0.0, apart = 0.0;
@@ -473,6 +486,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
         __syncthreads();
         for (int a = lt; a < last; a += kGroup) Sv[a + (size_t)apos * lds] = Sv[a + (size_t)last * lds];
       }
+      if (lt == 0 && apos != last) jiem[apos] = jiem[last];
       if (tid == 0) {
         jpos[slot - k0] = -1;
         if (apos != last) {
@@ -497,7 +511,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
         Sv[a + (size_t)r * lds] = -tv[a] * inv;
         Sv[r + (size_t)a * lds] = -tpv[a] * inv;
       }
-      if (lt == 0) Sv[r + (size_t)r * lds] = inv;
+      if (lt == 0) { Sv[r + (size_t)r * lds] = inv; jiem[r] = iem_own; }
       if (tid == 0) Js[r] = slot;
       errlvl = fmax(errlvl, amp);
       if (type == 0) {
@@ -583,7 +597,6 @@ __global__ void k_build_uv(DevCtx c) {
   const int* rowmap = c.rowmap + (size_t)w * c.cap;
   const int* J = c.J + (size_t)w * c.delay;
   const int ld = c.ld;
-  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
   const size_t total = (size_t)kn * r;
   for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
        idx += (size_t)gridDim.x * blockDim.x) {
@@ -593,8 +606,7 @@ __global__ void k_build_uv(DevCtx c) {
       const double dlt = (i == j) ? 1.0 : 0.0;
       double x;
       if (j < k0) {
-        const bool em = ((sp == 0) == (c.cfg_spin[off_old + j] > 0));
-        x = (dlt - Nsrc[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
+        x = (dlt - Nsrc[(size_t)j * ld + i]) * c.iem1(sp, c.cfg_spin[off_old + j], c.cfg_site[off_old + j]);
       } else {
         x = dlt - Gx[(size_t)(j - k0) * ld + i];
       }

@@ -16,7 +16,7 @@ namespace ctaux {
 constexpr int kClThreads = 512;
 
 struct ProposeClSmem {
-  int sinv, scol, srow, tv, tpv, red, snn, xch, live0, live1, spin, J, jpos, prop, flip, total;
+  int sinv, scol, srow, tv, tpv, jiem, red, snn, xch, live0, live1, spin, J, jpos, prop, flip, total;
 };
 __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
   ProposeClSmem L;
@@ -27,6 +27,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.srow = o; o += delay * 8;
   L.tv = o; o += delay * 8;
   L.tpv = o; o += delay * 8;
+  L.jiem = o; o += delay * 8;
   L.red = o; o += 2 * 16 * 8;
   L.snn = o; o += 2 * 8;
   L.xch = o; o += 2 * 2 * 4 * 8;      // [parity][spin][stil, ampnum, -, -]
@@ -57,6 +58,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   double* srow = reinterpret_cast<double*>(smcl + L.srow);
   double* tv = reinterpret_cast<double*>(smcl + L.tv);
   double* tpv = reinterpret_cast<double*>(smcl + L.tpv);
+  double* jiem = reinterpret_cast<double*>(smcl + L.jiem);   // 1/(E0 - 1) of the buffered block-start vertices (own spin)
   double* red = reinterpret_cast<double*>(smcl + L.red);    // [16] dot, [16] sum of magnitudes
   double* snn2 = reinterpret_cast<double*>(smcl + L.snn);   // [2 parities]
   double* xch = reinterpret_cast<double*>(smcl + L.xch);
@@ -75,7 +77,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   const double* Ncur = c.N(w, sp, st.n_cur);
   const double* Gx = c.Gx + ((size_t)w * 2 + sp) * (size_t)c.ld * c.mmax;
   const int ld = c.ld;
-  const double inv_em1_m = 1.0 / (c.egm - 1.0), inv_em1_p = 1.0 / (c.egp - 1.0);
+  const int32_t* pair_g = c.cfg_site + off_old;   // pair index of every extended slot
   // everything read from the walker state BEFORE the first cluster barrier; rank 0 alone writes it at the end
   int kcur = k0, r = 0, len = k0;
   int props_left = st.props_left, sweeps_left = st.sweeps_left;
@@ -95,12 +97,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   for (int i = tid; i <= c.winmax; i += kClThreads) jpos[i] = -1;
   cluster.sync();
 
-  auto X = [&](int i, int j) -> double {
+  auto X = [&](int i, int j, double iem_j) -> double {   // iem_j = 1/(E0_j - 1) of a block-start column j
     const double dlt = (i == j) ? 1.0 : 0.0;
-    if (j < k0) {
-      const bool em = ((sp == 0) == (spin_s[j] > 0));
-      return (dlt - Ncur[(size_t)j * ld + i]) * (em ? inv_em1_m : inv_em1_p);
-    }
+    if (j < k0) return (dlt - Ncur[(size_t)j * ld + i]) * iem_j;
     return dlt - Gx[(size_t)(j - k0) * ld + i];
   };
   // publish this spin's two scalars to both CTAs, one cluster barrier, read both spins' values
@@ -145,7 +144,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
-    double R = 0.0, stil_own = 1.0, amp = 1.0;
+    double R = 0.0, stil_own = 1.0, amp = 1.0, iem_own = 0.0;
     const bool down = (type == 1 && slot >= k0);
     int apos = -1;
     if (down) {
@@ -155,25 +154,29 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       const double sa_own = Sv[apos + (size_t)apos * lds];
       double o0[2], o1[2];
       exchange(sa_own, 0.0, o0, o1);
-      R = pref * ((o0[0] / (c.E(0, s) - 1.0)) * (o1[0] / (c.E(1, s) - 1.0)));
+      const int pr = pair_g[slot];
+      R = pref * ((o0[0] / (c.E(0, s, pr) - 1.0)) * (o1[0] / (c.E(1, s, pr) - 1.0)));
       accept = pi.u < fabs(R);
       stil_own = sa_own;
     } else if (slot >= 0) {
       const int s = spin_s[slot];
-      const double E0 = c.E(0, s), E1 = c.E(1, s);
+      const int pr = pair_g[slot];
+      const double E0 = c.E(0, s, pr), E1 = c.E(1, s, pr);
       // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s) - E0));
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s) - E1));
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s, pr) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s, pr) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
+      const double iem_slot = c.iem1(sp, s, pr);
+      iem_own = iem_slot;
       for (int a = rl; a < r; a += 256) {
         const int ja = Js[a];
-        if (role == 0) scol[a] = X(ja, slot);
-        else srow[a] = X(slot, ja);
+        if (role == 0) scol[a] = X(ja, slot, iem_slot);
+        else srow[a] = X(slot, ja, jiem[a]);
       }
       double* snn = snn2 + (i & 1);
       if (tid == 0) {
-        if (slot < k0 && type == 1) *snn = -Ncur[(size_t)slot * ld + slot] * (((sp == 0) == (s > 0)) ? inv_em1_m : inv_em1_p);
-        else *snn = 1.0 / dE_own + X(slot, slot);
+        if (slot < k0 && type == 1) *snn = -Ncur[(size_t)slot * ld + slot] * iem_slot;
+        else *snn = 1.0 / dE_own + X(slot, slot, iem_slot);
       }
       __syncthreads();
       double part = 0.0, apart = 0.0;
@@ -258,6 +261,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
         __syncthreads();
         for (int a = tid; a < last; a += kClThreads) Sv[a + (size_t)apos * lds] = Sv[a + (size_t)last * lds];
       }
+      if (tid == 0 && apos != last) jiem[apos] = jiem[last];
       if (tid == 0) {
         jpos[slot - k0] = -1;
         if (apos != last) {
@@ -282,7 +286,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
         Sv[a + (size_t)r * lds] = -tv[a] * inv;
         Sv[r + (size_t)a * lds] = -tpv[a] * inv;
       }
-      if (tid == 0) { Sv[r + (size_t)r * lds] = inv; Js[r] = slot; }
+      if (tid == 0) { Sv[r + (size_t)r * lds] = inv; Js[r] = slot; jiem[r] = iem_own; }
       errlvl = fmax(errlvl, amp);
       if (type == 0) {
         if (tid == 0) {

@@ -61,7 +61,15 @@ struct DevCtx {
   int ldm;   // leading dimension of Bm (mmax rounded up to 8)
   int ldr;   // leading dimension of Vt / Sinv in global memory (delay rounded up to 8)
   int log_capacity;
-  double beta, K, tau_scale, egp, egm, g00;
+  double beta, K, tau_scale, g00;
+  // Interacting pairs (Eq. (19)-(25)): H_int = sum_p U_p [n_{a_p up} n_{b_p dn} - ...]
+  // over n_pairs = N_corr pairs.  A vertex is (pair, tau, s): cfg_site holds the PAIR index; the up matrix sees site
+  // a_p, the down matrix site b_p, with gamma_p from Eq. (25).  The on-site Hubbard model is the identity table
+  // (pair p = site p, N_corr = Nc, one gamma), so every kernel goes through these tables.
+  int n_pairs;
+  const int32_t* pair_site;   // [2][n_pairs]  site of the up / down electron of pair p
+  const double* pair_E;       // [2][n_pairs]  E for sigma*s = +1 (e^{-gamma_p}), then for sigma*s = -1 (e^{+gamma_p})
+  const double* pair_iem1;    // [2][n_pairs]  1 / (E - 1) for the same two cases
   double guard_amp;  // rounding-amplification limit of the bordered ratio evaluation (k_propose)
   const double* table;  // [Nc][M+1]
   WalkerState* ws;      // [B]
@@ -70,7 +78,7 @@ struct DevCtx {
   PropInfo* prop;       // [B][winmax]
   double* Nbuf;         // [B][2 spins][2 bufs][ld*ld]
   double* Bm;           // [B][2][ldm*cap]   candidate rows  g(c,j)(E_j-1), m x k col-major
-  double* gxC;          // [B][ld*ldm]       g_ext[:, C] stored n-contiguous: element (i, c) at i*ldm + c (spin independent)
+  double* gxC;          // [B][2][ld*ldm]    g_ext[:, C] per spin sector, stored n-contiguous: element (i, c) at i*ldm + c
   double* Gx;           // [B][2][ld*mmax]   N_ext * g_ext[:, C]
   double* Tbuf;         // [B][2][ld*ld]  A*N of the Newton-Schulz refresh (rebuild_mode 1), else null
   unsigned long long* resid;  // [B*2]  max |A N - 1| per matrix as the bit pattern of a non-negative double
@@ -96,10 +104,16 @@ struct DevCtx {
   __device__ __forceinline__ double* N(int w, int s, int buf) const {
     return Nbuf + (((size_t)w * 2 + s) * 2 + buf) * (size_t)ld * ld;
   }
-  __device__ __forceinline__ double E(int sidx, int s) const {
-    // sigma = +1 for sidx 0 (up), -1 for sidx 1; E = exp(-gamma sigma s)
-    return ((sidx == 0) == (s > 0)) ? egm : egp;
+  // sigma = +1 for sidx 0 (up), -1 for sidx 1; E = exp(-gamma_p sigma s)
+  __device__ __forceinline__ double E(int sidx, int s, int p) const {
+    return __ldg(pair_E + (((sidx == 0) == (s > 0)) ? 0 : n_pairs) + p);
   }
+  __device__ __forceinline__ double iem1(int sidx, int s, int p) const {   // 1 / (E - 1)
+    return __ldg(pair_iem1 + (((sidx == 0) == (s > 0)) ? 0 : n_pairs) + p);
+  }
+  __device__ __forceinline__ int site(int sidx, int p) const { return __ldg(pair_site + sidx * n_pairs + p); }
+  // displacement index between the sites two vertices (pairs pi, pj) occupy in spin sector sidx
+  __device__ __forceinline__ int pdisp(int sidx, int pi, int pj) const { return disp(site(sidx, pi), site(sidx, pj)); }
   __device__ __forceinline__ int disp(int i, int j) const {
     const int xi = i % Lx, yi = i / Lx, xj = j % Lx, yj = j / Lx;
     int dx = xi - xj; if (dx < 0) dx += Lx;

@@ -25,11 +25,13 @@ N_FROB_TOL = 1e-10     # BASELINE.json north_star: relative Frobenius error of N
 WORST_R = {"frac": 0.0}   # largest R error seen in this session, in units of the tolerance (printed by conftest.py)
 
 
-def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None, flips=0):
+def run_oracle(cfg, table, seeds, n_sweeps, mode, init_k=None, flips=0, pairs=None):
     init_k = cfg["init_k"] if init_k is None else init_k
 
     def one(seed):
         w = OracleWalker.from_config(cfg, table, int(seed), mode)
+        if pairs is not None:
+            w.set_pairs(*pairs)
         if flips:
             w.set_flips(True)
         w.reset(init_k)
@@ -85,7 +87,8 @@ def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
 
 
 def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, init_k=None, seeds=None,
-                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0, rebuild_mode=0, flips=0):
+                check_N=True, cand_window=0, max_k=None, n_tol=N_FROB_TOL, fused=0, rebuild_mode=0, flips=0, pairs=None,
+                r_rtol=None):
     """reset + n_sweeps on both sides, compare logs, configurations, N, sign, counters."""
     from paper_1901_01047_b200 import Walkers
     table = table_for(cfg)
@@ -96,14 +99,15 @@ def full_parity(cfg, n_walkers, n_sweeps, mode, delay=None, rebuild_every=None, 
                 delay=cfg["delay"] if delay is None else delay, n_walkers=n_walkers, init_k=init_k,
                 max_k=cfg["max_k"] if max_k is None else max_k,
                 rebuild_every=cfg["rebuild_every"] if rebuild_every is None else rebuild_every,
-                log_capacity=cap, cand_window=cand_window, fused_small=fused, rebuild_mode=rebuild_mode, flip_moves=flips)
+                log_capacity=cap, cand_window=cand_window, fused_small=fused, rebuild_mode=rebuild_mode, flip_moves=flips,
+                pairs=pairs)
     W.reset(seeds)
     W.sweep(n_sweeps)
-    orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k, flips=flips)
+    orcs = run_oracle(cfg, table, seeds, n_sweeps, mode, init_k, flips=flips, pairs=pairs)
     worst = 0.0
     for w, o in enumerate(orcs):
         what = f"{cfg['name']} walker {w}"
-        compare_logs(W.get_log(w), o.log(), what)
+        compare_logs(W.get_log(w), o.log(), what, r_rtol=r_rtol)
         compare_configs(W.get_config(w), o.config(), what)
         st = W.get_stats(w)
         assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id, what
