@@ -655,10 +655,17 @@ int enqueue_block_step(ctaux_ctx* x) {
     }
     {
       Scoped t(x, C_PROPOSE, ps);
-      if (x->cluster_mode == 1) k_propose_cl<true><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
-      else if (x->cluster_mode == 2) k_propose_cl<false><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
-      else if (x->sinv_smem) k_propose<true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
-      else k_propose<false><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      if (d.onsite) {
+        if (x->cluster_mode == 1) k_propose_cl<true, true><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+        else if (x->cluster_mode == 2) k_propose_cl<false, true><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+        else if (x->sinv_smem) k_propose<true, true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+        else k_propose<false, true><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      } else {
+        if (x->cluster_mode == 1) k_propose_cl<true, false><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+        else if (x->cluster_mode == 2) k_propose_cl<false, false><<<2 * d.B, kClThreads, x->cluster_smem, ps>>>(d);
+        else if (x->sinv_smem) k_propose<true, false><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+        else k_propose<false, false><<<d.B, kPropThreads, x->propose_smem, ps>>>(d);
+      }
       tick(x, C_PROPOSE);
     }
     if (x->hi) {
@@ -707,7 +714,8 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
     CU_CHECK(cudaMemsetAsync(d.n_active, 0, 2 * sizeof(int), s));
     {
       Scoped t(x, C_PROPOSE);
-      k_walk_fused<<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
+      if (d.onsite) k_walk_fused<true><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
+      else k_walk_fused<false><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
       tick(x, C_PROPOSE);
       x->n_fresh = false;
     }
@@ -836,7 +844,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
           ok = ok && make_map_mmajor(m + TM_UT_M, d.Ut + ws2 * (size_t)d.ld * d.delay, d.ld, d.delay);
           ok = ok && make_map_mmajor(m + TM_V_N, d.Vt + ws2 * (size_t)d.ldr * d.ld, d.ld, d.delay);
           ok = ok && make_map_kmajor(m + TM_SINV_K, d.Sinv + ws2 * (size_t)d.ldr * d.delay, d.ldr, d.ldr, d.delay);
-          ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + ws2 * (size_t)d.ld * d.ldm, d.ldm, d.cap);
+          ok = ok && make_map_mmajor(m + TM_GX_N, d.gxC + (prm->n_pairs > 0 ? ws2 : (size_t)w * 2) * (size_t)d.ld * d.ldm, d.ldm, d.cap);
           ok = ok && make_map_mmajor(m + TM_LINV_M, (double*)(base + L.lu_inv) + ws2 * (size_t)kLuOuter * kLuOuter, kLuOuter, kLuOuter);
           if (prm->rebuild_mode == 1) ok = ok && make_map_kmajor(m + TM_T_K, (double*)(base + L.Tbuf) + ws2 * nn, d.ld, d.ld, d.ld);
           else m[TM_T_K] = m[TM_N0_K];
@@ -877,6 +885,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     h_piem[q] = 1.0 / (egm - 1.0); h_piem[d.n_pairs + q] = 1.0 / (egp - 1.0);
     any_free = any_free || egp == 1.0;
   }
+  d.onsite = prm->n_pairs > 0 ? 0 : 1;
+  d.egm = h_pE[0]; d.egp = h_pE[d.n_pairs]; d.iem_m = h_piem[0]; d.iem_p = h_piem[d.n_pairs];
   d.pair_site = (const int32_t*)(base + L.pair_site);
   d.pair_E = (const double*)(base + L.pair_E);
   d.pair_iem1 = (const double*)(base + L.pair_iem1);
@@ -909,8 +919,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
     x->propose_smem = Ls.total;
     if (Ls.total > max_smem) { free_pinned(x); delete x; return CTAUX_ECAPACITY; }
-    static SmemOptIn optin[2];   // the attribute is per function and device, shared by all contexts
-    e = x->sinv_smem ? optin[1].ensure(k_propose<true>, Ls.total) : optin[0].ensure(k_propose<false>, Ls.total);
+    static SmemOptIn optin[4];   // the attribute is per function and device, shared by all contexts
+    if (x->sinv_smem) { e = optin[1].ensure(k_propose<true, true>, Ls.total); if (e == cudaSuccess) e = optin[2].ensure(k_propose<true, false>, Ls.total); }
+    else { e = optin[0].ensure(k_propose<false, true>, Ls.total); if (e == cudaSuccess) e = optin[3].ensure(k_propose<false, false>, Ls.total); }
   }
   if (e != cudaSuccess) {
     g_last_cuda_error = std::string("ctaux_create: ") + cudaGetErrorString(e);
@@ -934,7 +945,8 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     x->fused_smem = need;
     if (x->fused) {
       static SmemOptIn optin;
-      if (optin.ensure(k_walk_fused, need) != cudaSuccess) x->fused = false;
+      static SmemOptIn optin2;
+      if (optin.ensure(k_walk_fused<true>, need) != cudaSuccess || optin2.ensure(k_walk_fused<false>, need) != cudaSuccess) x->fused = false;
     }
   }
   // S6 accumulator: window table and its Fourier coefficients (readings R4-R6 of DESIGN.md), shared-memory budget
@@ -1003,7 +1015,9 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (Lc.total > max_smem) { Lc = propose_cl_smem_layout(d.cap, d.delay, d.winmax, false); mode = 2; }
     if (Lc.total <= max_smem) {
       static SmemOptIn optin_cl[2];
-      cudaError_t ec = mode == 1 ? optin_cl[1].ensure(k_propose_cl<true>, Lc.total) : optin_cl[0].ensure(k_propose_cl<false>, Lc.total);
+      static SmemOptIn optin_clp[2];
+      cudaError_t ec = mode == 1 ? optin_cl[1].ensure(k_propose_cl<true, true>, Lc.total) : optin_cl[0].ensure(k_propose_cl<false, true>, Lc.total);
+      if (ec == cudaSuccess) ec = mode == 1 ? optin_clp[1].ensure(k_propose_cl<true, false>, Lc.total) : optin_clp[0].ensure(k_propose_cl<false, false>, Lc.total);
       if (ec == cudaSuccess) { x->cluster_mode = mode; x->cluster_smem = Lc.total; }
       else cudaGetLastError();
     }

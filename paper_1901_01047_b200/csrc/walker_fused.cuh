@@ -47,6 +47,7 @@ __host__ __device__ inline FusedSmem fused_smem_layout(int cap) {
   return L;
 }
 
+template <bool ONSITE>   // the on-site Hubbard model (one gamma, one site per vertex) or interacting pairs through the tables
 __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n_sweeps, int fcap) {
   extern __shared__ __align__(16) unsigned char fsm[];
   const int wk = blockIdx.x, tid = threadIdx.x;
@@ -123,14 +124,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         vtau = c.beta * unif53(wa[2], wa[3]);
         if (vtau >= c.beta) vtau = nextafter(c.beta, 0.0);
         arg = vsite;
-        const double Ev1 = c.E(sp, vs, vsite) - 1.0;          // E_v - 1
-        const int vs_site = c.site(sp, vsite);                // the site this spin sector sees
+        const double Ev1 = c.template Et<ONSITE>(sp, vs, vsite) - 1.0;          // E_v - 1
+        const int vs_site = c.template sitet<ONSITE>(sp, vsite);                // the site this spin sector sees
         for (int a = lt; a < hi; a += kFusedGroup) {
           double qa = 0.0, pa = 0.0;
           const int sa = spin_s[a];
           if (sa != 0) {
-            const double Ea1 = c.E(sp, sa, site_s[a]) - 1.0;
-            const int a_site = c.site(sp, site_s[a]);
+            const double Ea1 = c.template Et<ONSITE>(sp, sa, site_s[a]) - 1.0;
+            const int a_site = c.template sitet<ONSITE>(sp, site_s[a]);
             qa = -c.g(c.disp(a_site, vs_site), tau_s[a] - vtau) * Ev1;
             pa = -c.g(c.disp(vs_site, a_site), vtau - tau_s[a]) * Ea1;
           }
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
         if ((tid & 31) == 0) red[sp * 4 + (lt >> 5)] = part;
         __syncthreads();
-        const double e0 = c.E(0, vs, vsite) - 1.0, e1 = c.E(1, vs, vsite) - 1.0;   // E_v - 1 for spin up / down
+        const double e0 = c.template Et<ONSITE>(0, vs, vsite) - 1.0, e1 = c.template Et<ONSITE>(1, vs, vsite) - 1.0;   // E_v - 1 for spin up / down
         const double d0 = (e0 + 1.0) - c.g00 * e0;
         const double d1 = (e1 + 1.0) - c.g00 * e1;
         const double stil0 = d0 - ((red[0] + red[1]) + (red[2] + red[3]));
@@ -239,8 +240,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
         slot = live[j];
         const int so = spin_s[slot];
         const int pr = site_s[slot];
-        const double eo0 = c.E(0, so, pr) - 1.0, en0 = c.E(0, -so, pr) - 1.0;   // spin up: E(s) - 1, E(-s) - 1
-        const double eo1 = c.E(1, so, pr) - 1.0, en1 = c.E(1, -so, pr) - 1.0;   // spin down
+        const double eo0 = c.template Et<ONSITE>(0, so, pr) - 1.0, en0 = c.template Et<ONSITE>(0, -so, pr) - 1.0;   // spin up: E(s) - 1, E(-s) - 1
+        const double eo1 = c.template Et<ONSITE>(1, so, pr) - 1.0, en1 = c.template Et<ONSITE>(1, -so, pr) - 1.0;   // spin down
         const double n0 = Nup[slot + slot * lds], n1 = Ndn[slot + slot * lds];
         const double r0 = 1.0 + (en0 - eo0) * (1.0 - n0) / eo0;
         const double r1 = 1.0 + (en1 - eo1) * (1.0 - n1) / eo1;

@@ -214,7 +214,7 @@ __global__ void k_prep_fill(DevCtx c) {
       gic1 = same ? gic0 : c.g(c.disp(i1, c1), tau[i] - tau[sc]);
     }
     gx0[(size_t)i * c.ldm + cc] = gic0;
-    gx1[(size_t)i * c.ldm + cc] = gic1;
+    if (!c.onsite) gx1[(size_t)i * c.ldm + cc] = gic1;   // (on-site model: both sectors read the sp = 0 copy)
     // [*, cand] block of N_ext
     const double e = (i == sc) ? 1.0 : 0.0;
     N0[(size_t)sc * c.ld + i] = e;
@@ -267,7 +267,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   return L;
 }
 
-template <bool sinv_smem>   // S^-1 of both spins in shared memory (delay <= ~100) or in global memory
+template <bool sinv_smem, bool ONSITE>   // S^-1 of both spins in shared memory (delay <= ~100) or in global memory; model class
 __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const int w = blockIdx.x, tid = threadIdx.x;
@@ -360,19 +360,19 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       apos = jpos[slot - k0];
       const int s = spin_s[slot];
       const double sa0 = Sbase[apos + (size_t)apos * lds], sa1 = Sbase[sstride + apos + (size_t)apos * lds];
-      const int pr = pair_g[slot];
-      R = pref * ((sa0 / (c.E(0, s, pr) - 1.0)) * (sa1 / (c.E(1, s, pr) - 1.0)));
+      const int pr = (ONSITE ? 0 : pair_g[slot]);
+      R = pref * ((sa0 / (c.template Et<ONSITE>(0, s, pr) - 1.0)) * (sa1 / (c.template Et<ONSITE>(1, s, pr) - 1.0)));
       accept = pi.u < fabs(R);
       stil_own = sp == 0 ? sa0 : sa1;
     } else if (slot >= 0) {
       const int s = spin_s[slot];
-      const int pr = pair_g[slot];
-      const double E0 = c.E(0, s, pr), E1 = c.E(1, s, pr);
+      const int pr = (ONSITE ? 0 : pair_g[slot]);
+      const double E0 = c.template Et<ONSITE>(0, s, pr), E1 = c.template Et<ONSITE>(1, s, pr);
       // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s, pr) - E0));
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s, pr) - E1));
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.template Et<ONSITE>(0, -s, pr) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.template Et<ONSITE>(1, -s, pr) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
-      const double iem_slot = c.iem1(sp, s, pr);     // 1/(E0 - 1) of this slot's column (used when slot < k0)
+      const double iem_slot = c.template iem1t<ONSITE>(sp, s, pr);     // 1/(E0 - 1) of this slot's column (used when slot < k0)
       iem_own = iem_slot;
       // thread roles inside a spin group of 128: half 0 builds s_col and t = S^-1 s_col (and the dot
       // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass

@@ -42,7 +42,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   return L;
 }
 
-template <bool sinv_smem>
+template <bool sinv_smem, bool ONSITE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_propose_cl(DevCtx c) {
   namespace cg = cooperative_groups;
   cg::cluster_group cluster = cg::this_cluster();
@@ -154,19 +154,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       const double sa_own = Sv[apos + (size_t)apos * lds];
       double o0[2], o1[2];
       exchange(sa_own, 0.0, o0, o1);
-      const int pr = pair_g[slot];
-      R = pref * ((o0[0] / (c.E(0, s, pr) - 1.0)) * (o1[0] / (c.E(1, s, pr) - 1.0)));
+      const int pr = (ONSITE ? 0 : pair_g[slot]);
+      R = pref * ((o0[0] / (c.template Et<ONSITE>(0, s, pr) - 1.0)) * (o1[0] / (c.template Et<ONSITE>(1, s, pr) - 1.0)));
       accept = pi.u < fabs(R);
       stil_own = sa_own;
     } else if (slot >= 0) {
       const int s = spin_s[slot];
-      const int pr = pair_g[slot];
-      const double E0 = c.E(0, s, pr), E1 = c.E(1, s, pr);
+      const int pr = (ONSITE ? 0 : pair_g[slot]);
+      const double E0 = c.template Et<ONSITE>(0, s, pr), E1 = c.template Et<ONSITE>(1, s, pr);
       // column change of A: insert 1 -> E, remove E -> 1, flip E(s) -> E(-s)
-      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.E(0, -s, pr) - E0));
-      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.E(1, -s, pr) - E1));
+      const double dE0 = (type == 0) ? (E0 - 1.0) : (type == 1 ? (1.0 - E0) : (c.template Et<ONSITE>(0, -s, pr) - E0));
+      const double dE1 = (type == 0) ? (E1 - 1.0) : (type == 1 ? (1.0 - E1) : (c.template Et<ONSITE>(1, -s, pr) - E1));
       const double dE_own = sp == 0 ? dE0 : dE1;
-      const double iem_slot = c.iem1(sp, s, pr);
+      const double iem_slot = c.template iem1t<ONSITE>(sp, s, pr);
       iem_own = iem_slot;
       for (int a = rl; a < r; a += 256) {
         const int ja = Js[a];

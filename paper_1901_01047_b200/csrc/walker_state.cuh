@@ -67,6 +67,8 @@ struct DevCtx {
   // a_p, the down matrix site b_p, with gamma_p from Eq. (25).  The on-site Hubbard model is the identity table
   // (pair p = site p, N_corr = Nc, one gamma), so every kernel goes through these tables.
   int n_pairs;
+  int onsite;                 // 1: the on-site model (identity tables): the accessors below answer from the four constants
+  double egm, egp, iem_m, iem_p;   //    e^{-gamma}, e^{+gamma}, 1/(e^{-gamma} - 1), 1/(e^{+gamma} - 1) of that model
   const int32_t* pair_site;   // [2][n_pairs]  site of the up / down electron of pair p
   const double* pair_E;       // [2][n_pairs]  E for sigma*s = +1 (e^{-gamma_p}), then for sigma*s = -1 (e^{+gamma_p})
   const double* pair_iem1;    // [2][n_pairs]  1 / (E - 1) for the same two cases
@@ -106,12 +108,30 @@ struct DevCtx {
   }
   // sigma = +1 for sidx 0 (up), -1 for sidx 1; E = exp(-gamma_p sigma s)
   __device__ __forceinline__ double E(int sidx, int s, int p) const {
-    return __ldg(pair_E + (((sidx == 0) == (s > 0)) ? 0 : n_pairs) + p);
+    const bool minus = (sidx == 0) == (s > 0);
+    if (onsite) return minus ? egm : egp;
+    return __ldg(pair_E + (minus ? 0 : n_pairs) + p);
   }
   __device__ __forceinline__ double iem1(int sidx, int s, int p) const {   // 1 / (E - 1)
-    return __ldg(pair_iem1 + (((sidx == 0) == (s > 0)) ? 0 : n_pairs) + p);
+    const bool minus = (sidx == 0) == (s > 0);
+    if (onsite) return minus ? iem_m : iem_p;
+    return __ldg(pair_iem1 + (minus ? 0 : n_pairs) + p);
   }
-  __device__ __forceinline__ int site(int sidx, int p) const { return __ldg(pair_site + sidx * n_pairs + p); }
+  __device__ __forceinline__ int site(int sidx, int p) const { return onsite ? p : __ldg(pair_site + sidx * n_pairs + p); }
+  // compile-time forms for the latency-critical S3 kernels (instantiated once per model class)
+  template <bool ON> __device__ __forceinline__ double Et(int sidx, int s, int p) const {
+    const bool minus = (sidx == 0) == (s > 0);
+    if (ON) return minus ? egm : egp;
+    return __ldg(pair_E + (minus ? 0 : n_pairs) + p);
+  }
+  template <bool ON> __device__ __forceinline__ double iem1t(int sidx, int s, int p) const {
+    const bool minus = (sidx == 0) == (s > 0);
+    if (ON) return minus ? iem_m : iem_p;
+    return __ldg(pair_iem1 + (minus ? 0 : n_pairs) + p);
+  }
+  template <bool ON> __device__ __forceinline__ int sitet(int sidx, int p) const { return ON ? p : __ldg(pair_site + sidx * n_pairs + p); }
+  // pair index of an extended slot, for the E / site accessors (not needed, hence not loaded, in the on-site model)
+  __device__ __forceinline__ int pair_of(const int32_t* pairs, int slot) const { return onsite ? 0 : pairs[slot]; }
   // displacement index between the sites two vertices (pairs pi, pj) occupy in spin sector sidx
   __device__ __forceinline__ int pdisp(int sidx, int pi, int pj) const { return disp(site(sidx, pi), site(sidx, pj)); }
   __device__ __forceinline__ int disp(int i, int j) const {
