@@ -41,7 +41,7 @@ FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the flush kernel from the committed `ncu --set full`
 # capture of the SAME launch configuration, keyed (config, walkers per launch, delay): bytes per launch; absent = not
 # captured (the field is null then)
-FLUSH_TRAFFIC = {}
+FLUSH_TRAFFIC = {("cfg4_6x6_b20", 2, 64): 139.66e6}   # profiles/r2_flush_cand_full.md (third captured launch, k ~ 1700)
 
 
 def measured_peaks():
@@ -252,7 +252,7 @@ def run_reference(args):
 
 # --------------------------------------------------------------------------------------------
 def total_stats(W, n_walkers):
-    keys = ("proposals", "acc_ins", "acc_rem", "flops_cand", "flops_flush", "flops_usinv", "flops_rebuild",
+    keys = ("proposals", "acc_ins", "acc_rem", "flops_cand", "flops_cand_alg", "flops_flush", "flops_usinv", "flops_rebuild",
             "flushes", "sum_rank", "blocks", "sum_k", "sweeps", "rebuilds", "guard_ends", "acc_flip")
     tot = {k: 0.0 for k in keys}
     ks = []
@@ -363,8 +363,9 @@ def run_gpu(args):
         fl = tim["flush_gemm"]
         flush_tf = dk["flops_flush"] / (fl["ms"] * 1e-3) / 1e12 if fl["ms"] > 0 else 0.0
         per_launch_flops = dk["flops_flush"] / max(fl["launches"], 1)
-        roofline = {"kernel": "gemm_flush_kernel<64,64,2,2,2,5,DescFlush> (S4 rank-r flush, DMMA m8n8k4; 64x64 tiles at 5 CTAs/SM "
-                              "for k > 512, 8-warp 64x64 tiles below)", "bound": "tensor",
+        roofline = {"kernel": "gemm_tma_flush_kernel<2,4,TDescFlush> (S4 rank-r flush: DMMA m8n8k4 on 64x64 tiles, operand tiles "
+                              "staged by TMA through a 2-stage mbarrier ring, 4 CTAs/SM, compaction gather into the accumulators)",
+                    "bound": "tensor",
                     "achieved": flush_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flush_tf / fp64_peak if fp64_peak else None,
                     "traffic": FLUSH_TRAFFIC.get((cfg["name"], B // G, delay)),
                     "algorithmic_bytes": 2 * (B // G) * 16.0 * (s2["k_mean"] ** 2),   # read + write of N, both spins
@@ -389,10 +390,14 @@ def run_gpu(args):
                  "rebuild_all_groups_concurrent_tflops": rebuild_concurrent_flops / (rebuild_concurrent_ms * 1e-3) / 1e12
                  if rebuild_concurrent_ms > 0 else 0.0}
         cand_tf = other["cand_gemm_tflops"]
-        roofline_s2 = {"kernel": "gemm_grouped_kernel<DescCandRows/Cols[SK]> (S2 candidate products, the largest share of a "
-                                 "large-k step; ncu: DMMA pipe 81 % busy, profiles/r1_v4_kernels_full.md)",
-                       "bound": "tensor", "achieved": cand_tf, "peak": fp64_peak, "unit": "TFLOP/s",
-                       "frac": cand_tf / fp64_peak if fp64_peak else None}
+        cand_alg_tf = dk["flops_cand_alg"] / (tim["cand_gemm"]["ms"] * 1e-3) / 1e12 if tim["cand_gemm"]["ms"] > 0 else 0.0
+        roofline_s2 = {"kernel": "gemm_tma_kernel<TDescCandRows/TDescCandCols> (S2 candidate products, the largest share of a "
+                                 "large-k step)", "bound": "tensor",
+                       "achieved": cand_alg_tf, "peak": fp64_peak, "unit": "TFLOP/s",
+                       "frac": cand_alg_tf / fp64_peak if fp64_peak else None,
+                       "counting": "SURVEY 8d: 2 m k^2 (rows) + 2 n^2 r_ins (columns of ACCEPTED inserts only), both spins",
+                       "achieved_launched": cand_tf, "frac_launched": cand_tf / fp64_peak if fp64_peak else None,
+                       "launched_counting": "2 m k^2 + 2 n^2 m: the column product covers every candidate (DESIGN.md section 2)"}
         out = {"metric": METRIC, "value": acc_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

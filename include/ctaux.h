@@ -149,6 +149,7 @@ typedef struct ctaux_stats {
   int64_t acc_flip;        /* accepted auxiliary-spin flips since reset (flip_moves = 1)              */
   int64_t monitor_rebuilds;/* rebuilds triggered by the error monitor (ctaux_params.n_tol), included in `rebuilds` */
   double err_est;          /* last forward-error estimate of this walker's N (max over the two spins; 0 = none yet)  */
+  double flops_cand_alg;   /* S2 as SURVEY 8d counts it: 2*m*k*k (rows) + 2*n*n*r_ins (columns of ACCEPTED inserts only)   */
 } ctaux_stats;
 
 /* One entry of the decision log (48 bytes). */

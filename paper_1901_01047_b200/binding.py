@@ -39,7 +39,7 @@ class _Stats(C.Structure):
                 ("flops_flush", C.c_double), ("flops_rebuild", C.c_double),
                 ("min_margin", C.c_double), ("sum_k", C.c_double), ("flops_usinv", C.c_double),
                 ("guard_ends", C.c_int64), ("acc_flip", C.c_int64), ("monitor_rebuilds", C.c_int64),
-                ("err_est", C.c_double)]
+                ("err_est", C.c_double), ("flops_cand_alg", C.c_double)]
 
 
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)

@@ -1222,6 +1222,7 @@ static void fill_stats(const ctaux_ctx* x, int w, const WalkerState& st, ctaux_s
   out->min_margin = st.min_margin; out->sum_k = st.sum_k; out->flops_usinv = st.flops_usinv;
   out->guard_ends = st.guard_ends; out->acc_flip = st.acc_flip;
   out->monitor_rebuilds = x->mon_rebuilds[w]; out->err_est = x->last_est[w];
+  out->flops_cand_alg = st.flops_cand_alg;
 }
 
 int ctaux_get_stats(ctaux_ctx* x, int32_t w, ctaux_stats* out) {

@@ -571,6 +571,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     st.log_count = log_count;
     st.min_margin = min_margin; st.sum_k += sum_k;
     st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
+      st.flops_cand_alg += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * (double)acc_ins);   // columns of accepted inserts only
     st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);
     st.flops_usinv += 2.0 * (2.0 * (double)kcur * r * r);
     if (status) st.status = status;

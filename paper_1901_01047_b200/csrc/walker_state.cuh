@@ -48,7 +48,7 @@ struct WalkerState {
   int32_t pad0;
   // statistics
   int64_t acc_ins, acc_rem, sweeps, blocks, flushes, rebuilds, sum_rank, log_count, guard_ends, acc_flip;
-  double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k, flops_usinv;
+  double flops_cand, flops_flush, flops_rebuild, min_margin, sum_k, flops_usinv, flops_cand_alg;
 };
 
 // Everything a kernel needs: passed by value (fits the 4 KB parameter space easily).
