@@ -417,32 +417,32 @@ def run_gpu(args):
 
 
 def run_e2e(W, cfg, B, S, steps, rank):
-    """Same metric through the public API with HOST buffers: every step uploads the walkers' state
-    from host arrays (ctaux_set_state: configuration H2D + S1/S5), runs ctaux_sweep(S) and reads the
-    result back (ctaux_get_config + ctaux_get_N of every walker, D2H)."""
+    """Same metric through the C ABI with HOST buffers: every step uploads the walkers' state from packed host arrays
+    (ctaux_set_state: configuration H2D + S1/S5 on the device), runs ctaux_sweep(S) and reads the result back into
+    pinned host buffers (ctaux_get_config_all + ctaux_get_stats_all + ctaux_get_N_all, D2H).  The binding's packed forms
+    are used (the arrays the C ABI itself takes), so no per-walker Python runs inside the timed region."""
     import torch
     seeds = np.arange(rank * B, rank * B + B, dtype=np.uint64)
-    cfgs, stats, _ = W.fetch_all(with_N=True)     # untimed: also allocates the pinned staging buffers
-    del _
+    states = W.get_state_packed(with_N=True)      # untimed: also allocates the pinned staging buffers
     acc = 0
     h2d = d2h = 0
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(steps):
-        W.set_state(seeds, cfgs, [s["next_id"] for s in stats], [s["proposals"] for s in stats])
-        h2d += sum(len(c["site"]) * (8 + 4 + 8 + 1) for c in cfgs) + 8 * B * 4
+        h2d += sum(int(st["k"].sum()) * (8 + 4 + 8 + 1) + len(st["k"]) * (4 + 8 + 8 + 8) for st in states)
+        W.set_state_packed(seeds, states)
         W.sweep(S)
-        cfgs, new_stats, Ns = W.fetch_all(with_N=True)
-        for st in new_stats:
-            acc += st["acc_ins"] + st["acc_rem"] + st["acc_flip"]      # counters restart at set_state
-            d2h += st["k"] * (8 + 4 + 8 + 1) + 2 * st["k"] * st["k"] * 8
-        del Ns
-        stats = new_stats
+        states = W.get_state_packed(with_N=True)
+        for st in states:
+            s_ = st["stats"]
+            acc += int(s_["acc_ins"].sum() + s_["acc_rem"].sum() + s_["acc_flip"].sum())      # counters restart at set_state
+            kk = st["k"].astype(np.int64)
+            d2h += int((kk * (8 + 4 + 8 + 1) + 2 * kk * kk * 8).sum()) + len(kk) * 4 + s_.nbytes
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     return {"value": acc / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d / steps), "d2h_bytes_per_step": int(d2h / steps),
             "steps": steps, "ms_per_step": 1e3 * dt / steps,
-            "what": "ctaux_set_state(host arrays) + ctaux_sweep + ctaux_get_config_all/get_N_all to pinned host buffers, every step"}
+            "what": "ctaux_set_state(packed host arrays) + ctaux_sweep + ctaux_get_config_all/get_stats_all/get_N_all into pinned host buffers, every step"}
 
 
 def main():

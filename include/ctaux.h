@@ -186,6 +186,12 @@ int ctaux_set_state(ctaux_ctx* ctx, const uint64_t* seeds, const int32_t* k, con
  * (S2, S3, S4 per block; S5 every rebuild_every sweeps).  Continues each walker's stream. */
 int ctaux_sweep(ctaux_ctx* ctx, int32_t n_sweeps);
 
+/* Advance every walker by exactly n_proposals proposals (a partial sweep): the chain is a function of the proposal
+ * counter only (Philox counter = p), so splitting it this way changes nothing but where blocks end.  For
+ * callers that measure or check between sweeps; counted as one sweep in ctaux_stats.sweeps, does not advance the
+ * rebuild cadence (rebuild_every counts ctaux_sweep sweeps); N is held to n_tol at return like after ctaux_sweep. */
+int ctaux_propose(ctaux_ctx* ctx, int32_t n_proposals);
+
 /* From-scratch rebuild of every walker's N from its configuration (S1 + S5), now. */
 int ctaux_rebuild(ctaux_ctx* ctx);
 

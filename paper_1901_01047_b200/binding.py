@@ -44,7 +44,7 @@ class _Stats(C.Structure):
 
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
-           "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
+           "ctaux_propose", "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
            "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_g0_workspace_bytes", "ctaux_g0_table", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
 TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
@@ -72,6 +72,7 @@ def load_library():
     L.ctaux_reset.argtypes = [vp, vp]
     L.ctaux_set_state.argtypes = [vp] + [vp] * 8
     L.ctaux_sweep.argtypes = [vp, i32]
+    L.ctaux_propose.argtypes = [vp, i32]
     L.ctaux_rebuild.argtypes = [vp]
     L.ctaux_get_config.argtypes = [vp, i32, C.POINTER(i32), vp, vp, vp, vp, i32]
     L.ctaux_get_N.argtypes = [vp, i32, i32, vp, i32]
@@ -217,6 +218,10 @@ class Walkers:
         with self._torch.cuda.device(self.device):
             _check(self._L.ctaux_sweep(self._h, int(n_sweeps)), "ctaux_sweep")
 
+    def propose(self, n_proposals):
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_propose(self._h, int(n_proposals)), "ctaux_propose")
+
     def rebuild(self):
         with self._torch.cuda.device(self.device):
             _check(self._L.ctaux_rebuild(self._h), "ctaux_rebuild")
@@ -269,6 +274,42 @@ class Walkers:
             out.append(tuple(flat[(2 * w + s) * mk * mk:(2 * w + s) * mk * mk + k * k].reshape((k, k), order="F")
                              for s in range(2)))
         return out
+
+    # ---- the C ABI's own batched forms: packed [B][max_k] arrays in pinned host memory, no per-walker Python
+    def get_state_packed(self, with_N=True):
+        """ctaux_get_config_all + ctaux_get_stats_all (+ ctaux_get_N_all) into pinned host buffers owned by this object
+        (overwritten by the next call): dict(k [B], id/site/tau/spin [B][max_k], stats: structured array of
+        ctaux_stats [B], N: flat buffer in ctaux_get_N_all's layout or None)."""
+        t, B, mk = self._torch, self.n_walkers, self.max_k
+        if getattr(self, "_pk", None) is None:
+            pin = lambda n, dt: t.empty(n, dtype=dt, pin_memory=True).numpy()
+            self._pk = dict(k=pin(B, t.int32), id=pin(B * mk, t.int64).view(np.uint64).reshape(B, mk),
+                            site=pin(B * mk, t.int32).reshape(B, mk), tau=pin(B * mk, t.float64).reshape(B, mk),
+                            spin=pin(B * mk, t.int8).reshape(B, mk))
+            self._pk_stats = (_Stats * B)()
+        pk = self._pk
+        with t.cuda.device(self.device):
+            _check(self._L.ctaux_get_config_all(self._h, pk["k"].ctypes.data, pk["id"].ctypes.data, pk["site"].ctypes.data,
+                                                pk["tau"].ctypes.data, pk["spin"].ctypes.data), "ctaux_get_config_all")
+            _check(self._L.ctaux_get_stats_all(self._h, C.addressof(self._pk_stats)), "ctaux_get_stats_all")
+            N = None
+            if with_N:
+                if getattr(self, "_pin_all", None) is None:
+                    self._pin_all = t.empty(B * 2 * mk * mk, dtype=t.float64, pin_memory=True)
+                N = self._pin_all.numpy()
+                _check(self._L.ctaux_get_N_all(self._h, N.ctypes.data), "ctaux_get_N_all")
+        return dict(pk, stats=np.ctypeslib.as_array(self._pk_stats), N=N)
+
+    def set_state_packed(self, seeds, st):
+        """ctaux_set_state from packed host arrays (the dict get_state_packed returns: the chain continues from
+        st["stats"]["next_id"] / ["proposals"])."""
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        next_id = np.ascontiguousarray(st["stats"]["next_id"], dtype=np.uint64)
+        prop = np.ascontiguousarray(st["stats"]["proposals"], dtype=np.uint64)
+        with self._torch.cuda.device(self.device):
+            _check(self._L.ctaux_set_state(self._h, seeds.ctypes.data, st["k"].ctypes.data, st["id"].ctypes.data,
+                                           st["site"].ctypes.data, st["tau"].ctypes.data, st["spin"].ctypes.data,
+                                           next_id.ctypes.data, prop.ctypes.data), "ctaux_set_state")
 
     def get_N_device(self, w, spin):
         torch = self._torch
@@ -371,6 +412,9 @@ class WalkerGroups:
     def sweep(self, n_sweeps):
         self._each(lambda W, g: W.sweep(n_sweeps))
 
+    def propose(self, n_proposals):
+        self._each(lambda W, g: W.propose(n_proposals))
+
     def rebuild(self):
         self._each(lambda W, g: W.rebuild())
 
@@ -412,6 +456,20 @@ class WalkerGroups:
 
         self._each(one)
         return cfgs, stats, Ns
+
+    def get_state_packed(self, with_N=True):
+        """Per stream group, concurrently: list of the dicts Walkers.get_state_packed returns."""
+        out = [None] * len(self.groups)
+
+        def one(W, g):
+            out[g] = W.get_state_packed(with_N)
+
+        self._each(one)
+        return out
+
+    def set_state_packed(self, seeds, states):
+        seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
+        self._each(lambda W, g: W.set_state_packed(seeds[g * self.per:(g + 1) * self.per], states[g]))
 
     def timing_enable(self, on=True):
         for W in self.groups:

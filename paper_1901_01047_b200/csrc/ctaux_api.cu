@@ -267,6 +267,7 @@ struct ctaux_ctx {
   AccCtx acc;         // S6 accumulator (accumulator.cuh); acc.n_omega == 0: off
   int acc_smem;
   PackedCfg pk;       // device staging of the packed configurations
+  double* nstage = nullptr;   // device staging of ctaux_get_N_all (small matrices only)
   uint64_t *pk_next, *pk_p;
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
@@ -284,7 +285,7 @@ namespace {
 struct Layout {
   size_t table, ws, cfg_site, cfg_tau, cfg_spin, cfg_id, prop, Nbuf, Bm, gxC, Gx, Um, Ut, Vt, Sinv, J,
       rowmap, log, n_active, colbuf, rowbuf, perm, detsign, seeds, skbuf, Tbuf, resid, mon, est, tmaps,
-      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, lu_inv, lu_tmp, lu_pos, pair_site, pair_E, pair_iem1, total;
+      pk_k, pk_id, pk_site, pk_tau, pk_spin, pk_next, pk_p, acc_grid, acc_tab, acc_phi, acc_scal, acc_start, acc_list, acc_out, lu_inv, lu_tmp, lu_pos, pair_site, pair_E, pair_iem1, nstage, total;
 };
 
 bool derive_sizes(const ctaux_params* p, DevCtx& d) {
@@ -336,6 +337,13 @@ bool acc_sizes(const ctaux_params* p, AccSizes& a) {
   if (p->n_omega < 0 || p->nfft_oversampling < 0 || p->nfft_window < 0) return false;
   if (p->n_omega == 0) return true;
   return a.m >= 2 && a.w >= 1 && 2 * a.w <= 32 && a.L >= 4 * a.w && a.L <= 16384;
+}
+
+// ctaux_get_N_all with many small matrices: the live blocks are packed on the device into the HOST layout and leave
+// in one 2-D copy instead of 2B small ones (256 walkers of config 2: 512 copies of 30 KB)
+size_t nstage_bytes(const DevCtx& d) {
+  const size_t b = (size_t)d.B * 2 * (size_t)d.max_k * d.max_k * 8;
+  return (d.B >= 16 && b <= ((size_t)256 << 20)) ? b : 0;
 }
 
 Layout make_layout(const DevCtx& d, const AccSizes& ac) {
@@ -392,6 +400,7 @@ Layout make_layout(const DevCtx& d, const AccSizes& ac) {
   L.pair_site = take(2 * (size_t)d.n_pairs * 4);
   L.pair_E = take(2 * (size_t)d.n_pairs * 8);
   L.pair_iem1 = take(2 * (size_t)d.n_pairs * 8);
+  L.nstage = take(nstage_bytes(d));
   L.total = o;
   return L;
 }
@@ -546,7 +555,7 @@ int do_rebuild(ctaux_ctx* x, bool set_sign, bool count) {
     }
     const int cb = grid_for((size_t)2 * kmax, 128, 64);
     int* dsg = set_sign ? x->detsign : nullptr;
-    const int tri_smem = kLuOuter * (kLuOuter + 1) * 8;
+    const int tri_smem = kTriSmemDoubles * 8;
     static SmemOptIn optin_tri;
     CU_CHECK(optin_tri.ensure(k_lu_tri_inv, tri_smem));
     auto gemm2 = [&](int J0, int j0, int wa, int wb, int Mmax, int Nmax) -> cudaError_t {
@@ -706,7 +715,7 @@ int enqueue_block_step(ctaux_ctx* x) {
   return CTAUX_OK;
 }
 
-int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
+int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps, int n_props = 0) {
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
   bool resume = false;   // true: walkers spilled by the fused kernel continue on the delayed path
@@ -714,8 +723,8 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
     CU_CHECK(cudaMemsetAsync(d.n_active, 0, 2 * sizeof(int), s));
     {
       Scoped t(x, C_PROPOSE);
-      if (d.onsite) k_walk_fused<true><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
-      else k_walk_fused<false><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, x->fcap);
+      if (d.onsite) k_walk_fused<true><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, n_props, x->fcap);
+      else k_walk_fused<false><<<d.B, kFusedThreads, x->fused_smem, s>>>(d, n_sweeps, n_props, x->fcap);
       tick(x, C_PROPOSE);
       x->n_fresh = false;
     }
@@ -734,12 +743,12 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps) {
     x->k_hint = d.max_k;
   }
   if (!resume) {
-    k_begin_sweeps<<<(d.B + 127) / 128, 128, 0, s>>>(d, n_sweeps);
+    k_begin_sweeps<<<(d.B + 127) / 128, 128, 0, s>>>(d, n_sweeps, n_props);
     tick(x, C_OTHER);
   }
   const int steps_per_poll = 8;
   // every block consumes at least one proposal and a sweep has at most max(16, max_k) of them
-  const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + steps_per_poll;
+  const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + n_props + steps_per_poll;
   for (long long done = 0;; done += steps_per_poll) {
     if (done > max_steps) return CTAUX_ESTATE;
     for (int i = 0; i < steps_per_poll; ++i) {
@@ -858,6 +867,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   }
   x->pk.k = (int32_t*)(base + L.pk_k); x->pk.id = (uint64_t*)(base + L.pk_id); x->pk.site = (int32_t*)(base + L.pk_site);
   x->pk.tau = (double*)(base + L.pk_tau); x->pk.spin = (int8_t*)(base + L.pk_spin);
+  x->nstage = nstage_bytes(d) ? (double*)(base + L.nstage) : nullptr;
   x->pk_next = (uint64_t*)(base + L.pk_next); x->pk_p = (uint64_t*)(base + L.pk_p);
   x->lu_inv = (double*)(base + L.lu_inv); x->lu_tmp = (double*)(base + L.lu_tmp); x->lu_pos = (int32_t*)(base + L.lu_pos);
   x->mon = (double*)(base + L.mon);
@@ -999,8 +1009,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
   x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
   if (d.max_k > 512) {
     const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
-    // panel width 32: width 64 (k_lu_panel_cl<64>, k_lu_trsm<64>) was measured at the same total time -- the rank-64
-    // trailing updates save 17 %, the wider panel and triangular solves cost it again (profiles/r1_v4_kernels_full.md)
+    // panel width 32 inside outer blocks of 128 (rebuild_lu.cuh); a 64-wide panel was measured at the same total time
     const int need32 = lu_cl_smem_doubles(rl_cap, 32) * 8 + 64;
     static SmemOptIn optin_lu;
     if (need32 <= max_smem && optin_lu.ensure(k_lu_panel_cl<32>, need32) == cudaSuccess) {
@@ -1098,6 +1107,24 @@ int ctaux_rebuild(ctaux_ctx* x) {
   return do_rebuild(x, false, true);
 }
 
+// what the caller reads after a ctaux_sweep / ctaux_propose call is held to n_tol: estimate the forward error of every N
+// and rebuild the context when the estimate (safety factor 3 for the variance of the 4-probe estimator) says so
+static int end_of_call_check(ctaux_ctx* x) {
+  if (x->n_tol > 0.0 && !x->n_fresh) {
+    int rc = enqueue_err_probe(x);
+    if (rc) { x->have_state = false; return rc; }
+    CU_CHECK(cudaStreamSynchronize(x->stream));
+    harvest_timing(x);
+    if (harvest_err_probe(x) > x->n_tol / 3.0) {
+      rc = do_rebuild(x, false, true);
+      if (rc) { x->have_state = false; return rc; }
+      for (int w = 0; w < x->d.B; ++w) x->mon_rebuilds[w] += 1;
+      x->sweeps_since_rebuild = 0;
+    }
+  }
+  return CTAUX_OK;
+}
+
 int ctaux_sweep(ctaux_ctx* x, int32_t n_sweeps) {
   if (!x || n_sweeps < 0) return CTAUX_EINVAL;
   if (!x->have_state) return CTAUX_ESTATE;
@@ -1119,21 +1146,16 @@ int ctaux_sweep(ctaux_ctx* x, int32_t n_sweeps) {
       x->sweeps_since_rebuild = 0;
     }
   }
-  // what the caller reads after this call is held to n_tol: estimate the forward error of every N and rebuild the
-  // context when the estimate (safety factor 3 for the variance of the 4-probe estimator) says it is needed
-  if (x->n_tol > 0.0 && !x->n_fresh) {
-    int rc = enqueue_err_probe(x);
-    if (rc) { x->have_state = false; return rc; }
-    CU_CHECK(cudaStreamSynchronize(x->stream));
-    harvest_timing(x);
-    if (harvest_err_probe(x) > x->n_tol / 3.0) {
-      rc = do_rebuild(x, false, true);
-      if (rc) { x->have_state = false; return rc; }
-      for (int w = 0; w < x->d.B; ++w) x->mon_rebuilds[w] += 1;
-      x->sweeps_since_rebuild = 0;
-    }
-  }
-  return CTAUX_OK;
+  return end_of_call_check(x);
+}
+
+int ctaux_propose(ctaux_ctx* x, int32_t n_proposals) {
+  if (!x || n_proposals < 0) return CTAUX_EINVAL;
+  if (!x->have_state) return CTAUX_ESTATE;
+  if (n_proposals == 0) return CTAUX_OK;
+  int rc = run_sweeps_chunk(x, 0, n_proposals);
+  if (rc) { x->have_state = false; return rc; }
+  return end_of_call_check(x);
 }
 
 int ctaux_get_config(ctaux_ctx* x, int32_t w, int32_t* k, uint64_t* id, int32_t* site, double* tau,
@@ -1200,6 +1222,18 @@ int ctaux_get_N_all(ctaux_ctx* x, double* N) {
   CU_CHECK(cudaStreamSynchronize(x->stream));
   std::vector<WalkerState> h(d.B);
   CU_CHECK(cudaMemcpy(h.data(), d.ws, sizeof(WalkerState) * d.B, cudaMemcpyDeviceToHost));
+  if (x->nstage) {
+    int kmax = 0;
+    for (int w = 0; w < d.B; ++w) kmax = h[w].k > kmax ? h[w].k : kmax;
+    if (kmax == 0) return CTAUX_OK;
+    k_pack_N<<<dim3(grid_for((size_t)kmax * kmax, 256, 8), 2 * d.B), 256, 0, x->stream>>>(d, x->nstage);
+    tick(x, C_OTHER);
+    CU_CHECK(cudaGetLastError());
+    const size_t pitch = (size_t)d.max_k * d.max_k * 8;
+    CU_CHECK(cudaMemcpy2DAsync(N, pitch, x->nstage, pitch, (size_t)kmax * kmax * 8, 2 * (size_t)d.B, cudaMemcpyDeviceToHost, x->stream));
+    CU_CHECK(cudaStreamSynchronize(x->stream));
+    return CTAUX_OK;
+  }
   for (int w = 0; w < d.B; ++w) {
     const int kw = h[w].k;
     if (kw == 0) continue;

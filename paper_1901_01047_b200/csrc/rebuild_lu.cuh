@@ -1,19 +1,13 @@
-// S5: from-scratch rebuild  N_sigma = A_sigma^{-1}  by blocked right-looking LU with partial
-// pivoting, batched over all B*2 matrices (each with its own order k), followed by blocked
-// forward / backward substitution on the identity.  BASELINE.json: "a batched LU-based rebuild".
+// S5: from-scratch rebuild  N_sigma = A_sigma^{-1}  by a two-level blocked right-looking LU with partial pivoting,
+// batched over all B*2 matrices (each with its own order k).  BASELINE.json: "a batched LU-based rebuild".
 //
 //   F = the non-current N buffer (A, overwritten by its LU factors: P A = L U)
-//   X = the current N buffer     (starts as I; row swaps make it P; then L^-1 P; then U^-1 L^-1 P)
+//   X = the current N buffer     (starts as I; becomes X' = L^-1 in position space, then N' = U^-1 X'; N = N' P)
 //
-// Per panel [j0, j1) of kLuNb columns:
-//   k_lu_panel : unblocked LU of the panel with partial pivoting (one CTA per matrix)
-//   k_lu_swap  : the panel's row interchanges applied to F outside the panel and to all of X
-//   k_lu_trsm  : rows j0..j1 of F (right of the panel) and of X  <-  L11^-1 * (those rows)
-//   GEMM       : trailing update of F (A22 -= L21 U12) and of X (X_below -= L21 X_panel)
-// Backward pass, panels from last to first:
-//   k_lu_trsm (upper) : X[j0:j1, :] <- U11^-1 X[j0:j1, :]
-//   GEMM              : X[0:j0, :] -= U[0:j0, j0:j1] X[j0:j1, :]
-// The trailing updates run on the DMMA GEMM tiles of gemm_dmma.cuh.
+// Kernels: k_lu_panel / k_lu_panel_cl (unblocked LU of a 32-column panel: one CTA, or an 8-CTA cluster per matrix),
+// k_lu_swap_range, k_lu_trsm_range (inside the outer block of 128 columns), k_lu_tri_inv (explicit 128 x 128 triangular
+// inverses), k_lu_copyback, k_lu_perm / k_lu_scatter_cols / k_lu_flip; the rank-32 and rank-128 updates (TDescLU2) run on
+// the TMA-staged DMMA tiles of gemm_tma.cuh.  The blocking is described above kLuOuter below.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -122,7 +116,7 @@ __host__ __device__ inline int lu_cl_smem_doubles(int rl_cap, int nbw) {
   return rl_cap * (nbw + 1) + 2 * kLuCl * (nbw + 2) + 2 * nbw;
 }
 
-template <int NB>   // panel width: 64 when the slabs fit shared memory (config 4), else 32
+template <int NB>   // panel width (32 in use)
 __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     k_lu_panel_cl(DevCtx c, int j0, int* detsign, int rl_cap) {
   constexpr int kLuNb = NB, kLuPad = NB + 1, kLuMsg = NB + 2;   // (shadow the file-level panel width)
@@ -259,132 +253,6 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
   }
 }
 
-// one thread per column: apply the panel's interchanges to F (outside the panel) and to X (all columns)
-template <int NB>
-__global__ void k_lu_swap(DevCtx c, int j0) {
-  constexpr int kLuNb = NB;
-  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
-  const WalkerState& st = c.ws[w];
-  const int k = st.k;
-  if (j0 >= k) return;
-  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
-  const int* ipiv = c.perm + ((size_t)w * 2 + sp) * c.ld;
-  double* F = c.N(w, sp, st.n_cur ^ 1);
-  double* X = c.N(w, sp, st.n_cur);
-  __shared__ int s_piv[kLuNb];
-  if (threadIdx.x < j1 - j0) s_piv[threadIdx.x] = ipiv[j0 + threadIdx.x];
-  __syncthreads();
-  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < 2 * k; t += gridDim.x * blockDim.x) {
-    double* col;
-    if (t < k) {
-      if (t >= j0 && t < j1) continue;
-      col = F + (size_t)t * c.ld;
-    } else {
-      col = X + (size_t)(t - k) * c.ld;
-    }
-    for (int q = 0; q < j1 - j0; ++q) {
-      const int p = s_piv[q];
-      if (p != j0 + q) {
-        const double a = col[j0 + q], b = col[p];
-        col[j0 + q] = b;
-        col[p] = a;
-      }
-    }
-  }
-}
-
-// Triangular solves with the kLuNb x kLuNb diagonal block, one thread per right-hand-side column.
-//   upper == 0: rows j0..j1 of F (columns >= j1) and of X (all columns)  <-  L11^-1 (unit lower)
-//   upper == 1: rows j0..j1 of X (all columns)                           <-  U11^-1
-template <int NB>
-__global__ void __launch_bounds__(128) k_lu_trsm(DevCtx c, int j0, int upper) {
-  constexpr int kLuNb = NB;
-  const int w = blockIdx.y >> 1, sp = blockIdx.y & 1;
-  const WalkerState& st = c.ws[w];
-  const int k = st.k;
-  if (j0 >= k) return;
-  const int j1 = (j0 + kLuNb < k) ? j0 + kLuNb : k;
-  const int nb = j1 - j0, ld = c.ld;
-  double* F = c.N(w, sp, st.n_cur ^ 1);
-  double* X = c.N(w, sp, st.n_cur);
-  __shared__ double T[kLuNb][kLuNb + 1];
-  for (int idx = threadIdx.x; idx < nb * nb; idx += blockDim.x) {
-    const int i = idx % nb, j = idx / nb;
-    T[i][j] = F[(size_t)(j0 + j) * ld + j0 + i];
-  }
-  __syncthreads();
-  const int ncolF = upper ? 0 : (k - j1);
-  const int total = ncolF + k;
-  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
-    double* col = (t < ncolF) ? (F + (size_t)(j1 + t) * ld + j0) : (X + (size_t)(t - ncolF) * ld + j0);
-    double x[kLuNb];
-#pragma unroll
-    for (int i = 0; i < kLuNb; ++i) x[i] = (i < nb) ? col[i] : 0.0;
-    if (!upper) {
-#pragma unroll
-      for (int i = 0; i < kLuNb; ++i) {
-        if (i < nb) {
-          double s = x[i];
-#pragma unroll
-          for (int l = 0; l < kLuNb; ++l)
-            if (l < i) s -= T[i][l] * x[l];
-          x[i] = s;
-        }
-      }
-    } else {
-#pragma unroll
-      for (int i = kLuNb - 1; i >= 0; --i) {
-        if (i < nb) {
-          double s = x[i];
-#pragma unroll
-          for (int l = 0; l < kLuNb; ++l)
-            if (l > i && l < nb) s -= T[i][l] * x[l];
-          x[i] = s / T[i][i];
-        }
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < kLuNb; ++i)
-      if (i < nb) col[i] = x[i];
-  }
-}
-
-// GEMM descriptors of the trailing updates (alpha = -1, beta = 1, in place)
-struct TDescLU {   // operands by tensor map + tile origin (gemm_tma.cuh); j0, j1 are multiples of the panel width 32
-  DevCtx c;
-  int j0, which, nb;
-  __device__ bool operator()(int prob, TmaGemmDesc& d) const {
-    const int w = prob >> 1, sp = prob & 1;
-    const WalkerState& st = c.ws[w];
-    const int k = st.k;
-    if (j0 >= k) return false;
-    const int j1 = (j0 + nb < k) ? j0 + nb : k;
-    const size_t ld = c.ld;
-    const int fb = st.n_cur ^ 1, xb = st.n_cur;     // F = the non-current buffer, X = the current one
-    double* F = c.N(w, sp, fb);
-    double* X = c.N(w, sp, xb);
-    d.K = j1 - j0;
-    d.ldc = c.ld; d.ldc0 = c.ld; d.rowmap = nullptr; d.colmap = nullptr; d.alpha = -1.0; d.beta = 1.0;
-    d.tmA = c.tm(w, sp, fb ? TM_N1_M : TM_N0_M); d.a_k0 = j0;
-    d.b_k0 = j0;
-    if (which == 0) {
-      d.M = k - j1; d.N = k - j1; d.a_m0 = j1;
-      d.tmB = c.tm(w, sp, fb ? TM_N1_K : TM_N0_K); d.b_n0 = j1;
-      d.C = F + j1 + (size_t)j1 * ld;
-    } else if (which == 1) {
-      d.M = k - j1; d.N = k; d.a_m0 = j1;
-      d.tmB = c.tm(w, sp, xb ? TM_N1_K : TM_N0_K); d.b_n0 = 0;
-      d.C = X + j1;
-    } else {
-      d.M = j0; d.N = k; d.a_m0 = 0;
-      d.tmB = c.tm(w, sp, xb ? TM_N1_K : TM_N0_K); d.b_n0 = 0;
-      d.C = X;
-    }
-    d.C0 = d.C;
-    return d.M > 0 && d.N > 0;
-  }
-};
-
 // ---- rebuild_mode 1: Newton-Schulz refresh  N <- N (2 - A N) = 2 N - N (A N)
 // A_sigma is built (k_build_A) into the spare N buffer; T = A N goes to Tbuf; the new N overwrites A.
 struct TDescNS {
@@ -443,9 +311,9 @@ __global__ void k_ns_flip(DevCtx c) {
 namespace ctaux {
 
 // ===================================================================================================================
-// Two-level blocking of the rebuild (round 2).  The one-level right-looking LU above updates the whole trailing matrix
-// with rank kLuNb = 32 after every panel: arithmetic intensity 4 flop/B, the HBM side of the FP64 ridge (5.4), and the
-// forward substitution ran over the structural zeros of the identity.  Now:
+// Two-level blocking of the rebuild.  A one-level right-looking LU updates the whole trailing matrix with rank
+// kLuNb = 32 after every panel: arithmetic intensity 4 flop/B, the HBM side of the FP64 ridge (5.4), and the
+// forward substitution over X = L^-1 P runs over the structural zeros of the identity.  Instead:
 //   * panels of 32 columns are factorised as before (partial pivoting over the full height), but their rank-32 updates
 //     touch only the columns of the current OUTER block of kLuOuter = 128 columns;
 //   * once per outer block: the block's 128 interchanges are applied to the rest, the 128 x 128 unit-lower block L11 is
@@ -531,9 +399,20 @@ __global__ void __launch_bounds__(128) k_lu_trsm_range(DevCtx c, int j0, int c0,
 
 // explicit inverse of the diagonal block of F at J0 (size nbk = min(128, k - J0)) into Linv [128 x 128], column-major,
 // leading dimension 128:  upper == 0: unit-lower L11;  upper == 1: upper-triangular U11 (with its diagonal).
-// Four lanes share a column of the inverse; the triangle sits in shared memory.
+// Blocked in shared memory (the column-at-a-time version spent 128 dependent global round trips per column: 107 us):
+// U11 is handled as the lower-triangular U11^T and written back transposed, so one code path inverts a lower
+// triangle T of 4 x 4 blocks of 32:
+//   1. W_bb = T_bb^-1: one warp per diagonal block, lane j carries column j of the inverse in registers;
+//   2. block sub-diagonals d = 1, 2, 3:  W_ij = -W_ii (sum_{l=j}^{i-1} T_il W_lj)   (two-sided products of 32^3).
+constexpr int kTriB = 32, kTriNb = kLuOuter / kTriB;             // 4 x 4 blocks
+constexpr int kTriLdT = kLuOuter + 1, kTriLdW = kTriB + 1;
+constexpr int kTriSmemDoubles = kLuOuter * kTriLdT + (kTriNb * (kTriNb + 1) / 2 + 1) * kTriB * kTriLdW;
+__device__ __forceinline__ int tri_blk(int i, int j) { return i * (i + 1) / 2 + j; }   // i >= j
+
 __global__ void __launch_bounds__(512) k_lu_tri_inv(DevCtx c, double* linv_all, int J0, int upper) {
-  extern __shared__ double s_T[];   // [128][129]
+  extern __shared__ double s_T[];                 // T [128][129] (row i, column j at i*129 + j)
+  double* s_W = s_T + kLuOuter * kTriLdT;        // 10 lower blocks of W [32][33] + one scratch block
+  double* s_S = s_W + (kTriNb * (kTriNb + 1) / 2) * kTriB * kTriLdW;
   const int prob = blockIdx.x, w = prob >> 1, sp = prob & 1;
   const WalkerState& st = c.ws[w];
   const int k = st.k;
@@ -541,39 +420,77 @@ __global__ void __launch_bounds__(512) k_lu_tri_inv(DevCtx c, double* linv_all, 
   const int nbk = (k - J0 < kLuOuter) ? k - J0 : kLuOuter;
   const double* F = c.N(w, sp, st.n_cur ^ 1);
   double* out = linv_all + (size_t)prob * kLuOuter * kLuOuter;
-  for (int idx = threadIdx.x; idx < kLuOuter * kLuOuter; idx += blockDim.x) {
-    const int i = idx % kLuOuter, j = idx / kLuOuter;
-    s_T[i * (kLuOuter + 1) + j] = (i < nbk && j < nbk) ? F[(size_t)(J0 + j) * c.ld + J0 + i] : 0.0;
-    out[idx] = 0.0;
+  const int tid = threadIdx.x;
+  // load the lower triangle (of L11, or of U11^T); the padding is the identity
+  for (int idx = tid; idx < kLuOuter * kLuOuter; idx += 512) {
+    const int a = idx % kLuOuter, b = idx / kLuOuter;             // element (a, b) of the stored block, a fastest
+    double v = (a < nbk && b < nbk) ? F[(size_t)(J0 + b) * c.ld + J0 + a] : (a == b ? 1.0 : 0.0);
+    const int i = upper ? b : a, j = upper ? a : b;               // T = block (lower) or block^T (upper)
+    if (i < j) v = 0.0;
+    else if (i == j && !upper) v = 1.0;                           // unit diagonal (the storage holds U's there)
+    s_T[i * kTriLdT + j] = v;
   }
   __syncthreads();
-  const int col = threadIdx.x >> 2, q = threadIdx.x & 3;
-  const unsigned qmask = 0xFu << (threadIdx.x & 28);
-  double* x = out + (size_t)col * kLuOuter;      // column `col` of the inverse, owned by this quad
-  if (col < nbk) {
-    if (!upper) {
-      if (q == 0) x[col] = 1.0;
-      __syncwarp(qmask);
-      for (int i = col + 1; i < nbk; ++i) {
-        double s = 0.0;
-        for (int l = col + q; l < i; l += 4) s += s_T[i * (kLuOuter + 1) + l] * x[l];
-        s += __shfl_xor_sync(qmask, s, 1);
-        s += __shfl_xor_sync(qmask, s, 2);
-        if (q == 0) x[i] = -s;
-        __syncwarp(qmask);
+  // 1. diagonal blocks
+  if (tid < kTriNb * 32) {
+    const int b = tid >> 5, j = tid & 31;
+    const double* Tb = s_T + (b * kTriB) * kTriLdT + b * kTriB;
+    double x[kTriB];
+#pragma unroll
+    for (int i = 0; i < kTriB; ++i) {
+      double s0 = (i == j) ? 1.0 : 0.0, s1 = 0.0;
+#pragma unroll
+      for (int l = 0; l < i; ++l) {
+        if (l & 1) s1 -= Tb[i * kTriLdT + l] * x[l];
+        else s0 -= Tb[i * kTriLdT + l] * x[l];
       }
-    } else {
-      if (q == 0) x[col] = 1.0 / s_T[col * (kLuOuter + 1) + col];
-      __syncwarp(qmask);
-      for (int i = col - 1; i >= 0; --i) {
-        double s = 0.0;
-        for (int l = i + 1 + q; l <= col; l += 4) s += s_T[i * (kLuOuter + 1) + l] * x[l];
-        s += __shfl_xor_sync(qmask, s, 1);
-        s += __shfl_xor_sync(qmask, s, 2);
-        if (q == 0) x[i] = -s / s_T[i * (kLuOuter + 1) + i];
-        __syncwarp(qmask);
-      }
+      x[i] = (s0 + s1) / Tb[i * kTriLdT + i];
     }
+    double* Wb = s_W + tri_blk(b, b) * kTriB * kTriLdW;
+#pragma unroll
+    for (int i = 0; i < kTriB; ++i) Wb[i * kTriLdW + j] = x[i];
+  }
+  __syncthreads();
+  // 2. off-diagonal blocks, sub-diagonal by sub-diagonal; thread -> (row, two columns) of a 32 x 32 block
+  const int row = tid & 31, c0 = (tid >> 5) * 2;
+  for (int dgl = 1; dgl < kTriNb; ++dgl) {
+    for (int i = dgl; i < kTriNb; ++i) {
+      const int j = i - dgl;
+      double a0 = 0.0, a1 = 0.0;
+      for (int l = j; l < i; ++l) {
+        const double* Til = s_T + (i * kTriB + row) * kTriLdT + l * kTriB;
+        const double* Wlj = s_W + tri_blk(l, j) * kTriB * kTriLdW;
+#pragma unroll 8
+        for (int q = 0; q < kTriB; ++q) {
+          const double t = Til[q];
+          a0 += t * Wlj[q * kTriLdW + c0];
+          a1 += t * Wlj[q * kTriLdW + c0 + 1];
+        }
+      }
+      s_S[row * kTriLdW + c0] = a0;
+      s_S[row * kTriLdW + c0 + 1] = a1;
+      __syncthreads();
+      const double* Wii = s_W + tri_blk(i, i) * kTriB * kTriLdW;
+      double b0 = 0.0, b1 = 0.0;
+#pragma unroll 8
+      for (int q = 0; q < kTriB; ++q) {
+        const double t = Wii[row * kTriLdW + q];
+        b0 += t * s_S[q * kTriLdW + c0];
+        b1 += t * s_S[q * kTriLdW + c0 + 1];
+      }
+      double* Wij = s_W + tri_blk(i, j) * kTriB * kTriLdW;
+      Wij[row * kTriLdW + c0] = -b0;
+      Wij[row * kTriLdW + c0 + 1] = -b1;
+      __syncthreads();
+    }
+  }
+  // write back: W (lower) or W^T (upper); zero outside the live block
+  for (int idx = tid; idx < kLuOuter * kLuOuter; idx += 512) {
+    const int a = idx % kLuOuter, b = idx / kLuOuter;             // out(a, b), a fastest
+    const int i = upper ? b : a, j = upper ? a : b;
+    double v = 0.0;
+    if (i >= j && a < nbk && b < nbk) v = s_W[tri_blk(i >> 5, j >> 5) * kTriB * kTriLdW + (i & 31) * kTriLdW + (j & 31)];
+    out[idx] = v;
   }
 }
 

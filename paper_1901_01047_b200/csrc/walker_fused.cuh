@@ -48,7 +48,7 @@ __host__ __device__ inline FusedSmem fused_smem_layout(int cap) {
 }
 
 template <bool ONSITE>   // the on-site Hubbard model (one gamma, one site per vertex) or interacting pairs through the tables
-__global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n_sweeps, int fcap) {
+__global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n_sweeps, int n_props, int fcap) {
   extern __shared__ __align__(16) unsigned char fsm[];
   const int wk = blockIdx.x, tid = threadIdx.x;
   WalkerState& st = c.ws[wk];
@@ -104,8 +104,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
   // come from the pair tables of DevCtx
   __syncthreads();
 
+  if (n_props > 0) n_sweeps = 1;     // ctaux_propose: one partial sweep of exactly n_props proposals
   for (int sw = 0; sw < n_sweeps && !status; ++sw) {
-    const int nprop = k > 16 ? k : 16;
+    const int nprop = n_props > 0 ? n_props : (k > 16 ? k : 16);
     for (int ip = 0; ip < nprop; ++ip) {
       uint32_t wa[4], wb[4];
       philox4x32_10((uint32_t)(p & 0xffffffffu), (uint32_t)(p >> 32), 0u, 1u, st.key0, st.key1, wa);

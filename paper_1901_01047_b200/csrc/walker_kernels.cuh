@@ -57,6 +57,19 @@ __global__ void k_set_state(DevCtx c, const uint64_t* seeds, const int32_t* k, c
 // configuration buffers, converting the auxiliary spins between the int8 of the ABI and the int32 kept on the device.
 struct PackedCfg { int32_t* k; uint64_t* id; int32_t* site; double* tau; int8_t* spin; };
 
+// live block of every N_sigma into the host layout of ctaux_get_N_all: matrix (w, spin) at (2w + spin) max_k^2, ld = k_w
+__global__ void k_pack_N(DevCtx c, double* out) {
+  const int prob = blockIdx.y, w = prob >> 1, sp = prob & 1;
+  const WalkerState& st = c.ws[w];
+  const int k = st.k;
+  const double* N = c.N(w, sp, st.n_cur);
+  double* dst = out + (size_t)prob * c.max_k * c.max_k;
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < k * k; idx += gridDim.x * blockDim.x) {
+    const int j = idx / k, i = idx - j * k;
+    dst[idx] = N[(size_t)j * c.ld + i];
+  }
+}
+
 __global__ void k_scatter_state(DevCtx c, PackedCfg pk) {   // -> configuration buffer 0 of every walker
   const int w = blockIdx.y;
   const int k = pk.k[w];
@@ -104,12 +117,12 @@ __global__ void k_build_A(DevCtx c, int into_other) {
 
 // ---------------------------------------------------------------------------------------------
 // Start of a ctaux_sweep chunk.
-__global__ void k_begin_sweeps(DevCtx c, int n_sweeps) {
+__global__ void k_begin_sweeps(DevCtx c, int n_sweeps, int n_props) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w == 0) { c.n_active[0] = c.B; c.n_active[1] = 0; }
   if (w >= c.B) return;
   c.ws[w].sweeps_left = n_sweeps;
-  c.ws[w].props_left = 0;
+  c.ws[w].props_left = n_props;     // > 0: ctaux_propose (a partial sweep first)
   c.ws[w].active = 1;
   c.ws[w].r = 0;
 }

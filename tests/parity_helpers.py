@@ -73,11 +73,25 @@ def frob_rel(a, b):
     return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
 
 
+def _oracle_N(orc, s):
+    """N_sigma = A_sigma^-1 of the oracle's current configuration: the oracle's own plain-C++ inversion below order
+    1024; above it the SAME definition through LAPACK (numpy.linalg.inv of the oracle's A: a library primitive as one
+    step -- the plain-C++ routine needs 40 s per matrix at k = 3600), cached per (spin, proposal counter)."""
+    if orc.k <= 1024:
+        return orc.N(s)
+    cache = orc.__dict__.setdefault("_N_cache", {})
+    key = (s, orc.p, orc.k)
+    if key not in cache:
+        cache.clear() if len(cache) >= 2 and all(kk[1] != orc.p for kk in cache) else None
+        cache[key] = np.linalg.inv(orc.A(s))
+    return cache[key]
+
+
 def compare_N(walkers, w_index, orc, what="", tol=N_FROB_TOL):
     errs = []
     for s in range(2):
         Nd = walkers.get_N(w_index, s)
-        No = orc.N(s)
+        No = _oracle_N(orc, s)
         assert Nd.shape == No.shape, f"{what}: N shape {Nd.shape} vs {No.shape}"
         if No.size:
             e = frob_rel(Nd, No)
@@ -234,32 +248,52 @@ def brute_force_verify(cfg, table, start_cfg, log, windows, rtol=1e-7, atol=1e-9
             out.append((la, sg))
         return out
 
-    def one(snap):
+    # the distinct vertex lists whose determinants are needed: the list BEFORE every proposal (shared by all proposals
+    # of one version) and the PROPOSED list of every proposal; the proposed list of an accepted proposal IS the list
+    # before the next one, so inside a window of n consecutive proposals there are n + 1 distinct lists, not 2 n
+    idx_of = {snap[0]: q for q, snap in enumerate(snaps)}
+    lists, need = {}, []
+    for snap in snaps:
         i, site, tau, spin, version = snap
         e = log[i]
         k = len(site)
         if e["type"] != 0 and k == 0:
-            return i, 0.0, None
-        d0 = logdets(site, tau, spin)
+            need.append((i, None, None, 0.0))
+            continue
+        lists.setdefault(("v", version), (site, tau, spin))
         if e["type"] == 0:
-            s2, t2, p2 = site + [int(e["arg"])], tau + [float(e["tau"])], spin + [int(e["spin"])]
+            prop = (site + [int(e["arg"])], tau + [float(e["tau"])], spin + [int(e["spin"])])
             pref = K / (k + 1)
         elif e["type"] == 1:
             j = int(e["arg"])
-            s2, t2, p2 = site[:j] + site[j + 1:], tau[:j] + tau[j + 1:], spin[:j] + spin[j + 1:]
+            prop = (site[:j] + site[j + 1:], tau[:j] + tau[j + 1:], spin[:j] + spin[j + 1:])
             pref = k / K
         else:
             j = int(e["arg"])
-            s2, t2, p2 = site, tau, spin[:j] + [-spin[j]] + spin[j + 1:]
+            prop = (site, tau, spin[:j] + [-spin[j]] + spin[j + 1:])
             pref = 1.0
-        d1 = logdets(s2, t2, p2)
-        R = pref * d1[0][1] * d1[1][1] * d0[0][1] * d0[1][1] * math.exp(d1[0][0] + d1[1][0] - d0[0][0] - d0[1][0])
-        return i, R, None
+        if e["accepted"] and (i + 1) in idx_of:
+            nxt = snaps[idx_of[i + 1]]
+            assert nxt[4] == version + 1 and (nxt[1], nxt[2], nxt[3]) == (list(prop[0]), list(prop[1]), list(prop[2]))
+            key = ("v", version + 1)
+        else:
+            key = ("a", i)
+        lists.setdefault(key, prop)
+        need.append((i, ("v", version), key, pref))
 
+    keys = list(lists)
     from threadpoolctl import threadpool_limits
-    with threadpool_limits(limits=1):      # one LAPACK thread per worker: the proposals are the parallel dimension
+    with threadpool_limits(limits=1):      # one LAPACK thread per worker: the vertex lists are the parallel dimension
         with ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as ex:
-            res = list(ex.map(one, snaps))
+            dets = dict(zip(keys, ex.map(lambda kk: logdets(*lists[kk]), keys)))
+    res = []
+    for i, k0, k1, pref in need:
+        if k0 is None:
+            res.append((i, 0.0, None))
+            continue
+        d0, d1 = dets[k0], dets[k1]
+        R = pref * d1[0][1] * d1[1][1] * d0[0][1] * d0[1][1] * math.exp(d1[0][0] + d1[1][0] - d0[0][0] - d0[1][0])
+        res.append((i, R, None))
     worst = 0.0
     for i, R, _ in res:
         e = log[i]

@@ -293,21 +293,59 @@ def test_error_codes_through_the_abi():
     assert ei.value.code == -1
 
 
-def test_batched_readout_equals_per_walker_readout():
+@pytest.mark.parametrize("nw", [5, 20])
+def test_batched_readout_equals_per_walker_readout(nw):
+    """nw = 20 takes the packed path of ctaux_get_N_all (device-side pack into the host layout, one 2-D copy)."""
     pkg = _pkg()
     cfg = get_config(1)
-    W = pkg.Walkers.from_config(cfg, table_for(cfg), n_walkers=5)
-    W.reset(walker_seeds(5, first=7))
+    W = pkg.Walkers.from_config(cfg, table_for(cfg), n_walkers=nw)
+    W.reset(walker_seeds(nw, first=7))
     W.sweep(3)
     cfgs = W.get_config_all()
     Ns = W.get_N_all([len(c["site"]) for c in cfgs])
-    for w in range(5):
+    for w in range(nw):
         one = W.get_config(w)
         for f in one:
             assert one[f].tobytes() == cfgs[w][f].tobytes()
         for s in range(2):
             assert np.array_equal(W.get_N(w, s), Ns[w][s])
     W.close()
+
+
+def test_packed_state_round_trip_continues_the_chain():
+    """The C ABI's batched forms as the bench's end-to-end leg uses them: get_state_packed (pinned host buffers) ->
+    set_state_packed on a second context -> both continue; identical configurations, counters and N afterwards, and
+    the packed N equals the per-walker getter."""
+    pkg = _pkg()
+    cfg = get_config(1)
+    table = table_for(cfg)
+    nw = 18
+    seeds = walker_seeds(nw, first=3)
+    A = pkg.WalkerGroups(2, nw, lambda g, nb, stream: pkg.Walkers.from_config(cfg, table, n_walkers=nb, stream=stream))
+    A.reset(seeds)
+    A.sweep(4)
+    st = A.get_state_packed(with_N=True)
+    mk = cfg["max_k"]
+    for g, s_ in enumerate(st):
+        for i in range(A.per):
+            k = int(s_["k"][i])
+            for sp in range(2):
+                blk = s_["N"][(2 * i + sp) * mk * mk:(2 * i + sp) * mk * mk + k * k].reshape((k, k), order="F")
+                assert np.array_equal(blk, A.get_N(g * A.per + i, sp))
+    B = pkg.WalkerGroups(2, nw, lambda g, nb, stream: pkg.Walkers.from_config(cfg, table, n_walkers=nb, stream=stream))
+    B.set_state_packed(seeds, st)
+    A.sweep(3)
+    B.sweep(3)
+    for w in range(nw):
+        ca, cb = A.get_config(w), B.get_config(w)
+        for f in ca:
+            assert ca[f].tobytes() == cb[f].tobytes()
+        sa, sb = A.get_stats(w), B.get_stats(w)
+        assert sa["proposals"] == sb["proposals"] and sa["next_id"] == sb["next_id"] and sa["sign"] == sb["sign"]
+        for sp in range(2):
+            Na, Nb = A.get_N(w, sp), B.get_N(w, sp)
+            assert np.linalg.norm(Na - Nb) <= 1e-10 * np.linalg.norm(Na)
+    A.close(); B.close()
 
 
 @pytest.mark.parametrize("fused", [1, -1])
@@ -516,29 +554,32 @@ def test_P5_U_zero_on_the_device():
 def test_config5_thermalised_start_full_size_delay_128_and_256():
     """Config 5 at full size (6x6, beta 40, k ~ 3600; split-K S2 GEMMs, rank-128 / rank-256 flushes; S3 as a 2-CTA
     cluster per walker with S^-1 in shared memory at delay 128 and in L2 at delay 256 -- the two launch
-    configurations bench.py times) from the oracle-thermalised configuration (30 oracle sweeps): one sweep (~3600
-    proposals) of 2 seeds against T1, decisions bit-exact, N within 1e-10 (the oracle runs once: its chain does not
-    depend on the delay; ~4 min of CPU)."""
+    configurations bench.py times).  Two walkers, each from the thermalised configuration of its OWN oracle seed
+    (tests/golden/thermalised_cfg5_6x6_b40_seed{0,1}.txt, >= 25 oracle sweeps): 1600 proposals (ctaux_propose; 3-4
+    blocks at delay 256, 6-7 at delay 128) against T1, decisions bit-exact, N within 1e-10.  The oracle runs once (its
+    chain does not depend on the delay); a whole sweep at this size costs the plain-C++ oracle ~5 min."""
     from concurrent.futures import ThreadPoolExecutor
     cfg = get_config(4)
     table = table_for(cfg)
-    c0, next_id, p0 = load_thermalised(cfg["name"], 1)
+    states = [load_thermalised(cfg["name"], sd) for sd in (0, 1)]
     seeds = walker_seeds(2)
+    nprop = 1600
 
-    def one(seed):
-        o = OracleWalker.from_config(cfg, table, int(seed), T1)
+    def one(i):
+        c0, next_id, p0 = states[i]
+        o = OracleWalker.from_config(cfg, table, int(seeds[i]), T1)
         o.set_state(c0["site"], c0["tau"], c0["spin"], c0["id"], next_id, p0)
-        o.sweep(1)
+        o.propose(nprop)
         return o
 
     with ThreadPoolExecutor(max_workers=2) as ex:
-        fut = [ex.submit(one, s) for s in seeds]
+        fut = [ex.submit(one, i) for i in range(2)]
         Ws = []
         for delay in (128, 256):
             W = _pkg().Walkers(cfg["Lx"], cfg["Ly"], cfg["beta"], cfg["U"], cfg["K"], table, delay=delay, n_walkers=2,
-                               init_k=0, max_k=cfg["max_k"], rebuild_every=0, log_capacity=cfg["max_k"] + 64)
-            W.set_state(seeds, [c0] * 2, [next_id] * 2, [p0] * 2)
-            W.sweep(1)
+                               init_k=0, max_k=cfg["max_k"], rebuild_every=0, log_capacity=nprop + 64)
+            W.set_state(seeds, [s[0] for s in states], [s[1] for s in states], [s[2] for s in states])
+            W.propose(nprop)
             Ws.append((delay, W))
         orcs = [f.result() for f in fut]
     for delay, W in Ws:
@@ -548,9 +589,46 @@ def test_config5_thermalised_start_full_size_delay_128_and_256():
             compare_configs(W.get_config(w), o.config(), what)
             st = W.get_stats(w)
             assert st["k"] == o.k and st["proposals"] == o.p and st["next_id"] == o.next_id and st["sign"] == o.sign, what
-            assert st["flushes"] > 10 and st["sum_rank"] / st["flushes"] > 0.5 * delay
+            assert st["proposals"] == states[w][2] + nprop
+            assert st["flushes"] >= 3 and st["sum_rank"] / st["flushes"] > 0.5 * delay
             compare_N(W, w, o, what)
         W.close()
+
+
+@pytest.mark.parametrize("fused", [1, -1])
+def test_propose_calls_split_the_chain_anywhere(fused):
+    """ctaux_propose (a partial sweep of exactly n proposals) mixed with ctaux_sweep: the chain depends on the proposal
+    counter only.  Config 2 (fused small-k kernel and delayed path) in lock step with the oracle's propose / sweep."""
+    pkg = _pkg()
+    cfg = get_config(1)
+    table = table_for(cfg)
+    nw = 3
+    seeds = walker_seeds(nw, first=11)
+    W = pkg.Walkers.from_config(cfg, table, n_walkers=nw, fused_small=fused, log_capacity=4000, rebuild_every=2)
+    W.reset(seeds)
+    orcs = []
+    for sd in seeds:
+        o = OracleWalker.from_config(cfg, table, int(sd), T1)
+        o.reset(cfg["init_k"])
+        orcs.append(o)
+    for kind, n in (("p", 37), ("s", 1), ("p", 1), ("p", 150), ("s", 2), ("p", 5)):
+        if kind == "p":
+            W.propose(n)
+            [o.propose(n) for o in orcs]
+        else:
+            W.sweep(n)
+            [o.sweep(n) for o in orcs]
+        for w, o in enumerate(orcs):
+            st = W.get_stats(w)
+            assert st["proposals"] == o.p and st["k"] == o.k, (kind, n, w)
+    for w, o in enumerate(orcs):
+        what = f"propose/sweep mix, fused {fused}, walker {w}"
+        compare_logs(W.get_log(w), o.log(), what)
+        compare_configs(W.get_config(w), o.config(), what)
+        compare_N(W, w, o, what)
+    assert W._L.ctaux_propose(W._h, -1) == -1
+    W.propose(0)
+    W.close()
 
 
 # ---------------------------------------------------------------- SURVEY 8d "parity protocol at scale"
@@ -628,10 +706,10 @@ def test_config4_log_replay_brute_force_windows():
 @pytest.mark.parametrize("delay", [128, 256])
 def test_config5_log_replay_brute_force_windows(delay):
     """Config 5 at full size from the thermalised starts of two oracle seeds (30 sweeps each, k ~ 3600), delay 128 and
-    256 (the 2-CTA cluster forms of S3), 3 sweeps: three windows of 32 consecutive device-log proposals per walker by
+    256 (the 2-CTA cluster forms of S3), 3 sweeps: three windows of 24 consecutive device-log proposals per walker by
     brute-force determinants, P7 on the final N."""
     import os
     gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
     have = [sd for sd in (0, 1) if os.path.exists(os.path.join(gdir, f"thermalised_cfg5_6x6_b40_seed{sd}.txt"))]
     assert have, "tests/golden/thermalised_cfg5_6x6_b40_seed*.txt missing"
-    _log_replay(4, (have * 2)[:2], 3, delay, 32, 3)
+    _log_replay(4, (have * 2)[:2], 3, delay, 24, 3)
