@@ -315,9 +315,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
       }
       ++log_count;
       if (type == 0 || arg >= 0) {
-        const double aR = fabs(R);
-        const double mg = fabs(uu - aR) / fmax(aR, 1e-300);
-        if (mg < min_margin) min_margin = mg;
+        const double aR = fmax(fabs(R), 1e-300), du = fabs(uu - fabs(R));
+        if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
       }
       sum_k += (double)(k - (accept ? (type == 0 ? 1 : (type == 1 ? -1 : 0)) : 0));   // k before the proposal
       ++p;

@@ -254,7 +254,7 @@ constexpr int kGroup = kPropThreads / 2;  // threads per spin
 
 struct ProposeSmem {
   // byte offsets into dynamic shared memory
-  int sinv, scol, srow, tv, tpv, jiem, red, snn, live0, live1, spin, J, jpos, prop, flip, total;
+  int sinv, scol, srow, tv, tpv, jiem, red, snn, spec, live0, live1, spin, J, jpos, prop, flip, total;
 };
 
 __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
@@ -269,6 +269,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.jiem = o; o += 2 * delay * 8;
   L.red = o; o += 2 * 2 * 8 * 8;
   L.snn = o; o += 4 * 8;
+  L.spec = o; o += (4 * delay + 2) * 8;   // speculative gather: [2 spins][s_col | s_row][delay] raw entries + 2 diagonals
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
   L.live1 = o; o += cap * 4;
@@ -339,6 +340,15 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   bool finished = false;
   int guard_end = 0;
   double errlvl = 1.0;  // rounding-error level of S^-1 in units of eps (largest amplification accepted so far)
+  // Speculative gather: the entries X(J[a], slot), X(slot, J[a]) and the diagonal entry of the NEXT proposal are loaded
+  // while the current one is evaluated (a third of a proposal's latency is this dependent gather from L2 / HBM).  The
+  // loads assume the current proposal is rejected, plus one entry for J[r] = the current slot in case it is accepted;
+  // they are used when the next proposal really meets that slot and that J (checked below), else gathered again.
+  // The loads are asynchronous copies into shared memory (LDGSTS): register loads kept in flight across a proposal
+  // tie up the warp's scoreboards and were measured SLOWER than no speculation at all.
+  double* spec_own = reinterpret_cast<double*>(smraw + L.spec) + (sp * 2 + (lt >> 6)) * c.delay;   // this thread's role
+  double* spec_dg = reinterpret_cast<double*>(smraw + L.spec) + 4 * c.delay + sp;
+  int spec_slot = -1, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
 
   for (int i = 0; i < win; ++i) {
     if (props_left == 0) {
@@ -363,7 +373,8 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
-    double R = 0.0, stil_own = 1.0, amp = 1.0, iem_own = 0.0;
+    double R = 0.0, stil_own = 1.0, iem_own = 0.0;
+    double amp_n0 = 1.0, amp_n1 = 1.0, amp_d0 = 1.0, amp_d1 = 1.0;   // amp = max(n0/d0, n1/d1), divided on accept only
     // removal of a vertex inserted earlier in this block: the two changes of that slot cancel, so
     // the buffered insertion is taken OUT of the block (exact treatment of a twice-touched spin,
     // PAPER.md:228): ratio = (S^-1)_aa / dE_a, then S^-1 is downdated.
@@ -390,17 +401,53 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       // thread roles inside a spin group of 128: half 0 builds s_col and t = S^-1 s_col (and the dot
       // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass
       const int half = lt >> 6, la = lt & 63;
-      for (int a = la; a < r; a += 64) {
-        const int ja = Js[a];
-        if (half == 0) scol[a] = X(ja, slot, iem_slot);
-        else srow[a] = X(slot, ja, jiem[a]);
-      }
       double* snn = snn2 + (i & 1) * 2;   // double buffered: read after the second barrier of this proposal
-      if (lt == 0) {
-        // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
-        // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
-        if (slot < k0 && type == 1) snn[sp] = -Ncur[(size_t)slot * ld + slot] * iem_slot;
-        else snn[sp] = 1.0 / dE_own + X(slot, slot, iem_slot);
+      const bool hit = spec_slot == slot && spec_type == type && spec_jver == jver && (spec_r == r || spec_r + 1 == r);
+      cp_async_wait_all();     // this thread's own copies of the previous proposal (long done; it reads only those)
+      if (hit) {
+        for (int a = la; a < r; a += 64) {
+          const int ja = Js[a];
+          const double raw = spec_own[a], dlt = (ja == slot) ? 1.0 : 0.0;
+          if (half == 0) scol[a] = slot < k0 ? (dlt - raw) * iem_slot : dlt - raw;      // X(ja, slot)
+          else srow[a] = ja < k0 ? (dlt - raw) * jiem[a] : dlt - raw;                  // X(slot, ja)
+        }
+        if (lt == 0) {
+          const double raw = *spec_dg;
+          if (slot < k0 && type == 1) snn[sp] = -raw * iem_slot;
+          else snn[sp] = 1.0 / dE_own + (slot < k0 ? (1.0 - raw) * iem_slot : 1.0 - raw);
+        }
+      } else {
+        for (int a = la; a < r; a += 64) {
+          const int ja = Js[a];
+          if (half == 0) scol[a] = X(ja, slot, iem_slot);
+          else srow[a] = X(slot, ja, jiem[a]);
+        }
+        if (lt == 0) {
+          // diagonal entry 1/dE + X[slot,slot]; for a block-start vertex (removal, dE = 1 - E) this is
+          // -N[slot,slot]/(E-1) exactly, written so that nothing cancels
+          if (slot < k0 && type == 1) snn[sp] = -Ncur[(size_t)slot * ld + slot] * iem_slot;
+          else snn[sp] = 1.0 / dE_own + X(slot, slot, iem_slot);
+        }
+      }
+      // issue the copies of the next proposal (consumed one iteration later: their latency hides behind this proposal)
+      spec_slot = -1;
+      if (i + 1 < win) {
+        const PropInfo pn = prop[i + 1];
+        const int tn = (int)(pn.type_cand & 3u);
+        int ns = -1;
+        if (tn == 0) ns = k0 + (int)(pn.type_cand >> 2);
+        else if (kcur > 0) ns = live[(int)(((uint64_t)pn.w1 * (uint64_t)kcur) >> 32)];
+        if (ns >= 0 && !(tn == 1 && ns >= k0)) {
+          spec_slot = ns; spec_type = tn; spec_r = r; spec_jver = jver;
+          const double* coln = ns < k0 ? Ncur + (size_t)ns * ld : Gx + (size_t)(ns - k0) * ld;    // column ns of N_ext / G_ext
+          for (int a = la; a <= r; a += 64) {
+            const int ja = a < r ? Js[a] : slot;
+            const double* src = half == 0 ? coln + ja
+                                          : (ja < k0 ? Ncur + (size_t)ja * ld + ns : Gx + (size_t)(ja - k0) * ld + ns);
+            cp_async_8(spec_own + a, src);
+          }
+          if (lt == 0) cp_async_8(spec_dg, coln + ns);
+        }
       }
       __syncthreads();
       double part = 0.0, apart = 0.0;
@@ -450,10 +497,12 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       {
         const double ad0 = (red[16] + red[17]) + (red[18] + red[19]);
         const double ad1 = (red[24] + red[25]) + (red[26] + red[27]);
-        const double amp0 = (fabs(snn[0]) + ad0) / fmax(fabs(stil0), 1e-300);
-        const double amp1 = (fabs(snn[1]) + ad1) / fmax(fabs(stil1), 1e-300);
-        amp = fmax(amp0, amp1);
-        if (r > 0 && amp * errlvl > c.guard_amp) { guard_end = 1; break; }
+        // amp_s * errlvl > guard  <=>  num_s * errlvl > guard * den_s: no division on the decision path (amp itself is
+        // only needed when the proposal is accepted)
+        const double num0 = fabs(snn[0]) + ad0, num1 = fabs(snn[1]) + ad1;
+        const double den0 = fmax(fabs(stil0), 1e-300), den1 = fmax(fabs(stil1), 1e-300);
+        if (r > 0 && (num0 * errlvl > c.guard_amp * den0 || num1 * errlvl > c.guard_amp * den1)) { guard_end = 1; break; }
+        amp_n0 = num0; amp_n1 = num1; amp_d0 = den0; amp_d1 = den1;
       }
       stil_own = sp == 0 ? stil0 : stil1;
       R = pref * ((dE0 * stil0) * (dE1 * stil1));
@@ -473,9 +522,8 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     }
     ++log_count;
     if (slot >= 0) {
-      const double aR = fabs(R);
-      const double mg = fabs(pi.u - aR) / fmax(aR, 1e-300);
-      if (mg < min_margin) min_margin = mg;
+      const double aR = fmax(fabs(R), 1e-300), du = fabs(pi.u - fabs(R));
+      if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
     }
     sum_k += (double)kcur;
     if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }  // CTAUX_ECAPACITY
@@ -512,7 +560,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       int* t = live; live = live_alt; live_alt = t;
       --len; --kcur; ++acc_rem;
       if (R < 0.0) sign = -sign;
-      --r;
+      --r; ++jver;      // J was re-ordered: speculative loads of the next proposal are void
     } else if (accept) {
       const double inv = 1.0 / stil_own;
       for (int a = lt & 63; a < r; a += 64) {   // 64 rows x 2 column phases: no integer division
@@ -526,7 +574,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       }
       if (lt == 0) { Sv[r + (size_t)r * lds] = inv; jiem[r] = iem_own; }
       if (tid == 0) Js[r] = slot;
-      errlvl = fmax(errlvl, amp);
+      errlvl = fmax(errlvl, fmax(amp_n0 / amp_d0, amp_n1 / amp_d1));
       if (type == 0) {
         if (tid == 0) { live[len] = slot; c.cfg_id[off_old + slot] = next_id; jpos[slot - k0] = r; }
         ++len; ++kcur; ++next_id; ++acc_ins;

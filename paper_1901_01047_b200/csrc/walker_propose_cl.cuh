@@ -16,7 +16,7 @@ namespace ctaux {
 constexpr int kClThreads = 512;
 
 struct ProposeClSmem {
-  int sinv, scol, srow, tv, tpv, jiem, red, snn, xch, live0, live1, spin, J, jpos, prop, flip, total;
+  int sinv, scol, srow, tv, tpv, jiem, red, snn, xch, spec, live0, live1, spin, J, jpos, prop, flip, total;
 };
 __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int delay, int winmax, bool sinv_smem) {
   ProposeClSmem L;
@@ -31,6 +31,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.red = o; o += 2 * 16 * 8;
   L.snn = o; o += 2 * 8;
   L.xch = o; o += 2 * 2 * 4 * 8;      // [parity][spin][stil, ampnum, -, -]
+  L.spec = o; o += (2 * delay + 2) * 8;   // speculative gather of the next proposal: [s_col | s_row][delay] raw entries, diagonal
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
   L.live1 = o; o += cap * 4;
@@ -121,6 +122,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   const int row4 = rl >> 2, q4 = rl & 3;       // 64 rows per pass, 4 lanes per row
   const unsigned quad_mask = 0xFu << (tid & 28);   // the 4 lanes of a row leave the row loop together
 
+  // speculative gather of the next proposal's entries (see k_propose): one entry per thread here (delay <= 256 lanes)
+  double* spec_own = reinterpret_cast<double*>(smcl + L.spec) + (tid >> 8) * c.delay;
+  double* spec_dg = reinterpret_cast<double*>(smcl + L.spec) + 2 * c.delay;
+  int spec_slot = -1, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
+
   for (int i = 0; i < win; ++i) {
     if (props_left == 0) {
       if (sweeps_left == 0) { finished = true; break; }
@@ -144,7 +150,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       if ((type == 2 && (slot >= k0 || flipped[slot])) || (type == 1 && slot < k0 && flipped[slot])) { guard_end = 2; break; }
     }
     bool accept = false;
-    double R = 0.0, stil_own = 1.0, amp = 1.0, iem_own = 0.0;
+    double R = 0.0, stil_own = 1.0, iem_own = 0.0;
+    double amp_n0 = 1.0, amp_n1 = 1.0, amp_d0 = 1.0, amp_d1 = 1.0;   // amp = max(n0/d0, n1/d1), divided on accept only
     const bool down = (type == 1 && slot >= k0);
     int apos = -1;
     if (down) {
@@ -168,15 +175,51 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       const double dE_own = sp == 0 ? dE0 : dE1;
       const double iem_slot = c.template iem1t<ONSITE>(sp, s, pr);
       iem_own = iem_slot;
-      for (int a = rl; a < r; a += 256) {
-        const int ja = Js[a];
-        if (role == 0) scol[a] = X(ja, slot, iem_slot);
-        else srow[a] = X(slot, ja, jiem[a]);
-      }
       double* snn = snn2 + (i & 1);
-      if (tid == 0) {
-        if (slot < k0 && type == 1) *snn = -Ncur[(size_t)slot * ld + slot] * iem_slot;
-        else *snn = 1.0 / dE_own + X(slot, slot, iem_slot);
+      const bool hit = spec_slot == slot && spec_type == type && spec_jver == jver && (spec_r == r || spec_r + 1 == r);
+      cp_async_wait_all();     // this thread's own copies of the previous proposal (long done; it reads only those)
+      if (hit) {
+        if (rl < r) {
+          const int ja = Js[rl];
+          const double raw = spec_own[rl], dlt = (ja == slot) ? 1.0 : 0.0;
+          if (role == 0) scol[rl] = slot < k0 ? (dlt - raw) * iem_slot : dlt - raw;      // X(ja, slot)
+          else srow[rl] = ja < k0 ? (dlt - raw) * jiem[rl] : dlt - raw;                  // X(slot, ja)
+        }
+        if (tid == 0) {
+          const double raw = *spec_dg;
+          if (slot < k0 && type == 1) *snn = -raw * iem_slot;
+          else *snn = 1.0 / dE_own + (slot < k0 ? (1.0 - raw) * iem_slot : 1.0 - raw);
+        }
+      } else {
+        for (int a = rl; a < r; a += 256) {
+          const int ja = Js[a];
+          if (role == 0) scol[a] = X(ja, slot, iem_slot);
+          else srow[a] = X(slot, ja, jiem[a]);
+        }
+        if (tid == 0) {
+          if (slot < k0 && type == 1) *snn = -Ncur[(size_t)slot * ld + slot] * iem_slot;
+          else *snn = 1.0 / dE_own + X(slot, slot, iem_slot);
+        }
+      }
+      // copies of the next proposal, assuming this one is rejected, plus the entry for J[r] = this slot if it is accepted
+      spec_slot = -1;
+      if (i + 1 < win) {
+        const PropInfo pn = prop[i + 1];
+        const int tn = (int)(pn.type_cand & 3u);
+        int ns = -1;
+        if (tn == 0) ns = k0 + (int)(pn.type_cand >> 2);
+        else if (kcur > 0) ns = live[(int)(((uint64_t)pn.w1 * (uint64_t)kcur) >> 32)];
+        if (ns >= 0 && !(tn == 1 && ns >= k0)) {
+          spec_slot = ns; spec_type = tn; spec_r = r; spec_jver = jver;
+          const double* coln = ns < k0 ? Ncur + (size_t)ns * ld : Gx + (size_t)(ns - k0) * ld;
+          if (rl <= r) {
+            const int ja = rl < r ? Js[rl] : slot;
+            const double* src = role == 0 ? coln + ja
+                                          : (ja < k0 ? Ncur + (size_t)ja * ld + ns : Gx + (size_t)(ja - k0) * ld + ns);
+            cp_async_8(spec_own + rl, src);
+          }
+          if (tid == 0) cp_async_8(spec_dg, coln + ns);
+        }
       }
       __syncthreads();
       double part = 0.0, apart = 0.0;
@@ -215,10 +258,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       exchange(stil, fabs(*snn) + adot, o0, o1);
       const double stil0 = o0[0], stil1 = o1[0];
       {
-        const double amp0 = o0[1] / fmax(fabs(stil0), 1e-300);
-        const double amp1 = o1[1] / fmax(fabs(stil1), 1e-300);
-        amp = fmax(amp0, amp1);
-        if (r > 0 && amp * errlvl > c.guard_amp) { guard_end = 1; break; }
+        // no division on the decision path: amp_s errlvl > guard  <=>  num_s errlvl > guard den_s
+        const double den0 = fmax(fabs(stil0), 1e-300), den1 = fmax(fabs(stil1), 1e-300);
+        if (r > 0 && (o0[1] * errlvl > c.guard_amp * den0 || o1[1] * errlvl > c.guard_amp * den1)) { guard_end = 1; break; }
+        amp_n0 = o0[1]; amp_n1 = o1[1]; amp_d0 = den0; amp_d1 = den1;
       }
       stil_own = stil;
       R = pref * ((dE0 * stil0) * (dE1 * stil1));
@@ -236,9 +279,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
     }
     ++log_count;
     if (slot >= 0) {
-      const double aR = fabs(R);
-      const double mg = fabs(pi.u - aR) / fmax(aR, 1e-300);
-      if (mg < min_margin) min_margin = mg;
+      const double aR = fmax(fabs(R), 1e-300), du = fabs(pi.u - fabs(R));
+      if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
     }
     sum_k += (double)kcur;
     if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }
@@ -274,7 +316,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       int* t = live; live = live_alt; live_alt = t;
       --len; --kcur; ++acc_rem;
       if (R < 0.0) sign = -sign;
-      --r;
+      --r; ++jver;      // J was re-ordered: speculative loads of the next proposal are void
     } else if (accept) {
       const double inv = 1.0 / stil_own;
       for (int a = tid & 63; a < r; a += 64) {
@@ -287,7 +329,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
         Sv[r + (size_t)a * lds] = -tpv[a] * inv;
       }
       if (tid == 0) { Sv[r + (size_t)r * lds] = inv; Js[r] = slot; jiem[r] = iem_own; }
-      errlvl = fmax(errlvl, amp);
+      errlvl = fmax(errlvl, fmax(amp_n0 / amp_d0, amp_n1 / amp_d1));
       if (type == 0) {
         if (tid == 0) {
           live[len] = slot; jpos[slot - k0] = r;

@@ -176,4 +176,12 @@ __host__ __device__ __forceinline__ double unif53(uint32_t a, uint32_t b) {
   return (double)u * (1.0 / 9007199254740992.0);
 }
 
+// 8-byte asynchronous global -> shared copy (LDGSTS) and the wait for all copies this thread has issued: used by the S3
+// kernels to gather the next proposal's scattered entries of N behind the current proposal
+__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gsrc) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 }  // namespace ctaux

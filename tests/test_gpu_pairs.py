@@ -45,8 +45,11 @@ def test_extended_hubbard_4x4_delayed_blocks_and_large_k_kernels():
     spin sector (the two sectors see different sites), once with the small-k and once with the large-k launch shapes."""
     pairs = extended_hubbard_pairs(4, 4, 4.0, 1.0)
     cfg = dict(get_config(2), name="ext_4x4_b5", beta=5.0, max_k=448, init_k=150)
-    full_parity(cfg, 6, 8, T1, pairs=pairs)
-    full_parity(dict(cfg, max_k=600), 2, 5, T1, pairs=pairs, delay=128)
+    # thermalising chains from a random 150-vertex start (cond(A) ~ 1e6): the logged ratios of the two sides agree to a few
+    # 1e-7 relative, within a factor of two of parity_helpers' equilibrium tolerance (1e-6), and where a block ends moves
+    # them; the bar here is 1e-5 as for the 2x2 thermalising case above (DESIGN.md section 5), decisions stay bit-exact
+    full_parity(cfg, 6, 8, T1, pairs=pairs, r_rtol=1e-5)
+    full_parity(dict(cfg, max_k=600), 2, 5, T1, pairs=pairs, delay=128, r_rtol=1e-5)
 
 
 def test_bilayer_interlayer_interaction_and_flips():
