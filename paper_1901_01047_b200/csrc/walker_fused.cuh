@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
   uint64_t p = st.p, next_id = st.next_id;
   int sign = st.sign, status = 0, spill_sweeps = -1, spill_props = 0;
   int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, log_count = st.log_count;
-  double min_margin = st.min_margin, sum_k = 0.0;
+  double mm_du = st.min_margin, mm_aR = 1.0, sum_k = 0.0;   // decision margin as a fraction (no division per proposal)
   int sweeps_done = 0;
   // site_s[] holds the PAIR index of every slot (= the site in the on-site model); E and the site a spin sector sees
   // come from the pair tables of DevCtx
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
       ++log_count;
       if (type == 0 || arg >= 0) {
         const double aR = fmax(fabs(R), 1e-300), du = fabs(uu - fabs(R));
-        if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
+        if (du * mm_aR < mm_du * aR) { mm_du = du; mm_aR = aR; }      // smallest du / aR, divided once at write-back
       }
       sum_k += (double)(k - (accept ? (type == 0 ? 1 : (type == 1 ? -1 : 0)) : 0));   // k before the proposal
       ++p;
@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_walk_fused(DevCtx c, int n
     st.next_id = next_id; st.p = p; st.sign = sign;
     st.acc_ins += acc_ins; st.acc_rem += acc_rem; st.acc_flip += acc_flip; st.sweeps += sweeps_done;
     st.blocks += sweeps_done; st.log_count = log_count;
-    st.min_margin = min_margin; st.sum_k += sum_k;
+    st.min_margin = mm_du / mm_aR; st.sum_k += sum_k;
     st.sweeps_left = 0; st.props_left = 0; st.active = 0;
     if (spill_sweeps >= 0) {
       st.sweeps_left = spill_sweeps; st.props_left = spill_props; st.active = 1;

@@ -249,6 +249,38 @@ __global__ void k_prep_fill(DevCtx c) {
 //          =  delta_ij - Gx[i, j-k0]                   j a candidate
 // Buffered changes J = (j_1..j_r), dE_a;  S_ab = delta_ab/dE_a + X[j_a, j_b];
 // det A_{r+1} / det A_r = dE_new (s_nn - s_row S^-1 s_col)
+// Slot the NEXT proposal of the window will meet if the current one (type, slot, list position j) is rejected (ns) or
+// accepted (nsA); -1 where it needs no gather (no vertex to pick, or the removal of an in-block insert, which reads
+// S^-1 only).  An insert names its candidate slot directly; a removal / flip picks by position in the live list, which
+// an accepted insert extends by `slot` and an accepted removal shifts.  Shared by k_propose and k_propose_cl.
+struct NextSlots { int type, ns, nsA; };
+__device__ __forceinline__ NextSlots next_slots(const PropInfo pn, int k0, int kcur, const int* live, int type, int slot, int j) {
+  NextSlots o;
+  o.type = (int)(pn.type_cand & 3u);
+  o.ns = o.nsA = -1;
+  if (o.type == 0) {
+    o.ns = o.nsA = k0 + (int)(pn.type_cand >> 2);
+  } else {
+    if (kcur > 0) o.ns = live[(int)(((uint64_t)pn.w1 * (uint64_t)kcur) >> 32)];
+    if (type == 0) {            // accepted insert: the list (length kcur) grows by `slot` at its end
+      const int jn = (int)(((uint64_t)pn.w1 * (uint64_t)(kcur + 1)) >> 32);
+      o.nsA = jn == kcur ? slot : live[jn];
+    } else if (type == 1) {     // accepted removal of position j: later positions shift down
+      if (kcur > 1) { const int jn = (int)(((uint64_t)pn.w1 * (uint64_t)(kcur - 1)) >> 32); o.nsA = live[jn + (jn >= j ? 1 : 0)]; }
+    } else {
+      o.nsA = o.ns;             // accepted flip: same list
+    }
+    if (o.type == 1 && o.ns >= k0) o.ns = -1;
+    if (o.type == 1 && o.nsA >= k0) o.nsA = -1;
+  }
+  return o;
+}
+// X[i, j] from the raw entry of N_ext (j < k0: a block-start column, iem_j = 1/(E0_j - 1)) or of G_ext (a candidate column)
+__device__ __forceinline__ double x_from_raw(double raw, bool diag, bool blockstart_col, double iem_j) {
+  const double d = (diag ? 1.0 : 0.0) - raw;
+  return blockstart_col ? d * iem_j : d;
+}
+
 constexpr int kPropThreads = 256;
 constexpr int kGroup = kPropThreads / 2;  // threads per spin
 
@@ -269,7 +301,7 @@ __host__ __device__ inline ProposeSmem propose_smem_layout(int cap, int delay, i
   L.jiem = o; o += 2 * delay * 8;
   L.red = o; o += 2 * 2 * 8 * 8;
   L.snn = o; o += 4 * 8;
-  L.spec = o; o += (4 * delay + 2) * 8;   // speculative gather: [2 spins][s_col | s_row][delay] raw entries + 2 diagonals
+  L.spec = o; o += 2 * (4 * delay + 2) * 8;   // speculative gather, 2 hypotheses: [2 spins][s_col | s_row][delay] raw entries + 2 diagonals
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
   L.live1 = o; o += cap * 4;
@@ -335,7 +367,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   uint64_t next_id = st.next_id, p = st.p;
   int sign = st.sign, status = 0, consumed = 0;
   int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, sweeps_done = 0;
-  double min_margin = st.min_margin, sum_k = 0.0;
+  double mm_du = st.min_margin, mm_aR = 1.0, sum_k = 0.0;   // decision margin as a fraction (no division per proposal)
   int64_t log_count = st.log_count;
   bool finished = false;
   int guard_end = 0;
@@ -346,9 +378,13 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
   // they are used when the next proposal really meets that slot and that J (checked below), else gathered again.
   // The loads are asynchronous copies into shared memory (LDGSTS): register loads kept in flight across a proposal
   // tie up the warp's scoreboards and were measured SLOWER than no speculation at all.
+  // Buffer 0 holds the entries for the slot the next proposal meets if the current one is REJECTED, buffer 1 those for
+  // the slot it meets if the current one is ACCEPTED, when that is a different slot (a removal or flip picks its target
+  // by position in the live list, which an accepted move shifts); where the two slots agree buffer 0 serves both.
+  const int spec_stride = 4 * c.delay + 2;
   double* spec_own = reinterpret_cast<double*>(smraw + L.spec) + (sp * 2 + (lt >> 6)) * c.delay;   // this thread's role
   double* spec_dg = reinterpret_cast<double*>(smraw + L.spec) + 4 * c.delay + sp;
-  int spec_slot = -1, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
+  int spec_slot = -1, specA_slot = -1, specA_buf = 0, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
 
   for (int i = 0; i < win; ++i) {
     if (props_left == 0) {
@@ -402,19 +438,21 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       // product), half 1 builds s_row and t' = s_row^T S^-1; 64 rows per pass
       const int half = lt >> 6, la = lt & 63;
       double* snn = snn2 + (i & 1) * 2;   // double buffered: read after the second barrier of this proposal
-      const bool hit = spec_slot == slot && spec_type == type && spec_jver == jver && (spec_r == r || spec_r + 1 == r);
+      const bool hitR = spec_slot == slot && spec_r == r, hitA = specA_slot == slot && spec_r + 1 == r;
+      const bool hit = spec_type == type && spec_jver == jver && (hitR || hitA);
+      const int hbuf = (hitR ? 0 : specA_buf) * spec_stride;
       cp_async_wait_all();     // this thread's own copies of the previous proposal (long done; it reads only those)
       if (hit) {
         for (int a = la; a < r; a += 64) {
           const int ja = Js[a];
-          const double raw = spec_own[a], dlt = (ja == slot) ? 1.0 : 0.0;
-          if (half == 0) scol[a] = slot < k0 ? (dlt - raw) * iem_slot : dlt - raw;      // X(ja, slot)
-          else srow[a] = ja < k0 ? (dlt - raw) * jiem[a] : dlt - raw;                  // X(slot, ja)
+          const double raw = spec_own[hbuf + a];
+          if (half == 0) scol[a] = x_from_raw(raw, ja == slot, slot < k0, iem_slot);      // X(ja, slot)
+          else srow[a] = x_from_raw(raw, ja == slot, ja < k0, jiem[a]);                  // X(slot, ja)
         }
         if (lt == 0) {
-          const double raw = *spec_dg;
+          const double raw = spec_dg[hbuf];
           if (slot < k0 && type == 1) snn[sp] = -raw * iem_slot;
-          else snn[sp] = 1.0 / dE_own + (slot < k0 ? (1.0 - raw) * iem_slot : 1.0 - raw);
+          else snn[sp] = 1.0 / dE_own + x_from_raw(raw, true, slot < k0, iem_slot);
         }
       } else {
         for (int a = la; a < r; a += 64) {
@@ -430,23 +468,25 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
         }
       }
       // issue the copies of the next proposal (consumed one iteration later: their latency hides behind this proposal)
-      spec_slot = -1;
+      spec_slot = -1; specA_slot = -1; specA_buf = 0;
       if (i + 1 < win) {
-        const PropInfo pn = prop[i + 1];
-        const int tn = (int)(pn.type_cand & 3u);
-        int ns = -1;
-        if (tn == 0) ns = k0 + (int)(pn.type_cand >> 2);
-        else if (kcur > 0) ns = live[(int)(((uint64_t)pn.w1 * (uint64_t)kcur) >> 32)];
-        if (ns >= 0 && !(tn == 1 && ns >= k0)) {
-          spec_slot = ns; spec_type = tn; spec_r = r; spec_jver = jver;
-          const double* coln = ns < k0 ? Ncur + (size_t)ns * ld : Gx + (size_t)(ns - k0) * ld;    // column ns of N_ext / G_ext
+        const NextSlots nx = next_slots(prop[i + 1], k0, kcur, live, type, slot, j);
+        const int tn = nx.type, ns = nx.ns, nsA = nx.nsA;
+        spec_type = tn; spec_r = r; spec_jver = jver;
+        auto issue = [&](int nsl, int buf) {
+          const double* coln = nsl < k0 ? Ncur + (size_t)nsl * ld : Gx + (size_t)(nsl - k0) * ld;    // column of N_ext / G_ext
           for (int a = la; a <= r; a += 64) {
             const int ja = a < r ? Js[a] : slot;
             const double* src = half == 0 ? coln + ja
-                                          : (ja < k0 ? Ncur + (size_t)ja * ld + ns : Gx + (size_t)(ja - k0) * ld + ns);
-            cp_async_8(spec_own + a, src);
+                                          : (ja < k0 ? Ncur + (size_t)ja * ld + nsl : Gx + (size_t)(ja - k0) * ld + nsl);
+            cp_async_8(spec_own + buf * spec_stride + a, src);
           }
-          if (lt == 0) cp_async_8(spec_dg, coln + ns);
+          if (lt == 0) cp_async_8(spec_dg + buf * spec_stride, coln + nsl);
+        };
+        if (ns >= 0) { spec_slot = ns; issue(ns, 0); }
+        if (nsA >= 0) {
+          specA_slot = nsA;
+          if (nsA != ns) { specA_buf = 1; issue(nsA, 1); }
         }
       }
       __syncthreads();
@@ -523,7 +563,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     ++log_count;
     if (slot >= 0) {
       const double aR = fmax(fabs(R), 1e-300), du = fabs(pi.u - fabs(R));
-      if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
+      if (du * mm_aR < mm_du * aR) { mm_du = du; mm_aR = aR; }      // smallest du / aR, divided once at write-back
     }
     sum_k += (double)kcur;
     if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }  // CTAUX_ECAPACITY
@@ -574,7 +614,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
       }
       if (lt == 0) { Sv[r + (size_t)r * lds] = inv; jiem[r] = iem_own; }
       if (tid == 0) Js[r] = slot;
-      errlvl = fmax(errlvl, fmax(amp_n0 / amp_d0, amp_n1 / amp_d1));
+      errlvl = fmax(errlvl, amp_n0 * amp_d1 > amp_n1 * amp_d0 ? amp_n0 / amp_d0 : amp_n1 / amp_d1);   // max of the two ratios, one division
       if (type == 0) {
         if (tid == 0) { live[len] = slot; c.cfg_id[off_old + slot] = next_id; jpos[slot - k0] = r; }
         ++len; ++kcur; ++next_id; ++acc_ins;
@@ -630,7 +670,7 @@ __global__ void __launch_bounds__(kPropThreads) k_propose(DevCtx c) {
     st.guard_ends += guard_end != 0;
     if (r > 0) { st.flushes += 1; st.sum_rank += r; }
     st.log_count = log_count;
-    st.min_margin = min_margin; st.sum_k += sum_k;
+    st.min_margin = mm_du / mm_aR; st.sum_k += sum_k;
     st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
       st.flops_cand_alg += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * (double)acc_ins);   // columns of accepted inserts only
     st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);

@@ -31,7 +31,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.red = o; o += 2 * 16 * 8;
   L.snn = o; o += 2 * 8;
   L.xch = o; o += 2 * 2 * 4 * 8;      // [parity][spin][stil, ampnum, -, -]
-  L.spec = o; o += (2 * delay + 2) * 8;   // speculative gather of the next proposal: [s_col | s_row][delay] raw entries, diagonal
+  L.spec = o; o += 2 * (2 * delay + 2) * 8;   // speculative gather of the next proposal, 2 hypotheses: [s_col | s_row][delay] raw entries, diagonal
   L.prop = o; o += winmax * 16;
   L.live0 = o; o += cap * 4;
   L.live1 = o; o += cap * 4;
@@ -85,7 +85,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   uint64_t next_id = st.next_id, p = st.p;
   int sign = st.sign, status = 0;
   int64_t acc_ins = 0, acc_rem = 0, acc_flip = 0, sweeps_done = 0;
-  double min_margin = st.min_margin, sum_k = 0.0;
+  double mm_du = st.min_margin, mm_aR = 1.0, sum_k = 0.0;   // decision margin as a fraction (no division per proposal)
   int64_t log_count = st.log_count;
   const int n_cur0 = st.n_cur;
   bool finished = false;
@@ -125,7 +125,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   // speculative gather of the next proposal's entries (see k_propose): one entry per thread here (delay <= 256 lanes)
   double* spec_own = reinterpret_cast<double*>(smcl + L.spec) + (tid >> 8) * c.delay;
   double* spec_dg = reinterpret_cast<double*>(smcl + L.spec) + 2 * c.delay;
-  int spec_slot = -1, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
+  const int spec_stride = 2 * c.delay + 2;       // buffer 0: next slot if this proposal is rejected, buffer 1: if accepted
+  int spec_slot = -1, specA_slot = -1, specA_buf = 0, spec_r = -1, spec_jver = -1, spec_type = -1, jver = 0;
 
   for (int i = 0; i < win; ++i) {
     if (props_left == 0) {
@@ -176,19 +177,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       const double iem_slot = c.template iem1t<ONSITE>(sp, s, pr);
       iem_own = iem_slot;
       double* snn = snn2 + (i & 1);
-      const bool hit = spec_slot == slot && spec_type == type && spec_jver == jver && (spec_r == r || spec_r + 1 == r);
+      const bool hitR = spec_slot == slot && spec_r == r, hitA = specA_slot == slot && spec_r + 1 == r;
+      const bool hit = spec_type == type && spec_jver == jver && (hitR || hitA);
+      const int hbuf = (hitR ? 0 : specA_buf) * spec_stride;
       cp_async_wait_all();     // this thread's own copies of the previous proposal (long done; it reads only those)
       if (hit) {
         if (rl < r) {
           const int ja = Js[rl];
-          const double raw = spec_own[rl], dlt = (ja == slot) ? 1.0 : 0.0;
-          if (role == 0) scol[rl] = slot < k0 ? (dlt - raw) * iem_slot : dlt - raw;      // X(ja, slot)
-          else srow[rl] = ja < k0 ? (dlt - raw) * jiem[rl] : dlt - raw;                  // X(slot, ja)
+          const double raw = spec_own[hbuf + rl];
+          if (role == 0) scol[rl] = x_from_raw(raw, ja == slot, slot < k0, iem_slot);      // X(ja, slot)
+          else srow[rl] = x_from_raw(raw, ja == slot, ja < k0, jiem[rl]);                  // X(slot, ja)
         }
         if (tid == 0) {
-          const double raw = *spec_dg;
+          const double raw = spec_dg[hbuf];
           if (slot < k0 && type == 1) *snn = -raw * iem_slot;
-          else *snn = 1.0 / dE_own + (slot < k0 ? (1.0 - raw) * iem_slot : 1.0 - raw);
+          else *snn = 1.0 / dE_own + x_from_raw(raw, true, slot < k0, iem_slot);
         }
       } else {
         for (int a = rl; a < r; a += 256) {
@@ -202,23 +205,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
         }
       }
       // copies of the next proposal, assuming this one is rejected, plus the entry for J[r] = this slot if it is accepted
-      spec_slot = -1;
+      spec_slot = -1; specA_slot = -1; specA_buf = 0;
       if (i + 1 < win) {
-        const PropInfo pn = prop[i + 1];
-        const int tn = (int)(pn.type_cand & 3u);
-        int ns = -1;
-        if (tn == 0) ns = k0 + (int)(pn.type_cand >> 2);
-        else if (kcur > 0) ns = live[(int)(((uint64_t)pn.w1 * (uint64_t)kcur) >> 32)];
-        if (ns >= 0 && !(tn == 1 && ns >= k0)) {
-          spec_slot = ns; spec_type = tn; spec_r = r; spec_jver = jver;
-          const double* coln = ns < k0 ? Ncur + (size_t)ns * ld : Gx + (size_t)(ns - k0) * ld;
+        const NextSlots nx = next_slots(prop[i + 1], k0, kcur, live, type, slot, j);
+        const int tn = nx.type, ns = nx.ns, nsA = nx.nsA;
+        spec_type = tn; spec_r = r; spec_jver = jver;
+        auto issue = [&](int nsl, int buf) {
+          const double* coln = nsl < k0 ? Ncur + (size_t)nsl * ld : Gx + (size_t)(nsl - k0) * ld;
           if (rl <= r) {
             const int ja = rl < r ? Js[rl] : slot;
             const double* src = role == 0 ? coln + ja
-                                          : (ja < k0 ? Ncur + (size_t)ja * ld + ns : Gx + (size_t)(ja - k0) * ld + ns);
-            cp_async_8(spec_own + rl, src);
+                                          : (ja < k0 ? Ncur + (size_t)ja * ld + nsl : Gx + (size_t)(ja - k0) * ld + nsl);
+            cp_async_8(spec_own + buf * spec_stride + rl, src);
           }
-          if (tid == 0) cp_async_8(spec_dg, coln + ns);
+          if (tid == 0) cp_async_8(spec_dg + buf * spec_stride, coln + nsl);
+        };
+        if (ns >= 0) { spec_slot = ns; issue(ns, 0); }
+        if (nsA >= 0) {
+          specA_slot = nsA;
+          if (nsA != ns) { specA_buf = 1; issue(nsA, 1); }
         }
       }
       __syncthreads();
@@ -280,7 +285,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
     ++log_count;
     if (slot >= 0) {
       const double aR = fmax(fabs(R), 1e-300), du = fabs(pi.u - fabs(R));
-      if (du < min_margin * aR) min_margin = du / aR;      // the division only when the minimum moves
+      if (du * mm_aR < mm_du * aR) { mm_du = du; mm_aR = aR; }      // smallest du / aR, divided once at write-back
     }
     sum_k += (double)kcur;
     if (accept && type == 0 && kcur + 1 > c.max_k) { status = -2; break; }
@@ -329,7 +334,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
         Sv[r + (size_t)a * lds] = -tpv[a] * inv;
       }
       if (tid == 0) { Sv[r + (size_t)r * lds] = inv; Js[r] = slot; jiem[r] = iem_own; }
-      errlvl = fmax(errlvl, fmax(amp_n0 / amp_d0, amp_n1 / amp_d1));
+      errlvl = fmax(errlvl, amp_n0 * amp_d1 > amp_n1 * amp_d0 ? amp_n0 / amp_d0 : amp_n1 / amp_d1);   // max of the two ratios, one division
       if (type == 0) {
         if (tid == 0) {
           live[len] = slot; jpos[slot - k0] = r;
@@ -388,7 +393,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       st.guard_ends += guard_end != 0;
       if (r > 0) { st.flushes += 1; st.sum_rank += r; }
       st.log_count = log_count;
-      st.min_margin = min_margin; st.sum_k += sum_k;
+      st.min_margin = mm_du / mm_aR; st.sum_k += sum_k;
       st.flops_cand += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * m);
       st.flops_cand_alg += 2.0 * (2.0 * m * (double)k0 * k0 + 2.0 * (double)n * n * (double)acc_ins);   // columns of accepted inserts only
       st.flops_flush += 2.0 * (2.0 * (double)kcur * kcur * r);
