@@ -256,6 +256,22 @@ size_t ctaux_g0_workspace_bytes(int32_t Lx, int32_t Ly, int32_t n_omega, int32_t
 int ctaux_g0_table(void* stream, int32_t Lx, int32_t Ly, double t, double mu, double beta, int32_t n_omega, int32_t n_quad,
                    const double* sigma_c, int32_t n_tau, double* table, void* workspace, size_t workspace_bytes);
 
+/* ctaux_g0_table for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same operation (Eq. (6)-(9)), same kernels, same arguments and
+ * results (sigma_c HOST or NULL, table HOST, synchronises the stream), but the scratch is a static device array inside
+ * the library instead of a caller workspace; the call performs no cudaMalloc / cudaFree and calls no allocating library
+ * routine.  Limits and sharing:
+ *   - ctaux_g0_workspace_bytes(Lx, Ly, n_omega, n_tau) must not exceed CTAUX_G0_NOALLOC_MAX_BYTES (8 MiB: e.g. a 6x6
+ *     cluster with n_omega = 2048, n_tau = 4096); larger sizes return CTAUX_ECAPACITY and ctaux_last_cuda_error() names
+ *     the bytes needed.  Every GPU that loads the library holds the 8 MiB until the process exits.
+ *   - ALL calls on a device share the one array: two calls that overlap on the GPU (different streams or host threads)
+ *     race.  Serialise them.  The array keeps the last call's contents; every element a call reads is written earlier in
+ *     that same call, so no clearing is needed and results do not depend on earlier calls.
+ * Errors as ctaux_g0_table: CTAUX_EINVAL for invalid sizes / NULL table, CTAUX_ECUDA for CUDA failures. */
+#define CTAUX_G0_NOALLOC_MAX_BYTES (8u << 20)
+int ctaux_g0_table_noalloc(void* stream, int32_t Lx, int32_t Ly, double t, double mu, double beta, int32_t n_omega,
+                           int32_t n_quad, const double* sigma_c, int32_t n_tau, double* table);
+
 /* Kernel launches issued by this context since creation (bench.py's gpu_launches). */
 int64_t ctaux_launch_count(ctaux_ctx* ctx);
 

@@ -5,8 +5,8 @@ CUDA).  Argument marshalling only: every step of the path runs in the CUDA kerne
 used for device memory and streams.  There is no CPU fallback: if the extension cannot be loaded
 or no CUDA device is present, calls fail loudly.
 """
-from .binding import (CtauxError, Walkers, WalkerGroups, colmajor, ctaux_dgemm, debug_philox, exported_symbols, g0_table_from_sigma, lib_path, probe_fp64,
+from .binding import (CtauxError, Walkers, WalkerGroups, colmajor, ctaux_dgemm, debug_philox, exported_symbols, g0_table_from_sigma, g0_table_from_sigma_noalloc, lib_path, probe_fp64,
                       load_library, LOG_DTYPE, STEP_CLASSES)
 
-__all__ = ["CtauxError", "Walkers", "WalkerGroups", "colmajor", "ctaux_dgemm", "debug_philox", "exported_symbols", "g0_table_from_sigma", "lib_path", "probe_fp64",
+__all__ = ["CtauxError", "Walkers", "WalkerGroups", "colmajor", "ctaux_dgemm", "debug_philox", "exported_symbols", "g0_table_from_sigma", "g0_table_from_sigma_noalloc", "lib_path", "probe_fp64",
            "load_library", "LOG_DTYPE", "STEP_CLASSES"]

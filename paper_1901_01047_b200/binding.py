@@ -45,7 +45,7 @@ class _Stats(C.Structure):
 # include/ctaux.h (the walker boundary) and include/ctaux_testing.h (test / measurement helpers)
 EXPORTS = ["ctaux_workspace_bytes", "ctaux_create", "ctaux_reset", "ctaux_set_state", "ctaux_sweep",
            "ctaux_propose", "ctaux_rebuild", "ctaux_get_config", "ctaux_get_config_all", "ctaux_get_N", "ctaux_get_N_all", "ctaux_get_N_device", "ctaux_get_stats", "ctaux_get_stats_all",
-           "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_g0_workspace_bytes", "ctaux_g0_table", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
+           "ctaux_get_log", "ctaux_accumulate", "ctaux_get_M", "ctaux_reset_accumulator", "ctaux_g0_workspace_bytes", "ctaux_g0_table", "ctaux_g0_table_noalloc", "ctaux_launch_count", "ctaux_timing_enable", "ctaux_timing_get",
            "ctaux_destroy", "ctaux_strerror", "ctaux_last_cuda_error"]
 TEST_EXPORTS = ["ctaux_dgemm", "ctaux_probe_fp64", "ctaux_debug_philox"]
 
@@ -89,6 +89,7 @@ def load_library():
     L.ctaux_g0_workspace_bytes.restype = C.c_size_t
     L.ctaux_g0_workspace_bytes.argtypes = [i32, i32, i32, i32]
     L.ctaux_g0_table.argtypes = [vp, i32, i32, C.c_double, C.c_double, C.c_double, i32, i32, vp, i32, vp, vp, C.c_size_t]
+    L.ctaux_g0_table_noalloc.argtypes = [vp, i32, i32, C.c_double, C.c_double, C.c_double, i32, i32, vp, i32, vp]
     L.ctaux_launch_count.restype = i64
     L.ctaux_launch_count.argtypes = [vp]
     L.ctaux_timing_enable.argtypes = [vp, i32]
@@ -518,6 +519,34 @@ def g0_table_from_sigma(Lx, Ly, t, mu, beta, n_omega, n_quad, n_tau, sigma_c=Non
         ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
         _check(L.ctaux_g0_table(torch.cuda.current_stream(dev).cuda_stream, Lx, Ly, t, mu, beta, n_omega, n_quad, sig_ptr,
                                 n_tau, table.ctypes.data, ws.data_ptr(), nbytes), "ctaux_g0_table")
+    return table
+
+
+G0_NOALLOC_MAX_BYTES = 8 << 20      # CTAUX_G0_NOALLOC_MAX_BYTES of include/ctaux.h
+
+
+def g0_table_from_sigma_noalloc(Lx, Ly, t, mu, beta, n_omega, n_quad, n_tau, sigma_c=None, device="cuda:0"):
+    """g0_table_from_sigma through ctaux_g0_table_noalloc: no device memory is allocated by the call (the scratch is a
+    static 8 MiB device array inside the library, shared by all calls on a device: do not overlap calls).  Sizes whose
+    scratch exceeds the array raise CtauxError(-2)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise CtauxError(-3, "ctaux_g0_table_noalloc", "no CUDA device: this package has no CPU fallback")
+    L = load_library()
+    dev = torch.device(device)
+    sig_ptr = None
+    if sigma_c is not None:
+        sc = np.asarray(sigma_c, dtype=np.complex128)
+        assert sc.shape == (Lx * Ly, n_omega)
+        sig = np.ascontiguousarray(np.stack([sc.real, sc.imag], axis=-1))
+        sig_ptr = sig.ctypes.data
+    table = np.zeros((Lx * Ly, n_tau + 1), np.float64)
+    with torch.cuda.device(dev):
+        rc = L.ctaux_g0_table_noalloc(torch.cuda.current_stream(dev).cuda_stream, Lx, Ly, t, mu, beta, n_omega, n_quad,
+                                      sig_ptr, n_tau, table.ctypes.data)
+    if rc == -2:      # the library's message states the bytes needed and the size of the static array
+        raise CtauxError(rc, "ctaux_g0_table_noalloc", L.ctaux_last_cuda_error().decode())
+    _check(rc, "ctaux_g0_table_noalloc")
     return table
 
 

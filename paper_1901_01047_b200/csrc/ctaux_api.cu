@@ -1385,6 +1385,52 @@ int ctaux_g0_table(void* stream, int32_t Lx, int32_t Ly, double t, double mu, do
   return CTAUX_OK;
 }
 
+// ---- ctaux_g0_table for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+// that forbid cudaMalloc): the same kernels, with their scratch in a file-scope device array of CTAUX_G0_NOALLOC_MAX_BYTES
+// that every GPU loading this library holds until the process exits.  In host code the array's NAME is a host-side
+// stand-in, not a device address: the address is taken once per device, with that device current, by
+// cudaGetSymbolAddress, and only that pointer goes to the kernels.
+static __device__ __align__(256) unsigned char g_g0_noalloc_scratch[CTAUX_G0_NOALLOC_MAX_BYTES];
+
+static int g0_noalloc_scratch_ptr(void** out) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static void* ptr[kMaxDev];      // device address of g_g0_noalloc_scratch, per device
+  int dev = -1;
+  CU_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) { g_last_cuda_error = "ctaux_g0_table_noalloc: device index beyond 63"; return CTAUX_EINVAL; }
+  std::lock_guard<std::mutex> lk(mu);
+  if (!ptr[dev]) {
+    void* p = nullptr;
+    CU_CHECK(cudaGetSymbolAddress(&p, g_g0_noalloc_scratch));      // device `dev` is current
+    if (!p || ((uintptr_t)p & 255) != 0) { g_last_cuda_error = "ctaux_g0_table_noalloc: bad address of the static scratch"; return CTAUX_ECUDA; }
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return CTAUX_OK;
+}
+
+int ctaux_g0_table_noalloc(void* stream, int32_t Lx, int32_t Ly, double t, double mu, double beta, int32_t n_omega,
+                           int32_t n_quad, const double* sigma_c, int32_t n_tau, double* table) {
+  const size_t need = ctaux_g0_workspace_bytes(Lx, Ly, n_omega, n_tau);
+  if (need == 0 || !table) return CTAUX_EINVAL;
+  if (need > (size_t)CTAUX_G0_NOALLOC_MAX_BYTES) {
+    g_last_cuda_error = "ctaux_g0_table_noalloc: this size needs " + std::to_string(need) + " bytes of scratch, the static array holds " +
+                        std::to_string((size_t)CTAUX_G0_NOALLOC_MAX_BYTES) + " (use ctaux_g0_table with a caller workspace)";
+    return CTAUX_ECAPACITY;
+  }
+  int ndev = 0;
+  CU_CHECK(cudaGetDeviceCount(&ndev));
+  if (ndev == 0) { g_last_cuda_error = "no CUDA device"; return CTAUX_ECUDA; }
+  void* scratch = nullptr;
+  const int rc = g0_noalloc_scratch_ptr(&scratch);
+  if (rc) return rc;
+  // Every element of the scratch a kernel reads is written earlier in the same call (sigma by the copy below when given,
+  // remK / mom by k_g0_coarse, remR / momR by k_g0_to_r, the table by k_g0_to_tau; nothing accumulates), so what the
+  // last call left behind needs no clearing.  ctaux_g0_table itself allocates nothing.
+  return ctaux_g0_table(stream, Lx, Ly, t, mu, beta, n_omega, n_quad, sigma_c, n_tau, table, scratch, (size_t)CTAUX_G0_NOALLOC_MAX_BYTES);
+}
+
 int64_t ctaux_launch_count(ctaux_ctx* x) { return x ? x->launches : 0; }
 
 int ctaux_timing_enable(ctaux_ctx* x, int32_t on) {
