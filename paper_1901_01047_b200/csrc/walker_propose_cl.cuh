@@ -3,12 +3,16 @@
 // two CTAs per walker, one per spin.  Each CTA keeps the S^-1 of its own spin (132 KB at delay 128) in
 // its own shared memory (or in L2 when even that does not fit: delay 256), evaluates its spin's
 // determinant ratio with 512 threads (4 lanes per row of S^-1), and the two CTAs exchange their
-// per-proposal scalars through distributed shared memory with ONE cluster barrier per proposal.  All
+// per-proposal scalars through distributed shared memory: each sends its two values straight into the peer's shared
+// memory with st.async, which completes a transaction on the PEER's mbarrier -- data and signal travel together, so no
+// cluster barrier (whose release fence waited for every store and look-ahead copy in flight: 40 % of the warp-state
+// samples, profiles/r2_propose.md) sits on the per-proposal path.  All
 // bookkeeping (live list, J, counters) is replicated, so both CTAs take identical decisions.
 // PAPER.md:226-228 (submatrix updates), BASELINE.json config 5 (delay 128 and 256).
 #pragma once
 #include <cooperative_groups.h>
 
+#include "gemm_tma.cuh"      // mbarrier helpers
 #include "walker_kernels.cuh"
 
 namespace ctaux {
@@ -30,6 +34,7 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.jiem = o; o += delay * 8;
   L.red = o; o += 2 * 16 * 8;
   L.snn = o; o += 2 * 8;
+  o = (o + 15) & ~15;                 // st.async.v2.f64 wants 16-byte aligned slots
   L.xch = o; o += 2 * 2 * 4 * 8;      // [parity][spin][stil, ampnum, -, -]
   L.spec = o; o += 2 * (2 * delay + 2) * 8;   // speculative gather of the next proposal, 2 hypotheses: [s_col | s_row][delay] raw entries, diagonal
   L.prop = o; o += winmax * 16;
@@ -41,6 +46,18 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   L.flip = o; o += (cap + 15) / 16 * 16;
   L.total = o;
   return L;
+}
+
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+// two doubles into a peer CTA's shared memory; completes 16 bytes of transaction on the PEER's mbarrier
+__device__ __forceinline__ void st_async_2f64(uint32_t dst_cluster_addr, double a, double b, uint32_t mbar_cluster_addr) {
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];\n"
+               ::"r"(dst_cluster_addr), "d"(a), "d"(b), "r"(mbar_cluster_addr) : "memory");
 }
 
 template <bool sinv_smem, bool ONSITE>
@@ -63,7 +80,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   double* red = reinterpret_cast<double*>(smcl + L.red);    // [16] dot, [16] sum of magnitudes
   double* snn2 = reinterpret_cast<double*>(smcl + L.snn);   // [2 parities]
   double* xch = reinterpret_cast<double*>(smcl + L.xch);
-  double* xch_peer = cluster.map_shared_rank(xch, sp ^ 1);
+  __shared__ uint64_t xbar_storage;
+  uint64_t* xbar = &xbar_storage;
+  const uint32_t xch_peer_addr = mapa_u32(smem_u32(xch), (uint32_t)(sp ^ 1));      // shared::cluster addresses in the peer CTA
+  const uint32_t xbar_peer_addr = mapa_u32(smem_u32(xbar), (uint32_t)(sp ^ 1));
+  if (tid == 0) { mbar_init(xbar, 1); mbar_fence_init(); }      // visible to the peer after the first cluster.sync() below
   PropInfo* prop = reinterpret_cast<PropInfo*>(smcl + L.prop);
   int* live = reinterpret_cast<int*>(smcl + L.live0);
   int* live_alt = reinterpret_cast<int*>(smcl + L.live1);
@@ -104,18 +125,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
     return dlt - Gx[(size_t)(j - k0) * ld + i];
   };
   // publish this spin's two scalars to both CTAs, one cluster barrier, read both spins' values
+  // Every thread of a CTA holds its own spin's two values already (all threads evaluate the same reduction); thread 0
+  // sends them to slot [parity][sp] of the peer and arms the own mbarrier for the 16 bytes the peer sends; everybody
+  // waits on the own mbarrier and reads the peer's values.  Slot reuse (two exchanges later) is safe: the peer sends
+  // exchange e + 2 only after it has received e + 1, which this CTA's thread 0 sent after a __syncthreads() that all of
+  // its threads reach after their reads of slot e.
   int xpar = 0;
+  uint32_t xphase = 0;
   auto exchange = [&](double v0, double v1, double (&o0)[2], double (&o1)[2]) {
     if (tid == 0) {
-      double* mine = xch + (xpar * 2 + sp) * 4;
-      double* theirs = xch_peer + (xpar * 2 + sp) * 4;
-      mine[0] = v0; mine[1] = v1;
-      theirs[0] = v0; theirs[1] = v1;
+      mbar_expect_tx(xbar, 16);
+      st_async_2f64(xch_peer_addr + (uint32_t)((xpar * 2 + sp) * 4 * 8), v0, v1, xbar_peer_addr);
     }
-    cluster.sync();
-    o0[0] = xch[(xpar * 2 + 0) * 4]; o0[1] = xch[(xpar * 2 + 0) * 4 + 1];
-    o1[0] = xch[(xpar * 2 + 1) * 4]; o1[1] = xch[(xpar * 2 + 1) * 4 + 1];
-    xpar ^= 1;
+    mbar_wait(xbar, xphase);
+    const double* theirs = xch + (xpar * 2 + (sp ^ 1)) * 4;
+    const double p0 = theirs[0], p1 = theirs[1];
+    if (sp == 0) { o0[0] = v0; o0[1] = v1; o1[0] = p0; o1[1] = p1; }
+    else { o0[0] = p0; o0[1] = p1; o1[0] = v0; o1[1] = v1; }
+    xpar ^= 1; xphase ^= 1;
   };
 
   const int role = tid >> 8, rl = tid & 255;   // role 0: s_col and t; role 1: s_row and t'
