@@ -80,6 +80,24 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
   asm volatile("prefetch.tensormap [%0];\n" ::"l"(tm) : "memory");
 }
 
+// ---- distributed shared memory: data + signal in one message (st.async onto the receiver's mbarrier)
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+// two doubles into a peer CTA's shared memory; completes 16 bytes of transaction on the PEER's mbarrier
+__device__ __forceinline__ void st_async_2f64(uint32_t dst_cluster_addr, double a, double b, uint32_t mbar_cluster_addr) {
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];\n"
+               ::"r"(dst_cluster_addr), "d"(a), "d"(b), "r"(mbar_cluster_addr) : "memory");
+}
+// one double into a CTA of the cluster; completes 8 bytes of transaction on that CTA's mbarrier
+__device__ __forceinline__ void st_async_f64(uint32_t dst_cluster_addr, double a, uint32_t mbar_cluster_addr) {
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];\n"
+               ::"r"(dst_cluster_addr), "l"(__double_as_longlong(a)), "r"(mbar_cluster_addr) : "memory");
+}
+
 constexpr int kTmaBM = 64, kTmaBN = 64, kTmaBK = 16;
 constexpr int kTmaThreads = 128;   // 4 warps, 32 x 32 warp tiles (2 x 2)
 

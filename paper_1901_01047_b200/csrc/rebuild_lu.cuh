@@ -148,6 +148,16 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     const int i = idx % nloc, cc = idx / nloc;
     A[i * kLuPad + cc] = F[(size_t)(j0 + cc) * ld + r0 + i];
   }
+  // per-column exchange: every CTA sends its message (and the owner of row `col` that row) to all CTAs with st.async,
+  // which completes the bytes on the RECEIVER's mbarrier -- one one-way message instead of stores + a cluster barrier
+  // Two mbarriers, one per buffer parity: a fast CTA may send column cc + 1 while a slow one still waits for column cc;
+  // those bytes must not be counted on the phase of column cc.  (Messages for cc + 2 reach barrier cc & 1 only after its
+  // phase cc has completed everywhere: a CTA sends cc + 2 after it has received cc + 1 from all, and each of those was sent
+  // after its sender had passed the wait of column cc.)
+  __shared__ uint64_t cbar[2];
+  if (tid == 0) { mbar_init(cbar, 1); mbar_init(cbar + 1, 1); mbar_fence_init(); }
+  const uint32_t msg_a = smem_u32(msg), rowc_a = smem_u32(rowc);
+  constexpr uint32_t kColBytes = (uint32_t)((kLuCl * kLuMsg + kLuNb) * 8);
   cluster.sync();
 
   for (int cc = 0; cc < nb; ++cc) {
@@ -179,30 +189,33 @@ __global__ void __cluster_dims__(kLuCl, 1, 1) __launch_bounds__(kLuClThreads, 1)
     }
     __syncthreads();
     // 2. ONE message per CTA to every CTA: candidate magnitude, row index and the candidate row itself; the owner
-    //    of row `col` also sends that row (it travels to the pivot's slot).  One cluster barrier per column.
+    //    of row `col` also sends that row (it travels to the pivot's slot).  One mbarrier phase per column; buffer
+    //    `par` is overwritten two columns later, after every CTA has passed the __syncthreads() that end its reads.
     {
       const double b = s_val[0];
       const int ix = s_best;
       const bool have = ix != 0x7fffffff;
+      const uint32_t cbar_a = smem_u32(cbar + par);
+      if (tid == 0) mbar_expect_tx(cbar + par, kColBytes);
       for (int t = tid; t < kLuCl * kLuMsg; t += kLuClThreads) {
         const int q = t / kLuMsg, x = t % kLuMsg;
-        double* dst = cluster.map_shared_rank(msg, q) + ((size_t)par * kLuCl + rank) * kLuMsg;
         double v;
         if (x == 0) v = b;
         else if (x == 1) v = (double)ix;
         else v = (have && x - 2 < nb) ? A[(ix - r0) * kLuPad + (x - 2)] : 0.0;
-        dst[x] = v;
+        st_async_f64(mapa_u32(msg_a + (uint32_t)((((size_t)par * kLuCl + rank) * kLuMsg + x) * 8), (uint32_t)q), v,
+                     mapa_u32(cbar_a, (uint32_t)q));
       }
       const int qc = (col - j0) / R;
       if (rank == qc) {
         for (int t = tid; t < kLuCl * kLuNb; t += kLuClThreads) {
           const int q = t / kLuNb, x = t % kLuNb;
-          double* dst = cluster.map_shared_rank(rowc, q) + (size_t)par * kLuNb;
-          dst[x] = x < nb ? A[(col - r0) * kLuPad + x] : 0.0;
+          st_async_f64(mapa_u32(rowc_a + (uint32_t)(((size_t)par * kLuNb + x) * 8), (uint32_t)q),
+                       x < nb ? A[(col - r0) * kLuPad + x] : 0.0, mapa_u32(cbar_a, (uint32_t)q));
         }
       }
     }
-    cluster.sync();
+    mbar_wait(cbar + par, (uint32_t)((cc >> 1) & 1));
     // 3. everybody picks the same winner
     const double* mp = msg + (size_t)par * kLuCl * kLuMsg;
     int qw = 0;

@@ -12,7 +12,7 @@
 #pragma once
 #include <cooperative_groups.h>
 
-#include "gemm_tma.cuh"      // mbarrier helpers
+#include "gemm_tma.cuh"      // mbarrier and distributed-shared-memory helpers
 #include "walker_kernels.cuh"
 
 namespace ctaux {
@@ -48,18 +48,6 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   return L;
 }
 
-// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
-__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
-  uint32_t r;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
-  return r;
-}
-// two doubles into a peer CTA's shared memory; completes 16 bytes of transaction on the PEER's mbarrier
-__device__ __forceinline__ void st_async_2f64(uint32_t dst_cluster_addr, double a, double b, uint32_t mbar_cluster_addr) {
-  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];\n"
-               ::"r"(dst_cluster_addr), "d"(a), "d"(b), "r"(mbar_cluster_addr) : "memory");
-}
-
 template <bool sinv_smem, bool ONSITE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_propose_cl(DevCtx c) {
   namespace cg = cooperative_groups;
@@ -80,11 +68,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   double* red = reinterpret_cast<double*>(smcl + L.red);    // [16] dot, [16] sum of magnitudes
   double* snn2 = reinterpret_cast<double*>(smcl + L.snn);   // [2 parities]
   double* xch = reinterpret_cast<double*>(smcl + L.xch);
-  __shared__ uint64_t xbar_storage;
-  uint64_t* xbar = &xbar_storage;
+  __shared__ uint64_t xbar[2];      // one mbarrier per slot parity: bytes of exchange e + 1 never count on the phase of exchange e
   const uint32_t xch_peer_addr = mapa_u32(smem_u32(xch), (uint32_t)(sp ^ 1));      // shared::cluster addresses in the peer CTA
   const uint32_t xbar_peer_addr = mapa_u32(smem_u32(xbar), (uint32_t)(sp ^ 1));
-  if (tid == 0) { mbar_init(xbar, 1); mbar_fence_init(); }      // visible to the peer after the first cluster.sync() below
+  if (tid == 0) { mbar_init(xbar, 1); mbar_init(xbar + 1, 1); mbar_fence_init(); }      // visible to the peer after the first cluster.sync() below
   PropInfo* prop = reinterpret_cast<PropInfo*>(smcl + L.prop);
   int* live = reinterpret_cast<int*>(smcl + L.live0);
   int* live_alt = reinterpret_cast<int*>(smcl + L.live1);
@@ -134,15 +121,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
   uint32_t xphase = 0;
   auto exchange = [&](double v0, double v1, double (&o0)[2], double (&o1)[2]) {
     if (tid == 0) {
-      mbar_expect_tx(xbar, 16);
-      st_async_2f64(xch_peer_addr + (uint32_t)((xpar * 2 + sp) * 4 * 8), v0, v1, xbar_peer_addr);
+      mbar_expect_tx(xbar + xpar, 16);
+      st_async_2f64(xch_peer_addr + (uint32_t)((xpar * 2 + sp) * 4 * 8), v0, v1, xbar_peer_addr + (uint32_t)(xpar * 8));
     }
-    mbar_wait(xbar, xphase);
+    mbar_wait(xbar + xpar, xphase);
     const double* theirs = xch + (xpar * 2 + (sp ^ 1)) * 4;
     const double p0 = theirs[0], p1 = theirs[1];
     if (sp == 0) { o0[0] = v0; o0[1] = v1; o1[0] = p0; o1[1] = p1; }
     else { o0[0] = p0; o0[1] = p1; o1[0] = v0; o1[1] = v1; }
-    xpar ^= 1; xphase ^= 1;
+    xphase ^= (uint32_t)xpar;      // each barrier is used every other exchange
+    xpar ^= 1;
   };
 
   const int role = tid >> 8, rl = tid & 255;   // role 0: s_col and t; role 1: s_row and t'
