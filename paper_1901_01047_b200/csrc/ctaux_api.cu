@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <mutex>
@@ -269,6 +270,11 @@ struct ctaux_ctx {
   PackedCfg pk;       // device staging of the packed configurations
   double* nstage = nullptr;   // device staging of ctaux_get_N_all (small matrices only)
   uint64_t *pk_next, *pk_p;
+  // CUDA graph of one poll interval (steps_per_poll block steps) for the launch-bound sizes (max_k <= 512: a block step
+  // is ~13 launches of a few us each; config 3 spent more host time launching than the GPU spent computing)
+  bool use_graph = false, graph_warm = false;
+  cudaGraphExec_t graph_exec = nullptr;
+  int64_t graph_launches = 0, graph_nl[N_CLASS] = {};
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
   // timing
@@ -715,6 +721,38 @@ int enqueue_block_step(ctaux_ctx* x) {
   return CTAUX_OK;
 }
 
+// Capture `steps` block steps (launches on the context stream and on the forked S3 stream) into an executable graph.
+// Grids are sized for the capacity (the kernels read the live sizes on the device and stride / exit early), so one graph
+// serves every live size.  A failed capture switches the graph path off for this context; it is never an error.
+int capture_poll_graph(ctaux_ctx* x, int steps) {
+  cudaStream_t s = x->stream;
+  const int saved_hint = x->k_hint;
+  const int64_t l0 = x->launches;
+  int64_t nl0[N_CLASS];
+  memcpy(nl0, x->nl, sizeof(nl0));
+  x->k_hint = x->d.max_k;
+  cudaGraph_t g = nullptr;
+  int rc = CTAUX_OK;
+  cudaError_t e = cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal);
+  if (e == cudaSuccess) {
+    for (int i = 0; i < steps && rc == CTAUX_OK; ++i) rc = enqueue_block_step(x);
+    e = cudaStreamEndCapture(s, &g);
+  }
+  x->k_hint = saved_hint;
+  x->graph_launches = x->launches - l0;          // what one launch of the graph issues; the capture itself ran nothing
+  for (int c = 0; c < N_CLASS; ++c) x->graph_nl[c] = x->nl[c] - nl0[c];
+  x->launches = l0;
+  memcpy(x->nl, nl0, sizeof(nl0));
+  if (rc == CTAUX_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&x->graph_exec, g, 0);
+  if (g) cudaGraphDestroy(g);
+  if (rc != CTAUX_OK || e != cudaSuccess || !x->graph_exec) {
+    x->graph_exec = nullptr;
+    x->use_graph = false;
+    cudaGetLastError();
+  }
+  return CTAUX_OK;
+}
+
 int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps, int n_props = 0) {
   const DevCtx& d = x->d;
   cudaStream_t s = x->stream;
@@ -751,9 +789,18 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps, int n_props = 0) {
   const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + n_props + steps_per_poll;
   for (long long done = 0;; done += steps_per_poll) {
     if (done > max_steps) return CTAUX_ESTATE;
-    for (int i = 0; i < steps_per_poll; ++i) {
-      int rc = enqueue_block_step(x);
-      if (rc) return rc;
+    const bool graph_mode = x->use_graph && !x->timing;
+    if (graph_mode && x->graph_warm && !x->graph_exec) capture_poll_graph(x, steps_per_poll);
+    if (graph_mode && x->graph_exec) {
+      CU_CHECK(cudaGraphLaunch(x->graph_exec, s));
+      x->launches += x->graph_launches;
+      for (int c = 0; c < N_CLASS; ++c) x->nl[c] += x->graph_nl[c];
+    } else {
+      for (int i = 0; i < steps_per_poll; ++i) {
+        int rc = enqueue_block_step(x);
+        if (rc) return rc;
+      }
+      x->graph_warm = true;      // every kernel of a block step has been launched once: its shared-memory opt-in is done
     }
     x->n_fresh = false;
     // every 32 block steps at large k (two passes over N per check), every 8 where the matrices are small
@@ -1007,6 +1054,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (optin_acc.ensure(k_accumulate, x->acc_smem) != cudaSuccess) { free_pinned(x); delete x; return CTAUX_ECUDA; }
   }
   x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
+  x->use_graph = d.max_k <= 512 && getenv("CTAUX_NO_GRAPH") == nullptr;      // (the environment switch exists for A/B measurements)
   if (d.max_k > 512) {
     const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
     // panel width 32 inside outer blocks of 128 (rebuild_lu.cuh); a 64-wide panel was measured at the same total time
@@ -1051,6 +1099,7 @@ void ctaux_destroy(ctaux_ctx* x) {
   if (!x) return;
   cudaStreamSynchronize(x->stream);
   for (cudaEvent_t e : x->ev_pool) cudaEventDestroy(e);
+  if (x->graph_exec) cudaGraphExecDestroy(x->graph_exec);
   if (x->hi) { cudaStreamSynchronize(x->hi); cudaStreamDestroy(x->hi); cudaEventDestroy(x->ev_fork); cudaEventDestroy(x->ev_join); }
   free_pinned(x);
   delete x;
