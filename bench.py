@@ -300,7 +300,7 @@ def run_gpu(args):
     fp64_dmma = probe_fp64(0) if rank == 0 else 0.0
     W = WalkerGroups(G, B, lambda g, nb, stream: Walkers.from_config(
         cfg, table, n_walkers=nb, delay=delay, rebuild_every=S, device=dev, cand_window=args.cand_window, stream=stream,
-        rebuild_mode=args.rebuild_mode, flip_moves=args.flips))
+        rebuild_mode=args.rebuild_mode, flip_moves=args.flips, graph_mode=args.graph))
     W.reset(seeds)
     stream = torch.cuda.current_stream()
 
@@ -403,7 +403,7 @@ def run_gpu(args):
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                "config": {"workload": cfg["name"], "cluster": f"{cfg['Lx']}x{cfg['Ly']}", "beta": cfg["beta"], "U": cfg["U"],
                           "K": cfg["K"], "walkers_per_gpu": B, "stream_groups": G, "delay": delay, "sweeps_per_step": S,
-                          "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh",
+                          "rebuild_every": S, "rebuild_mode": "lu" if args.rebuild_mode == 0 else "newton-schulz refresh", "graph_mode": args.graph,
                           "moves": "insert/remove/flip" if args.flips else "insert/remove", "l2": "inputs larger than L2" if B * 4 * (s1["k_mean"] ** 2) * 8 > 126e6 else
                           "working set fits L2 (latency-bound chain; no flush between steps)",
                           "parallelism": "replicas only"},
@@ -458,6 +458,8 @@ def main():
     ap.add_argument("--groups", type=int, default=0, help="stream groups the walkers are split over (0 = per-config default)")
     ap.add_argument("--rebuild-mode", type=int, default=0, choices=[0, 1],
                     help="periodic rebuild: 0 = from-scratch LU (default, BASELINE.json), 1 = Newton-Schulz refresh (two GEMMs)")
+    ap.add_argument("--graph", type=int, default=0, choices=[-1, 0, 1],
+                    help="ctaux_params.graph_mode: CUDA graph per poll interval of block steps; 0 = library default (on for max_k <= 512), 1 = every size, -1 = off")
     ap.add_argument("--flips", type=int, default=0, choices=[0, 1],
                     help="1: auxiliary-spin flip as a third move (SURVEY NEXT-1; a different chain than BASELINE.json's)")
     ap.add_argument("--cand-window", type=int, default=0, help="insertion candidates pre-expanded per block")

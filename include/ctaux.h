@@ -125,6 +125,10 @@ typedef struct ctaux_params {
   int32_t nfft_oversampling;/* m of Eq. (31): the tau grid has m * N_w points.  0 = library default 4; >= 2. */
   int32_t nfft_window;     /* half-width w of the convolution kernel in grid cells (every sample touches 2w grid points,
                               2w <= 32).  0 = library default 6 (aliasing error ~2e-5 with m = 4; m = 8, w = 10: < 1e-9).   */
+  int32_t graph_mode;      /* CUDA graph of one poll interval of block steps (8 block steps, ~100 launches, incl. the fork to
+                              and join from the internal S3 stream), captured per context and grid size class and relaunched:
+                              0 = library default (on where a block step is launch bound: max_k <= 512), 1 = on for every
+                              size, -1 = off.  Never changes results; off while ctaux_timing_enable is on.                   */
 } ctaux_params;
 
 /* Per-walker counters.  flops are ALGORITHMIC (unpadded) counts of the GEMM steps. */

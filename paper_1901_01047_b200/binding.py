@@ -28,7 +28,7 @@ class _Params(C.Structure):
                 ("cand_window", C.c_int32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("stream", C.c_void_p), ("guard_amp", C.c_double), ("fused_small", C.c_int32), ("rebuild_mode", C.c_int32), ("flip_moves", C.c_int32),
                 ("n_tol", C.c_double), ("n_pairs", C.c_int32), ("pair_a", C.c_void_p), ("pair_b", C.c_void_p),
-                ("pair_U", C.c_void_p), ("n_omega", C.c_int32), ("nfft_oversampling", C.c_int32), ("nfft_window", C.c_int32)]
+                ("pair_U", C.c_void_p), ("n_omega", C.c_int32), ("nfft_oversampling", C.c_int32), ("nfft_window", C.c_int32), ("graph_mode", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -126,7 +126,7 @@ class Walkers:
     def __init__(self, Lx, Ly, beta, U, K, g0_table, delay, n_walkers, init_k, max_k,
                  rebuild_every=10, log_capacity=0, cand_window=0, device="cuda:0", stream=None,
                  guard_amp=0.0, fused_small=0, rebuild_mode=0, flip_moves=0, n_tol=0.0, n_omega=0, nfft_oversampling=0,
-                 nfft_window=0, pairs=None):
+                 nfft_window=0, pairs=None, graph_mode=0):
         import torch
         if not torch.cuda.is_available():
             raise CtauxError(-3, "ctaux_create", "no CUDA device: this package has no CPU fallback")
@@ -156,6 +156,7 @@ class Walkers:
             self._pairs = (pa, pb, pu)
             p.n_pairs, p.pair_a, p.pair_b, p.pair_U = pa.size, pa.ctypes.data, pb.ctypes.data, pu.ctypes.data
         p.n_omega, p.nfft_oversampling, p.nfft_window = n_omega, nfft_oversampling, nfft_window
+        p.graph_mode = graph_mode
         self.n_omega, self.Nc = n_omega, Lx * Ly
         nbytes = self._L.ctaux_workspace_bytes(C.byref(p))
         if nbytes == 0:

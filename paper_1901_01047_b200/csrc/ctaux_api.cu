@@ -7,9 +7,9 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
-#include <stdlib.h>
 #include <string.h>
 
+#include <map>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -273,7 +273,7 @@ struct ctaux_ctx {
   // CUDA graph of one poll interval (steps_per_poll block steps) for the launch-bound sizes (max_k <= 512: a block step
   // is ~13 launches of a few us each; config 3 spent more host time launching than the GPU spent computing)
   bool use_graph = false, graph_warm = false;
-  cudaGraphExec_t graph_exec = nullptr;
+  std::map<int, cudaGraphExec_t> graphs;      // keyed by the grid size the graph was captured for (kh of enqueue_block_step)
   int64_t graph_launches = 0, graph_nl[N_CLASS] = {};
   int k_hint;         // largest live expansion order seen at the last poll / rebuild: sizes the grids (the
                       // kernels stride over their tiles, so a stale hint costs balance, never correctness)
@@ -721,17 +721,19 @@ int enqueue_block_step(ctaux_ctx* x) {
   return CTAUX_OK;
 }
 
-// Capture `steps` block steps (launches on the context stream and on the forked S3 stream) into an executable graph.
-// Grids are sized for the capacity (the kernels read the live sizes on the device and stride / exit early), so one graph
-// serves every live size.  A failed capture switches the graph path off for this context; it is never an error.
-int capture_poll_graph(ctaux_ctx* x, int steps) {
+// Capture `steps` block steps (launches on the context stream and on the forked S3 stream) into an executable graph whose
+// grids cover live orders up to `kh` (the kernels read the live sizes on the device and stride / exit early, so a graph
+// captured for a larger size is always valid).  A failed capture switches the graph path off for this context; it is
+// never an error.
+cudaGraphExec_t capture_poll_graph(ctaux_ctx* x, int steps, int kh) {
   cudaStream_t s = x->stream;
   const int saved_hint = x->k_hint;
   const int64_t l0 = x->launches;
   int64_t nl0[N_CLASS];
   memcpy(nl0, x->nl, sizeof(nl0));
-  x->k_hint = x->d.max_k;
+  x->k_hint = kh - x->d.delay;                  // enqueue_block_step sizes its grids for min(k_hint + delay, max_k)
   cudaGraph_t g = nullptr;
+  cudaGraphExec_t exec = nullptr;
   int rc = CTAUX_OK;
   cudaError_t e = cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal);
   if (e == cudaSuccess) {
@@ -743,14 +745,14 @@ int capture_poll_graph(ctaux_ctx* x, int steps) {
   for (int c = 0; c < N_CLASS; ++c) x->graph_nl[c] = x->nl[c] - nl0[c];
   x->launches = l0;
   memcpy(x->nl, nl0, sizeof(nl0));
-  if (rc == CTAUX_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&x->graph_exec, g, 0);
+  if (rc == CTAUX_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&exec, g, 0);
   if (g) cudaGraphDestroy(g);
-  if (rc != CTAUX_OK || e != cudaSuccess || !x->graph_exec) {
-    x->graph_exec = nullptr;
+  if (rc != CTAUX_OK || e != cudaSuccess || !exec) {
+    exec = nullptr;
     x->use_graph = false;
     cudaGetLastError();
   }
-  return CTAUX_OK;
+  return exec;
 }
 
 int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps, int n_props = 0) {
@@ -789,10 +791,17 @@ int run_sweeps_chunk(ctaux_ctx* x, int n_sweeps, int n_props = 0) {
   const long long max_steps = (long long)n_sweeps * (d.max_k > 16 ? d.max_k : 16) + n_props + steps_per_poll;
   for (long long done = 0;; done += steps_per_poll) {
     if (done > max_steps) return CTAUX_ESTATE;
-    const bool graph_mode = x->use_graph && !x->timing;
-    if (graph_mode && x->graph_warm && !x->graph_exec) capture_poll_graph(x, steps_per_poll);
-    if (graph_mode && x->graph_exec) {
-      CU_CHECK(cudaGraphLaunch(x->graph_exec, s));
+    // graph path: one graph per grid size class (the live order rounded up to a multiple of 128, or the capacity)
+    cudaGraphExec_t gexec = nullptr;
+    if (x->use_graph && !x->timing && x->graph_warm) {
+      int khq = (x->k_hint + d.delay + 127) / 128 * 128;
+      if (khq > d.max_k || d.max_k <= 512) khq = d.max_k;
+      auto it = x->graphs.find(khq);
+      if (it != x->graphs.end()) gexec = it->second;
+      else if ((gexec = capture_poll_graph(x, steps_per_poll, khq)) != nullptr) x->graphs[khq] = gexec;
+    }
+    if (gexec) {
+      CU_CHECK(cudaGraphLaunch(gexec, s));
       x->launches += x->graph_launches;
       for (int c = 0; c < N_CLASS; ++c) x->nl[c] += x->graph_nl[c];
     } else {
@@ -1054,7 +1063,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (optin_acc.ensure(k_accumulate, x->acc_smem) != cudaSuccess) { free_pinned(x); delete x; return CTAUX_ECUDA; }
   }
   x->lu_cluster = false; x->lu_cluster_smem = 0; x->lu_nb = kLuNb;
-  x->use_graph = d.max_k <= 512 && getenv("CTAUX_NO_GRAPH") == nullptr;      // (the environment switch exists for A/B measurements)
+  x->use_graph = prm->graph_mode > 0 || (prm->graph_mode == 0 && d.max_k <= 512);
   if (d.max_k > 512) {
     const int rl_cap = (d.cap + kLuCl - 1) / kLuCl;
     // panel width 32 inside outer blocks of 128 (rebuild_lu.cuh); a 64-wide panel was measured at the same total time
@@ -1099,7 +1108,7 @@ void ctaux_destroy(ctaux_ctx* x) {
   if (!x) return;
   cudaStreamSynchronize(x->stream);
   for (cudaEvent_t e : x->ev_pool) cudaEventDestroy(e);
-  if (x->graph_exec) cudaGraphExecDestroy(x->graph_exec);
+  for (auto& kv : x->graphs) cudaGraphExecDestroy(kv.second);
   if (x->hi) { cudaStreamSynchronize(x->hi); cudaStreamDestroy(x->hi); cudaEventDestroy(x->ev_fork); cudaEventDestroy(x->ev_join); }
   free_pinned(x);
   delete x;

@@ -44,7 +44,7 @@ def test_ctypes_structs_match_the_header():
 #include "ctaux.h"
 int main(void) {
   printf("%zu %zu %zu %zu %zu %zu\n", sizeof(ctaux_params), sizeof(ctaux_stats), sizeof(ctaux_log_entry),
-         offsetof(ctaux_params, workspace), offsetof(ctaux_params, nfft_window), offsetof(ctaux_stats, flops_cand_alg));
+         offsetof(ctaux_params, workspace), offsetof(ctaux_params, graph_mode), offsetof(ctaux_stats, flops_cand_alg));
   return 0;
 }'''
     with tempfile.TemporaryDirectory() as td:
@@ -58,7 +58,7 @@ int main(void) {
     assert C.sizeof(binding._Stats) == ss
     assert binding.LOG_DTYPE.itemsize == sl == 48
     assert binding._Params.workspace.offset == ow
-    assert binding._Params.nfft_window.offset == of
+    assert binding._Params.graph_mode.offset == of
     assert binding._Stats.flops_cand_alg.offset == og
 
 
