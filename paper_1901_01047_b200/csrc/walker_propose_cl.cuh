@@ -26,12 +26,13 @@ __host__ __device__ inline ProposeClSmem propose_cl_smem_layout(int cap, int del
   ProposeClSmem L;
   int o = 0;
   const int lds = delay | 1;
-  L.sinv = o; o += sinv_smem ? lds * delay * 8 : 0;
-  L.scol = o; o += delay * 8;
-  L.srow = o; o += delay * 8;
-  L.tv = o; o += delay * 8;
-  L.tpv = o; o += delay * 8;
-  L.jiem = o; o += delay * 8;
+  const int dv = (delay + 1) & ~1;        // the vectors start on 16-byte boundaries (16-byte loads in the two products)
+  L.sinv = o; o += sinv_smem ? ((lds * delay * 8 + 15) & ~15) : 0;
+  L.scol = o; o += dv * 8;
+  L.srow = o; o += dv * 8;
+  L.tv = o; o += dv * 8;
+  L.tpv = o; o += dv * 8;
+  L.jiem = o; o += dv * 8;
   L.red = o; o += 2 * 16 * 8;
   L.snn = o; o += 2 * 8;
   o = (o + 15) & ~15;                 // st.async.v2.f64 wants 16-byte aligned slots
@@ -244,16 +245,45 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kClThreads, 1) k_pro
       __syncthreads();
       double part = 0.0, apart = 0.0;
       for (int a = row4; a < r; a += 64) {
+        // lane q4 of a row takes the entries b = 16 i + 4 q4 + (0..3): with the odd leading dimension of S^-1 the 16 lanes
+        // of a half-warp (4 rows x 4 lanes) then hit 16 different 8-byte banks for every one of the four loads (the
+        // interleaved assignment b = 4 i + q4 put (row a, lane q) and (row a + 1, lane q - 1) on the same bank: the two
+        // products were a third of the kernel's warp-state samples, MIO throttle and shared-memory scoreboard), and
+        // the vector operand arrives as two 16-byte broadcast loads
         double s0 = 0.0, s1 = 0.0;
-        int b = q4;
-        if (role == 0) {
+        if (!sinv_smem) {      // S^-1 in L2: the interleaved assignment keeps the four lanes of a row on one 32-byte sector
+          int b = q4;
+          if (role == 0) {
+            const double* Sa = Sv + a;
+            for (; b + 4 < r; b += 8) { s0 += Sa[(size_t)b * lds] * scol[b]; s1 += Sa[(size_t)(b + 4) * lds] * scol[b + 4]; }
+            if (b < r) s0 += Sa[(size_t)b * lds] * scol[b];
+          } else {
+            const double* Sa = Sv + (size_t)a * lds;
+            for (; b + 4 < r; b += 8) { s0 += srow[b] * Sa[b]; s1 += srow[b + 4] * Sa[b + 4]; }
+            if (b < r) s0 += srow[b] * Sa[b];
+          }
+        } else if (role == 0) {
           const double* Sa = Sv + a;
-          for (; b + 4 < r; b += 8) { s0 += Sa[(size_t)b * lds] * scol[b]; s1 += Sa[(size_t)(b + 4) * lds] * scol[b + 4]; }
-          if (b < r) s0 += Sa[(size_t)b * lds] * scol[b];
+          for (int b0 = 4 * q4; b0 < r; b0 += 16) {
+            if (b0 + 3 < r) {
+              const double2 v01 = *reinterpret_cast<const double2*>(scol + b0), v23 = *reinterpret_cast<const double2*>(scol + b0 + 2);
+              s0 += Sa[(size_t)b0 * lds] * v01.x;       s1 += Sa[(size_t)(b0 + 1) * lds] * v01.y;
+              s0 += Sa[(size_t)(b0 + 2) * lds] * v23.x; s1 += Sa[(size_t)(b0 + 3) * lds] * v23.y;
+            } else {
+              for (int b = b0; b < r; ++b) s0 += Sa[(size_t)b * lds] * scol[b];
+            }
+          }
         } else {
           const double* Sa = Sv + (size_t)a * lds;
-          for (; b + 4 < r; b += 8) { s0 += srow[b] * Sa[b]; s1 += srow[b + 4] * Sa[b + 4]; }
-          if (b < r) s0 += srow[b] * Sa[b];
+          for (int b0 = 4 * q4; b0 < r; b0 += 16) {
+            if (b0 + 3 < r) {
+              const double2 v01 = *reinterpret_cast<const double2*>(srow + b0), v23 = *reinterpret_cast<const double2*>(srow + b0 + 2);
+              s0 += v01.x * Sa[b0];     s1 += v01.y * Sa[b0 + 1];
+              s0 += v23.x * Sa[b0 + 2]; s1 += v23.y * Sa[b0 + 3];
+            } else {
+              for (int b = b0; b < r; ++b) s0 += srow[b] * Sa[b];
+            }
+          }
         }
         double t = s0 + s1;
         t += __shfl_xor_sync(quad_mask, t, 1);
