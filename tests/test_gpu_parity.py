@@ -264,6 +264,42 @@ def test_config4_thermalised_start_cluster_kernel(delay):
     assert max(W.get_stats(w)["sum_rank"] / max(W.get_stats(w)["flushes"], 1) for w in range(2)) > 0.5 * delay
 
 
+@pytest.mark.parametrize("ci,modes,nw,sweeps", [(2, (0, -1), 4, 6), (3, (1, -1), 2, 12)])
+def test_cuda_graph_path_runs_the_same_chain(ci, modes, nw, sweeps):
+    """ctaux_params.graph_mode: a poll interval of block steps relaunched as a CUDA graph (default for max_k <= 512, on
+    request for every size) against plain launches, device against device; the large configuration starts EMPTY, so that
+    its live order crosses several of the grid size classes a graph is captured for.
+    Same kernels, same arithmetic per tile: decisions, configurations and counters identical; on the large configuration
+    the split-K factor of the S2 products follows the grid size, so logged ratios and N agree to rounding only."""
+    pkg = _pkg()
+    cfg = get_config(ci)
+    table = table_for(cfg)
+    seeds = walker_seeds(nw, first=21)
+    runs = []
+    for mode in modes:
+        W = pkg.Walkers.from_config(cfg, table, n_walkers=nw, init_k=0 if ci == 3 else cfg["init_k"], graph_mode=mode, fused_small=-1,
+                                    log_capacity=sweeps * cfg["max_k"], rebuild_every=3)
+        W.reset(seeds)
+        W.sweep(2)
+        W.sweep(sweeps - 2)
+        runs.append(W)
+    A, B = runs
+    for w in range(nw):
+        what = f"{cfg['name']} graph_mode {modes[0]} vs {modes[1]}, walker {w}"
+        compare_logs(A.get_log(w), B.get_log(w), what)
+        compare_configs(A.get_config(w), B.get_config(w), what)
+        sa, sb = A.get_stats(w), B.get_stats(w)
+        for f in ("k", "proposals", "next_id", "sign", "acc_ins", "acc_rem", "sweeps", "blocks", "flushes"):
+            assert sa[f] == sb[f], (what, f)
+        assert sa["k"] > 150      # (the large configuration has crossed at least two grid size classes of 128 by then)
+        for sp in range(2):
+            Na, Nb = A.get_N(w, sp), B.get_N(w, sp)
+            assert np.linalg.norm(Na - Nb) <= 1e-10 * np.linalg.norm(Nb), what
+    if ci == 2:      # same grids, same split: the graph path counts exactly what it launches
+        assert A._L.ctaux_launch_count(A._h) == B._L.ctaux_launch_count(B._h)
+    A.close(); B.close()
+
+
 def test_error_codes_through_the_abi():
     """Calls that are not valid fail with their CTAUX_E* code and leave the process alive."""
     pkg = _pkg()
