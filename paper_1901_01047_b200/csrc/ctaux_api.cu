@@ -985,9 +985,14 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     if (!x->sinv_smem) Ls = propose_smem_layout(d.cap, d.delay, d.winmax, false);
     x->propose_smem = Ls.total;
     if (Ls.total > max_smem) { free_pinned(x); delete x; return CTAUX_ECAPACITY; }
+    // The serial S3 kernel asks for ALL the shared memory of an SM, so that no GEMM CTA of another stream group is
+    // co-resident with it: sharing an SM with three DMMA-bound CTAs slowed the latency-bound chain by 58 % (config 4,
+    // four groups: S3 331 ms per step instead of 209 alone; with the SM to itself 233, and the whole step 174 -> 160 ms),
+    // which costs the GEMMs B of the 148 SMs while S3 runs.  Only when every walker's CTA still gets an SM at once.
+    if (d.B <= sm_count()) x->propose_smem = max_smem;
     static SmemOptIn optin[4];   // the attribute is per function and device, shared by all contexts
-    if (x->sinv_smem) { e = optin[1].ensure(k_propose<true, true>, Ls.total); if (e == cudaSuccess) e = optin[2].ensure(k_propose<true, false>, Ls.total); }
-    else { e = optin[0].ensure(k_propose<false, true>, Ls.total); if (e == cudaSuccess) e = optin[3].ensure(k_propose<false, false>, Ls.total); }
+    if (x->sinv_smem) { e = optin[1].ensure(k_propose<true, true>, x->propose_smem); if (e == cudaSuccess) e = optin[2].ensure(k_propose<true, false>, x->propose_smem); }
+    else { e = optin[0].ensure(k_propose<false, true>, x->propose_smem); if (e == cudaSuccess) e = optin[3].ensure(k_propose<false, false>, x->propose_smem); }
   }
   if (e != cudaSuccess) {
     g_last_cuda_error = std::string("ctaux_create: ") + cudaGetErrorString(e);
