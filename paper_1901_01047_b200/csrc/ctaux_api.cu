@@ -214,6 +214,28 @@ cudaError_t launch_tma(const Fn& fn, int tiles_x, int problems, cudaStream_t s) 
   kern<<<dim3(tiles_x, problems), kTmaThreads, Cfg::SMEM_BYTES, s>>>(fn);
   return cudaGetLastError();
 }
+// launch with an execution priority of its own on whatever stream (cudaLaunchAttributePriority): the small kernels of a
+// block step jump the queue of GEMM CTAs the other stream groups have pending, without a second stream and its events
+template <class... KArgs, class... Args>
+cudaError_t launch_prio(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, int prio, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributePriority;
+  at[0].val.priority = prio;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+template <bool B_KMAJOR, int MINB, class Fn>
+cudaError_t launch_tma_prio(const Fn& fn, int tiles_x, int problems, cudaStream_t s, int prio) {
+  if (tiles_x < 1) tiles_x = 1;
+  using Cfg = TmaCfg<kTmaStages>;
+  auto kern = gemm_tma_kernel<kTmaStages, B_KMAJOR, MINB, Fn>;
+  static SmemOptIn optin;
+  cudaError_t e = optin.ensure(kern, Cfg::SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  return launch_prio(kern, dim3(tiles_x, problems), dim3(kTmaThreads), (size_t)Cfg::SMEM_BYTES, s, prio, fn);
+}
 struct TmaDescPlain {  // ctaux_dgemm
   TmaGemmDesc d;
   __device__ bool operator()(int, TmaGemmDesc& o) const { o = d; return true; }
@@ -246,6 +268,7 @@ struct ctaux_ctx {
                       // with events): when several contexts share the GPU its few CTAs must not queue behind
                       // thousands of GEMM CTAs of the other contexts
   cudaEvent_t ev_fork, ev_join;
+  int prio_hi = 0;    // numerically the highest stream priority of the device (0 when priorities are not available)
   bool lu_cluster;    // S5 panel factorisation on an 8-CTA cluster per matrix (large k)
   int lu_cluster_smem;
   int lu_nb;          // panel width: 64 with the cluster panel when its slabs fit shared memory, else 32
@@ -641,8 +664,8 @@ int enqueue_block_step(ctaux_ctx* x) {
   const int kcap = kh + d.mmax;
   {
     Scoped t(x, C_PREP);
-    k_prep_window<<<d.B, 1024, 0, s>>>(d);
-    k_prep_fill<<<dim3(grid_for((size_t)kcap * d.mmax, 256, 256), d.B), 256, 0, s>>>(d);
+    CU_CHECK(launch_prio(k_prep_window, dim3(d.B), dim3(1024), 0, s, x->prio_hi, d));
+    CU_CHECK(launch_prio(k_prep_fill, dim3(grid_for((size_t)kcap * d.mmax, 256, 256), d.B), dim3(256), 0, s, x->prio_hi, d));
     tick(x, C_PREP); tick(x, C_PREP);
   }
   {
@@ -657,10 +680,10 @@ int enqueue_block_step(ctaux_ctx* x) {
     CU_CHECK((launch_tma<true, 4>(TDescCandRows{d, S}, t1, P * S, s)));
     tick(x, C_CAND_GEMM);
     const int rb = grid_for((size_t)kcap * d.mmax, 256, 128);
-    if (S > 1) { k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 0); tick(x, C_CAND_GEMM); }
+    if (S > 1) { CU_CHECK(launch_prio(k_splitk_reduce, dim3(rb, P), dim3(256), 0, s, x->prio_hi, d, S, 0)); tick(x, C_CAND_GEMM); }
     CU_CHECK((launch_tma<false, 4>(TDescCandCols{d, S}, t2, P * S, s)));
     tick(x, C_CAND_GEMM);
-    if (S > 1) { k_splitk_reduce<<<dim3(rb, P), 256, 0, s>>>(d, S, 1); tick(x, C_CAND_GEMM); }
+    if (S > 1) { CU_CHECK(launch_prio(k_splitk_reduce, dim3(rb, P), dim3(256), 0, s, x->prio_hi, d, S, 1)); tick(x, C_CAND_GEMM); }
   }
   {
     cudaStream_t ps = x->hi ? x->hi : s;
@@ -690,13 +713,13 @@ int enqueue_block_step(ctaux_ctx* x) {
   }
   {
     Scoped t(x, C_UV);
-    k_build_uv<<<dim3(grid_for((size_t)kh * d.delay, 256, 512), P), 256, 0, s>>>(d);
+    CU_CHECK(launch_prio(k_build_uv, dim3(grid_for((size_t)kh * d.delay, 256, 512), P), dim3(256), 0, s, x->prio_hi, d));
     tick(x, C_UV);
   }
   {
     Scoped t(x, C_USINV_GEMM);
     cudaError_t e3;
-    e3 = launch_tma<true, 4>(TDescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s);
+    e3 = launch_tma_prio<true, 4>(TDescUSinv{d}, (kh + 63) / 64 * ((d.delay + 63) / 64), P, s, x->prio_hi);
     CU_CHECK(e3);
     tick(x, C_USINV_GEMM);
   }
@@ -1098,6 +1121,7 @@ int ctaux_create(const ctaux_params* prm, ctaux_ctx** out) {
     int lo = 0, hi = 0;
     if (cudaDeviceGetStreamPriorityRange(&lo, &hi) == cudaSuccess && hi < lo &&
         cudaStreamCreateWithPriority(&x->hi, cudaStreamNonBlocking, hi) == cudaSuccess) {
+      x->prio_hi = hi;
       if (cudaEventCreateWithFlags(&x->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
           cudaEventCreateWithFlags(&x->ev_join, cudaEventDisableTiming) != cudaSuccess) {
         cudaStreamDestroy(x->hi);
