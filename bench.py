@@ -1,5 +1,5 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the B200-native CT-AUX walker hot path (contract: see DESIGN.md section 6).
+"""bench.py -- throughput of the B200-native CT-AUX walker hot path (contract: see DESIGN.md section 10).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4_6x6_b20] [--sweeps-per-step S]
   python bench.py --impl reference ...     # the CPU oracle, as it stands, on the host cores
