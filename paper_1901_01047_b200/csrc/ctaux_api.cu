@@ -671,9 +671,11 @@ int enqueue_block_step(ctaux_ctx* x) {
   {
     Scoped t(x, C_CAND_GEMM);
     const int t1 = (d.mmax + 63) / 64 * ((kh + 63) / 64), t2 = (kcap + 63) / 64 * ((d.mmax + 63) / 64);
-    // split-K factor of the skinny S2 products: aim at >= 3 waves of the 148 x 4 CTA slots (measured optimum; a
-    // wave-count model was tried and lost 4 %), chunks of at least 128
-    int S = (12 * sm_count() + P * t1 - 1) / (P * t1);
+    // split-K factor of the skinny S2 products: enough CTAs for one wave of the 148 x 4 slots, and K chunks of about 360
+    // (measured inside the run, where the other stream groups fill the tails: config 4 wants 6 slices of 300, config 5
+    // 8 slices of 460; the earlier rule, three waves per launch, gave 8 everywhere and cost config 4 2 %)
+    int S = (4 * sm_count() + P * t1 - 1) / (P * t1);
+    if (S < (kh + 359) / 360) S = (kh + 359) / 360;
     if (S > kMaxSplitK) S = kMaxSplitK;
     while (S > 1 && kh / S < 128) --S;
     if (d.max_k <= 512) S = 1;   // the split-K scratch exists only for the large configurations
